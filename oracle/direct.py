@@ -1,0 +1,163 @@
+"""Oracle A: direct non-uniform Fourier sums, O(N*K), no grid (float64).
+
+TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).
+
+Definition (Eq. (5)-(6)), per channel a with exponent p:
+
+    rho_a(k) = sum_j q_j^a e^{i k.r_j},                    k = 2 pi (m_x/L_x, m_y/L_y, m_z/L_z)
+    E        = 1/(2V) sum_a [ sum_{k in K} Phi^_p(k) |rho_a(k)|^2 + Phi0_p (Q_net^a)^2 ]
+    phi_i^a  = dE/dq_i^a = (1/V) [ sum_K Phi^_p(k) Re(e^{-i k.r_i} rho_a(k)) + Phi0_p Q_net^a ]
+    F_i      = -dE/dr_i (q fixed)
+             = -(1/V) sum_a q_i^a sum_K Phi^_p(k) k Im(e^{-i k.r_i} rho_a(k))
+               (d|rho|^2/dr_i = 2 Re(conj(rho) i k q_i e^{ik.r_i}) = 2 q_i k Im(e^{-ik.r_i} rho))
+
+Mode set K (reading R-modes): all m != 0 with |k| r_c < c (Phi^_p == 0 beyond,
+PAPER.md:836) and, when a grid is given, |m_d| < M_d/2 (modes the grid can carry).
+No self term and no real-space term: this is the reciprocal part of (S65) only.
+"""
+import ctypes
+import os
+import subprocess
+import numpy as np
+from .kernels import Mollifier
+
+
+def mode_set(box, c, r_c, grid=None, half=False):
+    """Integer mode vectors m (K,3) of the set K above.  half=True keeps one of each
+    +-m pair (the first non-zero component positive)."""
+    box = np.asarray(box, dtype=np.float64)
+    kc = c / r_c
+    mmax = np.floor(kc * box / (2 * np.pi)).astype(int) + 1
+    if grid is not None:
+        # |m_d| < M_d/2  (strict: Nyquist planes excluded, reading R11)
+        lim = (np.asarray(grid) - 1) // 2
+        mmax = np.minimum(mmax, lim)
+    ax = [np.arange(-mm, mm + 1) for mm in mmax]
+    m = np.stack(np.meshgrid(*ax, indexing="ij"), axis=-1).reshape(-1, 3)
+    k = 2 * np.pi * m / box
+    kn = np.sqrt((k ** 2).sum(1))
+    keep = (kn * r_c < c) & np.any(m != 0, axis=1)
+    m = m[keep]
+    if half:
+        pos = (m[:, 0] > 0) | ((m[:, 0] == 0) & (m[:, 1] > 0)) | \
+              ((m[:, 0] == 0) & (m[:, 1] == 0) & (m[:, 2] > 0))
+        m = m[pos]
+    return m
+
+
+def direct_sums(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_mode=True,
+                chunk=2048):
+    """E (float), E_channels (C,), phi (C,n_sub), F (n_sub,3) by the sums above (numpy).
+
+    pos (N,3), q (C,N), exponents (C,), box (3,).  subset: indices of the atoms whose
+    phi/F are wanted (default all).  The sum runs over the FULL mode set (both +-k).
+    """
+    pos = np.asarray(pos, dtype=np.float64)
+    q = np.atleast_2d(np.asarray(q, dtype=np.float64))
+    box = np.asarray(box, dtype=np.float64)
+    C, N = q.shape
+    V = float(np.prod(box))
+    moll = Mollifier(c, r_c)
+    m = mode_set(box, c, r_c, grid, half=False)
+    k = 2 * np.pi * m / box                       # (K,3)
+    kn = np.sqrt((k ** 2).sum(1))
+    kn_u, inv = np.unique(kn, return_inverse=True)   # Phi^ depends on |k| only
+    idx = np.arange(N) if subset is None else np.asarray(subset)
+    # structure factors rho_a(k), Eq. (6)
+    rho = np.zeros((C, len(k)), dtype=np.complex128)
+    for s in range(0, N, chunk):
+        ph = np.exp(1j * pos[s:s + chunk] @ k.T)  # (n,K)
+        rho += q[:, s:s + chunk] @ ph
+    E_ch = np.zeros(C)
+    phi = np.zeros((C, len(idx)))
+    F = np.zeros((len(idx), 3))
+    for a, p in enumerate(exponents):
+        Ph = moll.Phi_hat(int(p), kn_u)[inv]      # (K,)
+        Qnet = q[a].sum()
+        E_ch[a] = (Ph * np.abs(rho[a]) ** 2).sum() / (2 * V)
+        if zero_mode:
+            E_ch[a] += moll.Phi0(int(p)) * Qnet ** 2 / (2 * V)
+        for s in range(0, len(idx), chunk):
+            ii = idx[s:s + chunk]
+            t = np.exp(-1j * pos[ii] @ k.T) * rho[a]          # e^{-ik.r_i} rho_a(k)
+            phi[a, s:s + chunk] = (t.real * Ph).sum(1) / V
+            F[s:s + chunk] -= q[a, ii, None] * ((t.imag * Ph) @ k) / V
+        if zero_mode:
+            phi[a] += moll.Phi0(int(p)) * Qnet / V
+    return float(E_ch.sum()), E_ch, phi, F
+
+
+# ---------------------------------------------------------------------------------
+# The same sums in plain C (oracle/direct_sum.c) for the large configurations.
+# ---------------------------------------------------------------------------------
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+
+def build_c(force=False):
+    """Compile oracle/direct_sum.c -> oracle/liboracle_direct.so (gcc -O2 -fopenmp)."""
+    src = os.path.join(_HERE, "direct_sum.c")
+    out = os.path.join(_HERE, "liboracle_direct.so")
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c11",
+                               "-o", out, src, "-lm"])
+    return out
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        _LIB = ctypes.CDLL(build_c())
+        _LIB.oracle_direct_sums.restype = ctypes.c_int
+        _LIB.oracle_threads.restype = ctypes.c_int
+    return _LIB
+
+
+def c_threads():
+    return int(_lib().oracle_threads())
+
+
+def direct_sums_c(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_mode=True,
+                  rho_atoms=None):
+    """Same contract as direct_sums(), evaluated by oracle/direct_sum.c over the half mode
+    set (x2; rho(-k) = conj rho(k) and Phi^ is even, so the +-k terms of Eq. (5) are equal).
+    The mollifier values Phi^_p(|k|) per mode are computed here with kernels.py and passed in.
+
+    rho_atoms: optional int -- use only the first rho_atoms atoms in rho(k) (bench sampling).
+    """
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    q = np.ascontiguousarray(np.atleast_2d(q), dtype=np.float64)
+    box = np.ascontiguousarray(box, dtype=np.float64)
+    C, N = q.shape
+    if rho_atoms is not None:
+        N = int(rho_atoms)
+        pos = np.ascontiguousarray(pos[:N])
+        q = np.ascontiguousarray(q[:, :N])
+    moll = Mollifier(c, r_c)
+    m = np.ascontiguousarray(mode_set(box, c, r_c, grid, half=True), dtype=np.int32)
+    K = len(m)
+    kn = np.sqrt(((2 * np.pi * m / box) ** 2).sum(1))
+    kn_u, inv = np.unique(kn, return_inverse=True)   # Phi^ depends on |k| only
+    Ph = np.empty((C, K))
+    cache = {}
+    for a, p in enumerate(exponents):
+        if int(p) not in cache:
+            cache[int(p)] = moll.Phi_hat(int(p), kn_u)[inv]
+        Ph[a] = cache[int(p)]
+    Phi0 = np.array([moll.Phi0(int(p)) if zero_mode else 0.0 for p in exponents])
+    idx = np.ascontiguousarray(np.arange(N) if subset is None else subset, dtype=np.int64)
+    E_ch = np.zeros(C)
+    phi = np.zeros((C, len(idx)))
+    F = np.zeros((len(idx), 3))
+    dp = ctypes.POINTER(ctypes.c_double)
+
+    def P(a, t=dp):
+        return a.ctypes.data_as(t)
+    rc = _lib().oracle_direct_sums(
+        ctypes.c_long(N), P(pos), ctypes.c_int(C), P(q), P(box),
+        ctypes.c_long(K), P(m, ctypes.POINTER(ctypes.c_int32)), P(Ph), P(Phi0),
+        ctypes.c_long(len(idx)), P(idx, ctypes.POINTER(ctypes.c_int64)),
+        P(E_ch), P(phi), P(F))
+    if rc != 0:
+        raise RuntimeError("oracle_direct_sums failed: %d" % rc)
+    return float(E_ch.sum()), E_ch, phi, F

@@ -1,0 +1,92 @@
+"""Validation scaffold: the pieces of (S65) that are NOT on the hot path (float64).
+
+TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).  Never timed, never compared with the GPU.
+It exists so the oracle's reciprocal part can be pinned to physics the paper fixes: the total
+
+    E^(p) = E_real + (1/2V) sum_{k!=0} Phi^ |rho|^2 + E_0 - E_self        (S65)
+
+must equal the plain periodic inverse-power energy, independently of (c, r_c).
+"""
+import itertools
+import numpy as np
+from scipy.special import erfc
+from .kernels import Mollifier
+from .direct import direct_sums
+
+
+def real_space_complement(pos, q, p, box, moll):
+    """E_real = 1/2 sum_n sum_{i,j}' q_i q_j L_{p,r_c}(|r_ij + n.L|)   (S64)-(S65).
+    L_{p,r_c} vanishes beyond r_c, so only images within r_c are visited."""
+    pos = np.asarray(pos, dtype=np.float64)
+    q = np.asarray(q, dtype=np.float64)
+    box = np.asarray(box, dtype=np.float64)
+    nmax = np.ceil(moll.r_c / box).astype(int)
+    E = 0.0
+    d0 = pos[:, None, :] - pos[None, :, :]
+    qq = q[:, None] * q[None, :]
+    for n in itertools.product(*[range(-k, k + 1) for k in nmax]):
+        d = d0 + np.asarray(n) * box
+        r = np.sqrt((d ** 2).sum(-1))
+        mask = (r > 0) & (r < moll.r_c)
+        if n == (0, 0, 0):
+            mask &= ~np.eye(len(pos), dtype=bool)
+        E += 0.5 * np.sum(qq[mask] * moll.L_phys(p, r[mask]))
+    return float(E)
+
+
+def self_energy(q, p, moll):
+    """E_self = S_p(0) Q_self / (2 r_c^p)      (S66)."""
+    q = np.asarray(q, dtype=np.float64)
+    return float(moll.S_zero(p) * np.sum(q ** 2) / (2 * moll.r_c ** p))
+
+
+def total_energy(pos, q, p, box, c, r_c):
+    """Full decomposition (S65) for one channel; reciprocal part = oracle A without a grid."""
+    moll = Mollifier(c, r_c)
+    E_rec, _, _, _ = direct_sums(pos, q[None, :], [p], box, c, r_c, grid=None)
+    return real_space_complement(pos, q, p, box, moll) + E_rec - self_energy(q, p, moll)
+
+
+def ewald_erfc_energy(pos, q, box, alpha, r_cut, kmax):
+    """Classical Coulomb Ewald sum (Eq. (12) with p = 1: G = erfc(alpha r)), tinfoil
+    boundary, neutralising background for net charge.  Independent of every PSWF routine."""
+    pos = np.asarray(pos, dtype=np.float64)
+    q = np.asarray(q, dtype=np.float64)
+    box = np.asarray(box, dtype=np.float64)
+    V = float(np.prod(box))
+    nmax = np.ceil(r_cut / box).astype(int)
+    E = 0.0
+    d0 = pos[:, None, :] - pos[None, :, :]
+    qq = q[:, None] * q[None, :]
+    for n in itertools.product(*[range(-k, k + 1) for k in nmax]):
+        d = d0 + np.asarray(n) * box
+        r = np.sqrt((d ** 2).sum(-1))
+        mask = (r > 0) & (r < r_cut)
+        E += 0.5 * np.sum(qq[mask] * erfc(alpha * r[mask]) / r[mask])
+    ax = [np.arange(-kmax, kmax + 1)] * 3
+    m = np.stack(np.meshgrid(*ax, indexing="ij"), -1).reshape(-1, 3)
+    m = m[np.any(m != 0, axis=1)]
+    k = 2 * np.pi * m / box
+    k2 = (k ** 2).sum(1)
+    rho = (q[None, :] * np.exp(1j * k @ pos.T)).sum(1)
+    E += (2 * np.pi / V) * np.sum(np.exp(-k2 / (4 * alpha ** 2)) / k2 * np.abs(rho) ** 2)
+    E -= alpha / np.sqrt(np.pi) * np.sum(q ** 2)
+    E -= np.pi * q.sum() ** 2 / (2 * V * alpha ** 2)
+    return float(E)
+
+
+def brute_force_image_sum(pos, q, p, box, nmax):
+    """1/2 sum_{|n_d|<=nmax} sum_{i,j}' q_i q_j / |r_ij + n.L|^p  (absolutely convergent for p > 3)."""
+    pos = np.asarray(pos, dtype=np.float64)
+    q = np.asarray(q, dtype=np.float64)
+    box = np.asarray(box, dtype=np.float64)
+    d0 = pos[:, None, :] - pos[None, :, :]
+    qq = q[:, None] * q[None, :]
+    E = 0.0
+    rng = range(-nmax, nmax + 1)
+    for n in itertools.product(rng, rng, rng):
+        d = d0 + np.asarray(n) * box
+        r2 = (d ** 2).sum(-1)
+        mask = r2 > 0
+        E += 0.5 * np.sum(qq[mask] * r2[mask] ** (-p / 2.0))
+    return float(E)

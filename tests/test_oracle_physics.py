@@ -1,0 +1,197 @@
+"""Physics pins for oracle A (oracle/direct.py, oracle/direct_sum.c): the reciprocal sum, completed
+by the validation scaffold to the full decomposition (S65), must reproduce lattice energies the
+mathematics fixes, for every exponent, independently of (c, r_c)."""
+import itertools
+import numpy as np
+import pytest
+
+from oracle import scaffold
+from oracle.direct import direct_sums, direct_sums_c, mode_set
+from oracle.kernels import Mollifier
+
+
+def _rock_salt():
+    pos, q = [], []
+    for i, j, k in itertools.product(range(2), repeat=3):
+        pos.append([i, j, k])
+        q.append((-1.0) ** (i + j + k))
+    return np.array(pos, float), np.array(q), [2.0, 2.0, 2.0]
+
+
+@pytest.mark.parametrize("c,r_c", [(30.0, 1.3), (24.0, 1.7)])
+def test_madelung_nacl(golden, c, r_c):
+    """north_star pin: NaCl Madelung constant 1.747565 (p = 1), via (S65) with tinfoil E_IB = 0."""
+    pos, q, box = _rock_salt()
+    E = scaffold.total_energy(pos, q, 1, box, c, r_c)
+    M = -E / 4.0          # 8 ions, nearest-neighbour distance 1: E = -(8/2) M
+    assert abs(M - golden["madelung_nacl_northstar"]) < 5e-7
+    assert abs(M - golden["madelung_nacl"]) < 2e-9
+
+
+def _sc_sum_brute(p, R=24):
+    """sum_{0<|n|<=R} |n|^-p + 4 pi int_R^inf r^(2-p) dr, shell-corrected (independent of the oracle)."""
+    ax = np.arange(-R, R + 1)
+    n2 = (ax[:, None, None] ** 2 + ax[None, :, None] ** 2 + ax[None, None, :] ** 2).astype(float)
+    mask = (n2 > 0) & (n2 <= R * R)
+    tail = 4 * np.pi * R ** (3.0 - p) / (p - 3.0)
+    return float(np.sum(n2[mask] ** (-p / 2.0)) + tail)
+
+
+@pytest.mark.parametrize("p", [4, 5, 6])
+def test_simple_cubic_lattice_sums(golden, p):
+    """One unit 'charge' in a unit cube: 2E = sum_{n != 0} |n|^-p.  Exercises the non-neutral zero
+    mode (S79) and the self term (S66)-(S67)."""
+    ref = golden["sc_lattice_sum_p%d" % p]
+    # the golden value itself is checked by brute force (tolerance = its truncation error)
+    assert abs(_sc_sum_brute(p) - ref) < {4: 2e-2, 5: 3e-4, 6: 1e-5}[p]
+    E = scaffold.total_energy(np.zeros((1, 3)), np.ones(1), p, [1.0, 1.0, 1.0], 30.0, 0.9)
+    assert abs(2 * E - ref) < {4: 2e-9, 5: 1e-7, 6: 2e-9}[p] * ref   # p = 5 golden has 9 digits
+
+
+@pytest.mark.parametrize("p,nmax,tol", [(6, 6, 2e-6), (5, 8, 2e-4), (4, 10, 2e-3)])
+def test_brute_force_image_sums_random_box(p, nmax, tol):
+    """Random 6-atom non-neutral box, orthorhombic: (S65) vs 1/2 sum_n sum' q_i q_j / r^p (p > 3
+    converges absolutely; the remainder is bounded by the integral tail and corrected with it)."""
+    rng = np.random.default_rng(42 + p)
+    box = np.array([3.1, 2.7, 3.6])
+    pos = rng.uniform(0, 1, (6, 3)) * box
+    q = rng.normal(0, 1, 6)
+    E = scaffold.total_energy(pos, q, p, box, 24.0, 1.2)
+    brute = scaffold.brute_force_image_sum(pos, q, p, box, nmax)
+    # tail of the image sum beyond the summed block, continuum estimate
+    R = (nmax + 0.5) * box.min()
+    tail = 0.5 * q.sum() ** 2 * 4 * np.pi * R ** (3.0 - p) / ((p - 3.0) * np.prod(box))
+    assert abs(E - brute) < max(tol * abs(E), 3 * abs(tail)), (E, brute, tail)
+
+
+def test_p3_neutral_vs_brute_force():
+    """p = 3, neutral random box: spherical image sum converges like 1/R^2; Richardson-extrapolated
+    brute force against (S65).  (A charged p = 3 channel is pinned by invariance below.)"""
+    rng = np.random.default_rng(7)
+    box = np.array([2.0, 2.0, 2.0])
+    pos = rng.uniform(0, 2, (4, 3))
+    q = rng.normal(0, 1, 4)
+    q -= q.mean()
+    E = scaffold.total_energy(pos, q, 3, box, 24.0, 0.9)
+    b = [scaffold.brute_force_image_sum(pos, q, 3, box, n) for n in (6, 12)]
+    # cubic-block truncation of a neutral 1/r^3 sum: error ~ 1/n^2
+    extrap = (4 * b[1] - b[0]) / 3
+    assert abs(E - extrap) < 3e-4 * max(1.0, abs(E)), (E, b, extrap)
+
+
+@pytest.mark.parametrize("p", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("neutral", [True, False])
+def test_total_energy_independent_of_c_and_rc(p, neutral):
+    """'SR+LR split' pin for every exponent: (S65) must not depend on (c, r_c), including the
+    zero-mode conventions (S73), (S75), (S78) for charged channels."""
+    rng = np.random.default_rng(100 + p)
+    box = np.array([3.0, 3.4, 2.8])
+    pos = rng.uniform(0, 1, (5, 3)) * box
+    q = rng.normal(0, 1, 5)
+    if neutral:
+        q -= q.mean()
+    E1 = scaffold.total_energy(pos, q, p, box, 30.0, 1.1)
+    E2 = scaffold.total_energy(pos, q, p, box, 26.0, 1.35)
+    assert abs(E1 - E2) < 2e-9 * max(1.0, abs(E1)), (E1, E2)
+
+
+@pytest.mark.parametrize("neutral", [True, False])
+def test_p1_matches_classical_erfc_ewald(neutral):
+    """'short-range-plus-long-range split matches full Ewald' (north_star): p = 1 PSWF total vs the
+    classical erfc Ewald sum (Eq. (12) special case) on the same box."""
+    rng = np.random.default_rng(3)
+    box = np.array([3.0, 3.3, 2.9])
+    pos = rng.uniform(0, 1, (6, 3)) * box
+    q = rng.normal(0, 1, 6)
+    if neutral:
+        q -= q.mean()
+    E_pswf = scaffold.total_energy(pos, q, 1, box, 30.0, 1.2)
+    E_ewald = scaffold.ewald_erfc_energy(pos, q, box, alpha=2.6, r_cut=2.9, kmax=16)
+    assert abs(E_pswf - E_ewald) < 1e-8 * max(1.0, abs(E_ewald)), (E_pswf, E_ewald)
+
+
+# ---- derivatives and invariants of oracle A itself ------------------------------------------
+
+def _small_system(seed=5, N=9, C=3):
+    rng = np.random.default_rng(seed)
+    box = np.array([9.0, 10.0, 8.5])
+    pos = rng.uniform(0, 1, (N, 3)) * box
+    q = rng.normal(0, 0.7, (C, N))
+    q[0] -= q[0].mean()
+    return pos, q, box, [1, 3, 6]
+
+
+def test_forces_are_minus_gradient_fd():
+    pos, q, box, ex = _small_system()
+    c, r_c = 12.024, 3.0
+    E, _, phi, F = direct_sums(pos, q, ex, box, c, r_c)
+    h = 1e-5
+    for i in (0, 4):
+        for d in range(3):
+            pp, pm = pos.copy(), pos.copy()
+            pp[i, d] += h
+            pm[i, d] -= h
+            fd = -(direct_sums(pp, q, ex, box, c, r_c)[0] - direct_sums(pm, q, ex, box, c, r_c)[0]) / (2 * h)
+            assert abs(fd - F[i, d]) < 1e-7 * np.abs(F).max()
+
+
+def test_phi_is_dE_dq_fd():
+    pos, q, box, ex = _small_system()
+    c, r_c = 12.024, 3.0
+    E, _, phi, F = direct_sums(pos, q, ex, box, c, r_c)
+    h = 1e-6
+    for a, i in ((0, 1), (1, 3), (2, 8)):
+        qp, qm = q.copy(), q.copy()
+        qp[a, i] += h
+        qm[a, i] -= h
+        fd = (direct_sums(pos, qp, ex, box, c, r_c)[0] - direct_sums(pos, qm, ex, box, c, r_c)[0]) / (2 * h)
+        assert abs(fd - phi[a, i]) < 1e-8 * np.abs(phi).max()
+    assert abs(E - 0.5 * np.sum(q * phi)) < 1e-13 * abs(E)
+
+
+def test_net_force_zero_and_translation_invariance():
+    pos, q, box, ex = _small_system()
+    c, r_c = 12.024, 3.0
+    E, Ech, phi, F = direct_sums(pos, q, ex, box, c, r_c)
+    assert np.abs(F.sum(0)).max() < 1e-13 * np.abs(F).max()
+    shift = np.array([0.37, -1.21, 4.4])
+    E2, _, phi2, F2 = direct_sums(pos + shift, q, ex, box, c, r_c)
+    assert abs(E - E2) < 1e-13 * abs(E)
+    assert np.abs(F - F2).max() < 1e-12 * np.abs(F).max()
+    assert np.abs(phi - phi2).max() < 1e-12 * np.abs(phi).max()
+    # periodic images: moving one atom by a lattice vector changes nothing
+    pos3 = pos.copy()
+    pos3[2] += box * np.array([1, -2, 3])
+    assert abs(direct_sums(pos3, q, ex, box, c, r_c)[0] - E) < 1e-12 * abs(E)
+
+
+def test_c_oracle_equals_numpy_oracle_and_half_equals_full():
+    pos, q, box, ex = _small_system(seed=11, N=40, C=3)
+    c, r_c = 12.024, 2.5
+    grid = [16, 18, 14]
+    a = direct_sums(pos, q, ex, box, c, r_c, grid=grid)
+    b = direct_sums_c(pos, q, ex, box, c, r_c, grid=grid)
+    assert abs(a[0] - b[0]) < 1e-13 * abs(a[0])
+    assert np.allclose(a[1], b[1], rtol=1e-12)
+    assert np.allclose(a[2], b[2], rtol=0, atol=1e-13 * np.abs(a[2]).max())
+    assert np.allclose(a[3], b[3], rtol=0, atol=1e-13 * np.abs(a[3]).max())
+    sub = np.array([3, 17, 39])
+    bs = direct_sums_c(pos, q, ex, box, c, r_c, grid=grid, subset=sub)
+    assert np.allclose(bs[2], a[2][:, sub], rtol=0, atol=1e-13 * np.abs(a[2]).max())
+    assert np.allclose(bs[3], a[3][sub], rtol=0, atol=1e-13 * np.abs(a[3]).max())
+    full, half = mode_set(box, c, r_c, grid), mode_set(box, c, r_c, grid, half=True)
+    assert len(full) == 2 * len(half)
+    assert {tuple(v) for v in full} == {tuple(v) for v in half} | {tuple(-v) for v in half}
+
+
+def test_mode_set_limits():
+    box = np.array([10.0, 10.0, 10.0])
+    c, r_c = 12.024, 4.78
+    m = mode_set(box, c, r_c, grid=[16, 16, 16])
+    k = 2 * np.pi * m / box
+    assert np.all(np.sqrt((k ** 2).sum(1)) * r_c < c)
+    assert np.abs(m).max() <= 7
+    assert not np.any(np.all(m == 0, axis=1))
+    # |m| < c L / (2 pi r_c) = 4.0035: lattice points with 0 < |m|^2 <= 16 (Gauss sphere count
+    # 1+6+12+8+6+24+24+0+12+30+24+24+8+24+48+0+6 = 257 including the origin)
+    assert len(m) == 256
