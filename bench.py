@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the PSWF-LR reciprocal-space hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--cfg 4]
+
+A "step" is one pass of the whole hot path (bin/sort, spread, forward FFT, scale+reduce, inverse
+FFT, gather: energy + potentials + forces) over one synthetic system of BASELINE.json's
+configuration 4 (N = 1,000,000 atoms, 128^3 grid, w = 8, channels p = 1,1,3,6, fp32), positions
+advanced between steps by seeded displacements sigma = 0.01 A.  Metric: atom-steps/s (= atoms x
+evaluations per second); evals/s is reported beside it.
+
+N > 1 (launched by torch.distributed.run): every rank evaluates its own independent replica of the
+system (its own seed) -- no data-path collective; value = atoms of all ranks / max-over-ranks time
+("weak" scaling).
+
+--impl reference times the CPU oracle (oracle/direct_sum.c, as it stands) on this box's host cores
+on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "LR energy+force atom-steps/s at 1M atoms (evals/s x atoms)"
+UNIT = "atom-steps/s"
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def reduce_times(elapsed_s, units, backend_device=None):
+    """max over ranks of the elapsed time, sum over ranks of the units processed (host logic of the
+    N > 1 path; covered by a world_size-2 gloo test)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return elapsed_s, units
+    dev = backend_device if backend_device is not None else torch.device("cpu")
+    t = torch.tensor([elapsed_s], dtype=torch.float64, device=dev)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def rank_seed(cfg, rank):
+    """Replica seed of a rank: rank 0 keeps the configuration's own seed."""
+    return cfg if rank == 0 else 1000 * cfg + rank
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+def algorithmic_bytes(N, C, M, B=4):
+    """SURVEY.md §8(d) / DESIGN.md §6: bytes each stage must move per evaluation."""
+    Mtot = M[0] * M[1] * M[2]
+    Mhalf = M[0] * M[1] * (M[2] // 2 + 1)
+    atoms_in = N * (3 + C) * B
+    atoms_out = N * (3 + C) * B
+    return {
+        "bin_sort": atoms_in + 2 * N * 4 + atoms_in,          # read pos,q; keys+perm; sorted copy
+        "spread": atoms_in + C * Mtot * B,
+        "fft_forward": C * Mtot * B + C * Mhalf * 2 * B,
+        "scale_reduce": 2 * C * Mhalf * 2 * B,
+        "fft_inverse": C * Mtot * B + C * Mhalf * 2 * B,
+        "gather": C * Mtot * B + atoms_in + atoms_out,
+    }
+
+
+def cpu_baseline(wl, r_c, seconds_target=15.0):
+    """The oracle as it stands (oracle/direct_sum.c), on a bounded sample: rho(k), E, phi and F of the
+    first n_s atoms over ALL modes of the workload.  Cost per atom does not depend on N (the mode
+    set is fixed by box, c, r_c), so atoms/s of the sample is the oracle's atom-steps/s."""
+    from oracle.direct import direct_sums_c, c_threads, mode_set
+    K = len(mode_set(wl["box"], wl["c"], r_c, wl["grid"], half=True))
+    n_s = 2000
+    pos, q = wl["pos"], wl["q"]
+    t0 = time.perf_counter()
+    direct_sums_c(pos[:n_s], q[:, :n_s], wl["exponents"], wl["box"], wl["c"], r_c, grid=wl["grid"])
+    dt = time.perf_counter() - t0          # includes the one-off kernel-table evaluation
+    t0 = time.perf_counter()
+    direct_sums_c(pos[:n_s], q[:, :n_s], wl["exponents"], wl["box"], wl["c"], r_c, grid=wl["grid"])
+    dt2 = time.perf_counter() - t0
+    rate = n_s / max(dt2, 1e-9)
+    n_big = int(min(len(pos), max(n_s, rate * seconds_target)))
+    t0 = time.perf_counter()
+    direct_sums_c(pos[:n_big], q[:, :n_big], wl["exponents"], wl["box"], wl["c"], r_c, grid=wl["grid"])
+    dt3 = time.perf_counter() - t0
+    return {"value": n_big / dt3, "unit": UNIT, "cores": c_threads(), "kind": "oracle",
+            "sample": "oracle A (direct k-sum, float64, oracle/direct_sum.c): E, phi, F of the first %d atoms "
+                      "of the workload over all %d half-space modes, %.1f s" % (n_big, K, dt3)}
+
+
+def run_reference(args):
+    rank, local, world = dist_env()
+    if rank != 0:
+        return 0
+    from paper_2606_06617_b200 import workloads
+    from oracle import gridded as G
+    from oracle.direct import direct_sums_c, c_threads, mode_set
+    wl = workloads.make(args.cfg, n_atoms=args.atoms)
+    r_c = G.default_r_c(wl["box"], wl["grid"], wl["c"])
+    K = len(mode_set(wl["box"], wl["c"], r_c, wl["grid"], half=True))
+    n_s = args.ref_atoms
+    run = lambda: direct_sums_c(wl["pos"][:n_s], wl["q"][:, :n_s], wl["exponents"], wl["box"], wl["c"], r_c,
+                                grid=wl["grid"])
+    for _ in range(args.warmup):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run()
+    dt = time.perf_counter() - t0
+    val = n_s * args.steps / dt
+    sample = ("each step = oracle A (direct k-sum, float64) on the first %d atoms of the workload over all %d "
+              "half-space modes" % (n_s, K))
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl["name"], "n_atoms": len(wl["pos"]), "grid": wl["grid"], "w": wl["w"],
+                       "exponents": wl["exponents"], "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": c_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_06617_b200 import binding, build, workloads
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    build.build()
+    wl = workloads.make(args.cfg, n_atoms=args.atoms, seed=rank_seed(args.cfg, rank))
+    N, C = len(wl["pos"]), len(wl["exponents"])
+    dt_t = torch.float32 if wl["precision"] == "f32" else torch.float64
+    plan = binding.Plan(wl["box"], wl["grid"], wl["w"], wl["c"], wl["exponents"], precision=wl["precision"],
+                        max_atoms=N, kernel_path=args.kernel_path)
+    info = plan.info()
+    n_sets = args.steps + args.warmup
+    # positions of every step, advanced by seeded displacements (config 4's stepping loop)
+    box = np.asarray(wl["box"])
+    pos_sets = []
+    p = wl["pos"].copy()
+    for dsp in workloads.md_displacements(rank_seed(args.cfg, rank), n_sets, N, sigma=0.01):
+        pos_sets.append(torch.as_tensor(np.mod(p, box), dtype=dt_t))
+        p = p + dsp
+    q_h = torch.as_tensor(wl["q"], dtype=dt_t).pin_memory()
+    pos_h = [t.pin_memory() for t in pos_sets]
+    pos_d = [t.to(dev) for t in pos_h]
+    q_d = q_h.to(dev)
+    E_d = torch.zeros(1, dtype=torch.float64, device=dev)
+    phi_d = torch.empty((C, N), dtype=dt_t, device=dev)
+    F_d = torch.empty((N, 3), dtype=dt_t, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+    sp = stream.cuda_stream
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ----
+    for i in range(args.warmup):
+        plan.execute(N, pos_d[i], q_d, E_d, phi_d, F_d, sp)
+    torch.cuda.synchronize()
+    plan.set_profiling(True)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    clocks = ClockSampler(local)
+    clocks.start()
+    barrier()
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)                       # L2 flush between timed iterations (not timed)
+        evs[i][0].record(stream)
+        plan.execute(N, pos_d[args.warmup + i], q_d, E_d, phi_d, F_d, sp)
+        evs[i][1].record(stream)
+    barrier()
+    clk = clocks.stop()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_s = sum(step_ms) / 1e3
+    stage_ms, n_prof = plan.stage_ms()
+    plan.set_profiling(False)
+    E_last = float(E_d.item())
+    total_s_max, atoms_all = reduce_times(total_s, N, dev)
+    value = atoms_all * args.steps / total_s_max
+
+    # ---- end to end through the C ABI with host buffers (H2D + compute + D2H every step) ----
+    E_h = torch.zeros(1, dtype=torch.float64).pin_memory()
+    phi_h = torch.empty((C, N), dtype=dt_t).pin_memory()
+    F_h = torch.empty((N, 3), dtype=dt_t).pin_memory()
+    for i in range(min(args.warmup, 3)):
+        plan.execute_host(N, pos_h[i], q_h, E_h, phi_h, F_h, sp)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        plan.execute_host(N, pos_h[args.warmup + i], q_h, E_h, phi_h, F_h, sp)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    barrier()
+    e2e_s_max, _ = reduce_times(e2e_s, N, dev)
+    rs = 4 if wl["precision"] == "f32" else 8
+    h2d = N * (3 + C) * rs
+    d2h = 8 + N * (3 + C) * rs
+    assert abs(E_h.item() - E_last) <= 1e-4 * abs(E_last), "e2e and device-resident energies differ"
+
+    if rank != 0:
+        plan.destroy()
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel ----
+    peak_gbs, peak_src, sm_max = measured_peaks()
+    bytes_alg = algorithmic_bytes(N, C, wl["grid"], rs)
+    dom = max(("spread", "gather"), key=lambda k: stage_ms[k])
+    w3 = wl["w"] ** 3
+    flops_alg = {"spread": 2.0 * N * C * w3, "gather": 2.0 * 2.0 * N * C * w3}
+    alu_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12          # fp32 FMA peak at max clock, TFLOP/s
+    ach = flops_alg[dom] / (stage_ms[dom] * 1e-3) / 1e12
+    roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": ach / alu_peak, "traffic": None,
+                "peak_source": "148 SM x 128 FMA/clk x 2 x %.0f MHz (DESIGN.md §6)" % sm_max,
+                "hbm_achieved_gbs": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9,
+                "hbm_frac": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9 / peak_gbs}
+    stages = {k: {"ms": stage_ms[k], "alg_bytes": bytes_alg[k],
+                  "gbs": (bytes_alg[k] / (stage_ms[k] * 1e-3) / 1e9) if stage_ms[k] > 0 else None,
+                  "hbm_frac": (bytes_alg[k] / (stage_ms[k] * 1e-3) / 1e9 / peak_gbs) if stage_ms[k] > 0 else None}
+              for k in binding.STAGE_NAMES}
+    pipeline_bytes = sum(bytes_alg.values())
+    ms_per_step = 1e3 * total_s_max / args.steps
+
+    # ---- CPU baseline: the oracle on this box's host cores ----
+    cb = None
+    if not args.no_cpu_baseline:
+        cb = cpu_baseline(wl, info["r_c"])
+
+    launches_per_step = {"ref": 9, "fast": 10}["fast" if args.kernel_path == 0 else "ref"]
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": wl["precision"], "data": "synthetic",
+        "evals_per_s": world * args.steps / total_s_max,
+        "config": {"workload": wl["name"], "n_atoms": N, "box": wl["box"], "grid": wl["grid"], "w": wl["w"],
+                   "exponents": wl["exponents"], "c": wl["c"], "r_c": info["r_c"], "c_window": info["c_window"],
+                   "timing": "per-step CUDA events on the execute stream, summed over %d steps" % args.steps,
+                   "l2": "flushed between timed steps (256 MiB write, outside the events)",
+                   "parallelism": "independent replica per GPU" if world > 1 else "single GPU",
+                   "kernel_path": args.kernel_path},
+        "e2e": {"value": atoms_all * args.steps / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s_max / args.steps,
+                "api": "pswf_lr_execute_host (pinned host buffers)"},
+        "gpu_launches": args.steps * launches_per_step,
+        "clocks": clk,
+        "roofline": roofline,
+        "stages": stages,
+        "pipeline": {"alg_bytes": pipeline_bytes, "gbs": pipeline_bytes / (ms_per_step * 1e-3) / 1e9,
+                     "hbm_frac": pipeline_bytes / (ms_per_step * 1e-3) / 1e9 / peak_gbs,
+                     "hbm_peak_gbs": peak_gbs, "hbm_peak_source": peak_src},
+        "cpu_baseline": cb,
+        "energy_last_step": E_last,
+    }
+    print(json.dumps(line))
+    plan.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)     # paper's protocol: 5 warm-up + 20 timed
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cfg", type=int, default=4)
+    ap.add_argument("--atoms", type=int, default=None, help="override the atom count (same box and grid)")
+    ap.add_argument("--kernel-path", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-atoms", type=int, default=4000, help="atoms per reference step (bounded sample)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,147 @@
+/* pswf_lr.h -- C ABI of the B200-native PSWF-LR reciprocal-space library.
+ *
+ * What it computes (arxiv/paper_2606_06617; line numbers refer to /root/reference/PAPER.md):
+ * the reciprocal-space part of the PSWF-mollified inverse-power energy, Eq. (5),
+ *
+ *     E = 1/(2V) sum_a sum_{k != 0} Phi^_{p_a}(k) |rho_a(k)|^2 + sum_a E_0^{(p_a)},
+ *     rho_a(k) = sum_j q_j^a exp(i k.r_j)                                   Eq. (6)
+ *
+ * for several channels a (latent charges q^a, exponent p_a in 1..6), by the gridded algorithm of
+ * (i) spread with the separable PSWF window, Eq. (20)-(21),(24); (ii) batched
+ * forward 3-D FFT; (iii) diagonal scaling by Phi^_p(k)/W^(k)^2, Eq. (22),(25), with Phi^_p from
+ * Eq. (14) / SI Theorem 1 (S47)-(S52) and the k = 0 constants of Eq. (17)-(19) / (S73),(S75),(S78),
+ * (S79); (iv) Fourier-space reduction to E, Eq. (26); then -- as BASELINE.json's north_star asks,
+ * and as the automatic-differentiation backward of (i)-(iv) does -- an inverse
+ * FFT and a gather with the window and its derivative, giving per-atom potentials
+ * phi_i^a = dE/dq_i^a and forces F_i = -dE/dr_i (q fixed).
+ * No self term, no real-space term: those are off the hot path ("out of scope").
+ *
+ * All kernels are CUDA for sm_100a; the 3-D FFTs are cuFFT.  There is no CPU fallback: every
+ * call fails with PSWF_LR_ERR_CUDA when no device is usable.
+ *
+ * Conventions
+ *   - Orthorhombic periodic box (Lx,Ly,Lz), k = 2 pi (mx/Lx, my/Ly, mz/Lz).
+ *   - Lengths in Angstrom, energies in q^2 / A^p (Eq. (2) carries no prefactor).
+ *   - "real" is float when the plan's precision is PSWF_LR_F32 and double for PSWF_LR_F64.
+ *   - Every function returns 0 on success or a negative pswf_lr_status; no exception crosses
+ *     the ABI.  pswf_lr_error_string() names a code.
+ *   - A plan is bound to the CUDA device current at creation and owns every workspace, table
+ *     and cuFFT plan.  One plan must not be executed from two streams at once.
+ */
+#ifndef PSWF_LR_H
+#define PSWF_LR_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pswf_lr_plan pswf_lr_plan; /* opaque */
+
+typedef enum {
+  PSWF_LR_OK = 0,
+  PSWF_LR_ERR_INVALID_ARG = -1,          /* null pointer, non-positive size, w out of range ...   */
+  PSWF_LR_ERR_UNSUPPORTED_EXPONENT = -2, /* p outside 1..6 (p >= 7: PAPER.md:878, out of scope)   */
+  PSWF_LR_ERR_GRID_TOO_COARSE = -3,      /* h > pi r_c / c (Eq. (29)), w > M_d, or the window      */
+                                         /* transform would be used outside its band              */
+  PSWF_LR_ERR_ALLOC = -4,
+  PSWF_LR_ERR_CUDA = -5,
+  PSWF_LR_ERR_CUFFT = -6
+} pswf_lr_status;
+
+enum { PSWF_LR_F32 = 0, PSWF_LR_F64 = 1 };
+
+/* Optional plan parameters; zero-initialise and set what you need (0 = default). */
+typedef struct {
+  double r_c;       /* mollifier cutoff r_c (A), Eq. (3),(13).  Default: c * max_d(h_d) / (0.5 pi),    */
+                    /* i.e. eta = 0.5 in Eq. (29) (reading R2).                               */
+  double c_window;  /* PSWF bandwidth of the spreading window (reading R3: separate from c).           */
+                    /* Default: w * (3.55 - 1.55 eta), eta = c * max_d(h_d) / (pi r_c).                 */
+  int precision;    /* PSWF_LR_F32 (default) or PSWF_LR_F64: type of pos, q, phi, F and the grids.     */
+  int max_atoms;    /* capacity hint; buffers grow on demand.                                          */
+  int zero_mode;    /* 0: the paper's k = 0 conventions (S73)/(S75)/(S78)/(S79), E_IB = 0 (default);   */
+                    /* 1: drop the k = 0 mode.                                                          */
+  int kernel_path;  /* 0: fastest available kernels (default); 1: simple reference kernels            */
+                    /* (one warp per atom, global atomics) -- same arithmetic, for cross-checks.        */
+  double poly_eps;  /* tolerance of the Horner tables.  Default 1e-7 (f32), 1e-12 (f64) */
+  int host_only;    /* 1: build the host-side tables only (no device is touched); such a plan serves    */
+                    /* pswf_lr_get_info / pswf_lr_eval_window / pswf_lr_eval_kernel and every compute    */
+                    /* call on it fails with PSWF_LR_ERR_CUDA.  Not a CPU fallback.                      */
+} pswf_lr_opts;
+
+/* Read-back of what the plan resolved (all host values). */
+typedef struct {
+  double r_c, c, c_window, eta;
+  int w, precision, n_channels, n_distinct_p;
+  int grid[3];
+  int window_degree;     /* degree of the per-panel window polynomials                  */
+  int kernel_degree;     /* degree of the per-panel polynomials for Phi^_p              */
+  int kernel_panels;
+  long long modes_in_ball;    /* half-spectrum modes with a non-zero multiplier          */
+  long long workspace_bytes;  /* device memory owned by the plan                         */
+} pswf_lr_info;
+
+/* Create a plan.  box[3]: edge lengths; grid[3]: M_x,M_y,M_z (each >= w, product < 2^31);
+ * w: window width P in grid points (even, 2..16); c: mollifier bandwidth
+ * (Eq. (28)), 2 <= c <= 60; exponents[n_channels]: p_a in 1..6, repeats allowed.
+ * Host pointers; nothing is retained.  Runs the host-side PSWF eigen-solve, fits the Horner
+ * tables, builds cuFFT plans, allocates workspaces. */
+int pswf_lr_plan_create(pswf_lr_plan** plan, const double box[3], const int grid[3], int w, double c,
+                        const int* exponents, int n_channels);
+int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int grid[3], int w,
+                           double c, const int* exponents, int n_channels, const pswf_lr_opts* opts);
+
+/* One evaluation, asynchronous on `stream` (a cudaStream_t; NULL = default stream).  No host
+ * synchronisation and no host<->device copy happens inside (workspaces grow, with a sync, only
+ * when n_atoms exceeds the capacity seen so far).
+ *   pos  device, real[n_atoms][3]; any real coordinates (wrapped into the box internally)
+ *   q    device, real[n_channels][n_atoms]
+ *   E    device, double[1]: total energy, Eq. (26) (accumulated in double); may be NULL
+ *   phi  device, real[n_channels][n_atoms], phi_i^a = dE/dq_i^a; may be NULL
+ *   F    device, real[n_atoms][3], F_i = -dE/dr_i; may be NULL
+ * Outputs are in the caller's atom order.  If phi and F are both NULL the inverse FFT and the
+ * gather are skipped (the paper's energy-only path).  n_atoms = 0 is legal. */
+int pswf_lr_execute(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, void* E,
+                    void* phi, void* F, void* stream);
+
+/* Same evaluation with HOST buffers (pinned or pageable): copies pos and q to the device,
+ * executes, copies E, phi, F back, all on `stream`, and synchronises the stream before
+ * returning.  This is the end-to-end entry point bench.py times as "e2e". */
+int pswf_lr_execute_host(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, double* E,
+                         void* phi, void* F, void* stream);
+
+/* Per-channel energies of the most recent execute: device double[n_channels] (async on stream).
+ * The paper reports per-component contributions. */
+int pswf_lr_channel_energies(pswf_lr_plan* plan, void* E_channels, void* stream);
+
+int pswf_lr_get_info(const pswf_lr_plan* plan, pswf_lr_info* info);
+
+/* Stage timing with CUDA events recorded on the execute stream (for bench.py's roofline line).
+ * Stages: 0 bin+sort, 1 spread, 2 forward FFT, 3 scale+reduce, 4 inverse FFT, 5 gather.
+ * pswf_lr_stage_ms synchronises on the last event and returns, per stage, the mean milliseconds
+ * over the executes since profiling was enabled (or last read), then resets the accumulation. */
+enum { PSWF_LR_N_STAGES = 6 };
+int pswf_lr_set_profiling(pswf_lr_plan* plan, int enabled);
+int pswf_lr_stage_ms(pswf_lr_plan* plan, double ms[PSWF_LR_N_STAGES], int* n_executes);
+
+/* Test hook: copy an intermediate of the most recent execute to a caller's DEVICE buffer.
+ *   what = 0: real grid after spreading, real[n_channels][Mx][My][Mz]
+ *   what = 1: scaled half-spectrum, 2*real[n_channels][Mx][My][Mz/2+1] (re,im interleaved)
+ *   what = 2: potential grid after the inverse FFT, real[n_channels][Mx][My][Mz]
+ * Only meaningful when the intermediate still exists (call right after execute; the real grid is
+ * overwritten by the inverse FFT, so what = 0 needs an execute with phi = F = NULL). */
+int pswf_lr_debug_copy(pswf_lr_plan* plan, int what, void* dst, void* stream);
+
+/* Host-side evaluation of the plan's fitted tables (tests compare them with the oracle):
+ *   window:  W(z) and dW/dz for z in [-1,1) from the panel polynomials
+ *   kernel:  Phi^_p(k) as the scale kernel evaluates it (k in 1/A) */
+int pswf_lr_eval_window(const pswf_lr_plan* plan, int n, const double* z, double* W, double* dW);
+int pswf_lr_eval_kernel(const pswf_lr_plan* plan, int p, int n, const double* k, double* Phi);
+
+int pswf_lr_destroy(pswf_lr_plan* plan);
+const char* pswf_lr_error_string(int code);
+const char* pswf_lr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSWF_LR_H */

@@ -1,0 +1,390 @@
+// Reference-quality CUDA kernels of the PSWF-LR path: binning/counting sort, warp-per-atom
+// spread with global atomics, the fused scale+reduce kernel over the half spectrum, and a
+// warp-per-atom gather.  They run every configuration in both precisions (any even w <= 16,
+// any channel count); the fp64 path and kernel_path = 1 always use them.  The tiled fp32
+// kernels in kernels_fast.cu replace spread and gather on the default path.
+#include "kernels_common.cuh"
+#include "launch.hpp"
+
+namespace pswf {
+
+// ------------------------------------------------------------------------------------------------
+// a0. bin + counting sort (not in the paper, required by tiled kernels).
+// Key = stencil cell (s_x, s_y, s_z), s_d = i0_d mod M_d, z fastest.
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void k_bin_count(int n, const T* __restrict__ pos, GridGeom<T> g, int* __restrict__ count,
+                            int* __restrict__ key, int* __restrict__ rank) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int s[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    int i0;
+    double delta;
+    stencil_1d((double)pos[3 * (size_t)i + d], g.invL[d], g.M[d], g.w, i0, delta);
+    s[d] = wrap_index(i0, g.M[d]);
+  }
+  int k = (s[0] * g.M[1] + s[1]) * g.M[2] + s[2];
+  key[i] = k;
+  rank[i] = atomicAdd(&count[k], 1);
+}
+
+// Exclusive scan of count[0..n) in place, three kernels (block scan, scan of block sums, add).
+constexpr int kScanThreads = 512;
+constexpr int kScanItems = 8;
+
+__global__ void k_scan_blocks(int n, int* __restrict__ data, int* __restrict__ blocksums) {
+  __shared__ int warp_tot[kScanThreads / 32];
+  const int base = (blockIdx.x * kScanThreads + threadIdx.x) * kScanItems;
+  int v[kScanItems];
+  int sum = 0;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    v[j] = (base + j < n) ? data[base + j] : 0;
+    sum += v[j];
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int incl = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) warp_tot[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    int t = (lane < kScanThreads / 32) ? warp_tot[lane] : 0;
+    int inc = t;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int u = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += u;
+    }
+    if (lane < kScanThreads / 32) warp_tot[lane] = inc - t;  // exclusive warp offsets
+    if (lane == 31) blocksums[blockIdx.x] = inc;
+  }
+  __syncthreads();
+  int run = warp_tot[wid] + incl - sum;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) {
+    if (base + j < n) data[base + j] = run;
+    run += v[j];
+  }
+}
+
+__global__ void k_scan_sums(int nblocks, int* __restrict__ blocksums) {
+  // single block: exclusive scan of blocksums, any length
+  __shared__ int warp_tot[32];
+  __shared__ int carry_s;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int base = 0; base < nblocks; base += blockDim.x) {
+    int i = base + threadIdx.x;
+    int v = (i < nblocks) ? blocksums[i] : 0;
+    int incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (lane == 31) warp_tot[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+      int t = warp_tot[lane];
+      int inc = t;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        int u = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += u;
+      }
+      warp_tot[lane] = inc - t;
+    }
+    __syncthreads();
+    int carry = carry_s;
+    if (i < nblocks) blocksums[i] = carry + warp_tot[wid] + incl - v;
+    __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) carry_s = carry + warp_tot[wid] + incl;
+    __syncthreads();
+  }
+}
+
+__global__ void k_scan_add(int n, int* __restrict__ data, const int* __restrict__ blocksums, int total_slot,
+                           int total) {
+  const int base = (blockIdx.x * kScanThreads + threadIdx.x) * kScanItems;
+  const int add = blocksums[blockIdx.x];
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j)
+    if (base + j < n) data[base + j] += add;
+  if (blockIdx.x == 0 && threadIdx.x == 0) data[total_slot] = total;
+}
+
+template <class T>
+__global__ void k_scatter(int n, int C, int cap, const T* __restrict__ pos, const T* __restrict__ q,
+                          GridGeom<T> g, const int* __restrict__ start, const int* __restrict__ key,
+                          const int* __restrict__ rank, int* __restrict__ perm, int* __restrict__ si0,
+                          T* __restrict__ sdelta, T* __restrict__ sq) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int dst = start[key[i]] + rank[i];
+  perm[dst] = i;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    int i0;
+    double delta;
+    stencil_1d((double)pos[3 * (size_t)i + d], g.invL[d], g.M[d], g.w, i0, delta);
+    si0[(size_t)d * cap + dst] = i0;
+    sdelta[(size_t)d * cap + dst] = (T)delta;
+  }
+  for (int c = 0; c < C; ++c) sq[(size_t)c * cap + dst] = q[(size_t)c * n + i];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1. spread, reference kernel: one warp per atom, w^3 global atomic adds per channel.
+// rho_g^a = sum_j q_j^a prod_d psi((x_{g,d} - r_{j,d}) / omega_d)     Eq. (20)-(21),(24)
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void k_spread_ref(int n, int C, int cap, GridGeom<T> g, const int* __restrict__ si0,
+                             const T* __restrict__ sdelta, const T* __restrict__ sq, T* __restrict__ grid) {
+  __shared__ T wts[8][3 * kMaxW];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int j = blockIdx.x * 8 + wid;
+  if (j >= n) return;
+  const int w = g.w;
+  for (int t = lane; t < 3 * w; t += 32) {
+    int d = t / w, tt = t - d * w;
+    T xi = (T)2 * sdelta[(size_t)d * cap + j] - (T)1;
+    wts[wid][d * kMaxW + tt] = horner_panel(g.wcoef, w, tt, g.wdeg, xi);
+  }
+  __syncwarp();
+  const int i0x = si0[j], i0y = si0[(size_t)cap + j], i0z = si0[2 * (size_t)cap + j];
+  const size_t Mtot = (size_t)g.M[0] * g.M[1] * g.M[2];
+  const int w3 = w * w * w;
+  for (int idx = lane; idx < w3; idx += 32) {
+    int a = idx / (w * w), r = idx - a * w * w, b = r / w, cc = r - b * w;
+    T wt = wts[wid][a] * wts[wid][kMaxW + b] * wts[wid][2 * kMaxW + cc];
+    size_t gi = ((size_t)wrap_index(i0x + a, g.M[0]) * g.M[1] + wrap_index(i0y + b, g.M[1])) * g.M[2] +
+                wrap_index(i0z + cc, g.M[2]);
+    for (int c = 0; c < C; ++c) atomicAdd(&grid[(size_t)c * Mtot + gi], sq[(size_t)c * cap + j] * wt);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3. scale (deconvolve x Green) + Fourier-space energy reduction, fused over channels.
+// phi^_a(m) = D_{p_a}(m) rho^_a(m),  D_p(m) = (h_x h_y h_z / M_tot) Phi^_p(|k_m|) / W^(k_m)^2
+// (Eq. (22),(25); reading R10), zero for |k| r_c >= c and on Nyquist planes (R11);
+// E_a = 1/2 sum_m D |rho^_a(m)|^2 (Eq. (26)) with Hermitian weights over the half spectrum.
+// Phi^_p is evaluated once per distinct exponent per mode by Horner on the smooth part
+// and reused by every channel with that exponent.
+// ------------------------------------------------------------------------------------------------
+template <class T>
+struct Cplx { T x, y; };
+
+template <class T>
+__device__ __forceinline__ T kernel_value(const ScaleParams<T>& P, int slot, T x, T kappa) {
+  // x = kappa / c in (0,1)
+  int j = min((int)(x * (T)P.panels), P.panels - 1);
+  T xi = (T)2 * (x * (T)P.panels - (T)j) - (T)1;
+  const T* cf = P.kcoef + ((size_t)slot * P.panels + j) * (P.degree + 1);
+  T t = cf[P.degree];
+  for (int m = P.degree - 1; m >= 0; --m) t = fma(t, xi, cf[m]);
+  T s;
+  switch (P.slot_p[slot]) {
+    case 1: s = t / (kappa * kappa); break;            // x 4 pi r_c^2      (S47)
+    case 2: s = t / kappa; break;                      // x 2 pi^2 r_c      (S48)
+    case 3: s = t - log(x); break;                     // x 4 pi            (S49)
+    case 4: s = t; break;                              // x pi^2 c / r_c    (S50)
+    case 5: s = t + x * x * log(x); break;             // x 2 pi c^2/(3 r_c^2)  (S51)
+    default: s = t; break;                             // x pi^2 c^3/(12 r_c^3) (S52)
+  }
+  return s * P.slot_pre[slot];
+}
+
+template <class T>
+__global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __restrict__ Ech, int want_E) {
+  const size_t Mhalf = (size_t)P.M[0] * P.M[1] * P.Mzh;
+  const size_t m = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  __shared__ double red[kMaxChannels];
+  if (threadIdx.x < kMaxChannels) red[threadIdx.x] = 0.0;
+  __syncthreads();
+  bool active = m < Mhalf;
+  bool inside = false;
+  T D[6];
+  T herm = (T)0;
+  int iz = 0;
+  bool is_zero_mode = false;
+  if (active) {
+    iz = (int)(m % P.Mzh);
+    size_t r = m / P.Mzh;
+    int iy = (int)(r % P.M[1]);
+    int ix = (int)(r / P.M[1]);
+    int fx = ix <= P.M[0] / 2 ? ix : ix - P.M[0];
+    int fy = iy <= P.M[1] / 2 ? iy : iy - P.M[1];
+    int fz = iz;
+    bool nyq = ((P.M[0] % 2 == 0) && ix == P.M[0] / 2) || ((P.M[1] % 2 == 0) && iy == P.M[1] / 2) ||
+               ((P.M[2] % 2 == 0) && iz == P.M[2] / 2);
+    T kx = P.kfac[0] * (T)fx, ky = P.kfac[1] * (T)fy, kz = P.kfac[2] * (T)fz;
+    T kn = sqrt(kx * kx + ky * ky + kz * kz);
+    T x = kn * P.x_per_k;
+    is_zero_mode = (ix == 0 && iy == 0 && iz == 0);
+    inside = !nyq && !is_zero_mode && x < (T)1;
+    herm = (iz == 0 || ((P.M[2] % 2 == 0) && iz == P.M[2] / 2)) ? (T)1 : (T)2;
+    if (inside) {
+      T base = P.base * P.invW2[0][ix] * P.invW2[1][iy] * P.invW2[2][iz];
+      T kappa = x * P.c;
+      for (int s = 0; s < P.nslots; ++s) D[s] = base * kernel_value(P, s, x, kappa);
+    }
+  }
+  for (int c = 0; c < P.C; ++c) {
+    double e = 0.0;
+    if (active) {
+      Cplx<T>* ptr = spec + (size_t)c * Mhalf + m;
+      if (inside || is_zero_mode) {
+        T d = is_zero_mode ? P.chan_D0[c] : D[P.chan_slot[c]];
+        Cplx<T> v = *ptr;
+        e = (double)(herm * d * (v.x * v.x + v.y * v.y));
+        v.x *= d;
+        v.y *= d;
+        *ptr = v;
+      } else {
+        Cplx<T> z;
+        z.x = (T)0;
+        z.y = (T)0;
+        *ptr = z;  // outside the band: no read, just clear
+      }
+    }
+    if (want_E) {
+      e = warp_sum(e);
+      if ((threadIdx.x & 31) == 0 && e != 0.0) atomicAdd(&red[c], e);
+    }
+  }
+  if (want_E) {
+    __syncthreads();
+    if (threadIdx.x < P.C && red[threadIdx.x] != 0.0) atomicAdd(&Ech[threadIdx.x], 0.5 * red[threadIdx.x]);
+  }
+}
+
+__global__ void k_finalize_energy(int C, const double* __restrict__ Ech, double* __restrict__ E) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    double s = 0.0;
+    for (int c = 0; c < C; ++c) s += Ech[c];
+    *E = s;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5. gather + force, reference kernel: one warp per atom.
+// phi_i^a = sum_g W(x_g - r_i) phi_g^a;  grad = sum_g grad_{r_i} W phi_g^a (derivative of the SAME
+// panel polynomials);  F_i = - sum_a q_i^a grad phi_i^a.
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void k_gather_ref(int n, int C, int cap, GridGeom<T> g, const int* __restrict__ si0,
+                             const T* __restrict__ sdelta, const T* __restrict__ sq,
+                             const int* __restrict__ perm, const T* __restrict__ grid, T* __restrict__ phi,
+                             T* __restrict__ F) {
+  __shared__ T wts[8][6 * kMaxW];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int j = blockIdx.x * 8 + wid;
+  if (j >= n) return;
+  const int w = g.w;
+  for (int t = lane; t < 3 * w; t += 32) {
+    int d = t / w, tt = t - d * w;
+    T xi = (T)2 * sdelta[(size_t)d * cap + j] - (T)1;
+    wts[wid][d * kMaxW + tt] = horner_panel(g.wcoef, w, tt, g.wdeg, xi);
+    wts[wid][(3 + d) * kMaxW + tt] = horner_panel(g.wdcoef, w, tt, g.wdeg - 1, xi) * g.dxi_dr[d];
+  }
+  __syncwarp();
+  const int i0x = si0[j], i0y = si0[(size_t)cap + j], i0z = si0[2 * (size_t)cap + j];
+  const size_t Mtot = (size_t)g.M[0] * g.M[1] * g.M[2];
+  const int w3 = w * w * w;
+  const int dst = perm[j];
+  T fx = 0, fy = 0, fz = 0;
+  for (int c = 0; c < C; ++c) {
+    T v = 0, gx = 0, gy = 0, gz = 0;
+    const T* gc = grid + (size_t)c * Mtot;
+    for (int idx = lane; idx < w3; idx += 32) {
+      int a = idx / (w * w), r = idx - a * w * w, b = r / w, cc = r - b * w;
+      size_t gi = ((size_t)wrap_index(i0x + a, g.M[0]) * g.M[1] + wrap_index(i0y + b, g.M[1])) * g.M[2] +
+                  wrap_index(i0z + cc, g.M[2]);
+      T val = gc[gi];
+      T wx = wts[wid][a], wy = wts[wid][kMaxW + b], wz = wts[wid][2 * kMaxW + cc];
+      T dx = wts[wid][3 * kMaxW + a], dy = wts[wid][4 * kMaxW + b], dz = wts[wid][5 * kMaxW + cc];
+      T yz = wy * wz * val;
+      v += wx * yz;
+      gx += dx * yz;
+      gy += wx * dy * wz * val;
+      gz += wx * wy * dz * val;
+    }
+    v = warp_sum(v);
+    gx = warp_sum(gx);
+    gy = warp_sum(gy);
+    gz = warp_sum(gz);
+    T qc = sq[(size_t)c * cap + j];
+    fx -= qc * gx;
+    fy -= qc * gy;
+    fz -= qc * gz;
+    if (lane == 0 && phi) phi[(size_t)c * n + dst] = v;
+  }
+  if (lane == 0 && F) {
+    F[3 * (size_t)dst + 0] = fx;
+    F[3 * (size_t)dst + 1] = fy;
+    F[3 * (size_t)dst + 2] = fz;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host launchers
+// ------------------------------------------------------------------------------------------------
+template <class T>
+void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, cudaStream_t st) {
+  const int Mtot = p->M[0] * p->M[1] * p->M[2];
+  cudaMemsetAsync(p->d_count, 0, sizeof(int) * ((size_t)Mtot + 1), st);
+  if (n > 0)
+    k_bin_count<T><<<(n + 255) / 256, 256, 0, st>>>(n, pos, g, p->d_count, p->d_key, p->d_rank);
+  k_scan_blocks<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_blocksums);
+  k_scan_sums<<<1, 1024, 0, st>>>(p->n_scan_blocks, p->d_blocksums);
+  k_scan_add<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_blocksums, Mtot, n);
+  if (n > 0)
+    k_scatter<T><<<(n + 255) / 256, 256, 0, st>>>(n, p->C, p->cap_atoms, pos, q, g, p->d_count, p->d_key,
+                                                   p->d_rank, p->d_perm, p->d_si0, (T*)p->d_sdelta,
+                                                   (T*)p->d_sq);
+}
+
+template <class T>
+void launch_spread_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, cudaStream_t st) {
+  const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
+  cudaMemsetAsync(p->d_grid, 0, sizeof(T) * Mtot * p->C, st);
+  if (n > 0)
+    k_spread_ref<T><<<(n + 7) / 8, 256, 0, st>>>(n, p->C, p->cap_atoms, g, p->d_si0, (const T*)p->d_sdelta,
+                                                  (const T*)p->d_sq, (T*)p->d_grid);
+}
+
+template <class T>
+void launch_scale(pswf_lr_plan* p, const ScaleParams<T>& P, bool want_E, cudaStream_t st) {
+  const size_t Mhalf = (size_t)P.M[0] * P.M[1] * P.Mzh;
+  const int threads = 256;
+  k_scale<T><<<(unsigned)((Mhalf + threads - 1) / threads), threads, 0, st>>>(P, (Cplx<T>*)p->d_spec, p->d_Ech,
+                                                                              want_E ? 1 : 0);
+}
+
+void launch_finalize_energy(pswf_lr_plan* p, double* E, cudaStream_t st) {
+  k_finalize_energy<<<1, 32, 0, st>>>(p->C, p->d_Ech, E);
+}
+
+template <class T>
+void launch_gather_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, T* phi, T* F, cudaStream_t st) {
+  if (n > 0)
+    k_gather_ref<T><<<(n + 7) / 8, 256, 0, st>>>(n, p->C, p->cap_atoms, g, p->d_si0, (const T*)p->d_sdelta,
+                                                  (const T*)p->d_sq, p->d_perm, (const T*)p->d_grid, phi, F);
+}
+
+#define PSWF_INSTANTIATE(T)                                                                               \
+  template void launch_bin_sort<T>(pswf_lr_plan*, int, const T*, const T*, const GridGeom<T>&, cudaStream_t); \
+  template void launch_spread_ref<T>(pswf_lr_plan*, int, const GridGeom<T>&, cudaStream_t);              \
+  template void launch_scale<T>(pswf_lr_plan*, const ScaleParams<T>&, bool, cudaStream_t);               \
+  template void launch_gather_ref<T>(pswf_lr_plan*, int, const GridGeom<T>&, T*, T*, cudaStream_t);
+PSWF_INSTANTIATE(float)
+PSWF_INSTANTIATE(double)
+
+}  // namespace pswf

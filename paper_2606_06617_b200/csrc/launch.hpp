@@ -1,0 +1,26 @@
+// Host-side launchers of the PSWF-LR kernels (declarations).
+#pragma once
+#include "plan.hpp"
+
+namespace pswf {
+
+template <class T>
+void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, cudaStream_t st);
+template <class T>
+void launch_spread_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, cudaStream_t st);
+template <class T>
+void launch_scale(pswf_lr_plan* p, const ScaleParams<T>& P, bool want_E, cudaStream_t st);
+void launch_finalize_energy(pswf_lr_plan* p, double* E, cudaStream_t st);
+template <class T>
+void launch_gather_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, T* phi, T* F, cudaStream_t st);
+
+// fast fp32 path (kernels_fast.cu)
+bool fast_path_supported(const pswf_lr_plan* p);
+size_t fast_record_bytes(const pswf_lr_plan* p);
+void launch_fast_prepare(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
+                         cudaStream_t st);
+void launch_fast_spread(pswf_lr_plan* p, int n, const GridGeom<float>& g, cudaStream_t st);
+void launch_fast_gather(pswf_lr_plan* p, int n, const GridGeom<float>& g, float* phi, float* F,
+                        cudaStream_t st);
+
+}  // namespace pswf

@@ -1,0 +1,106 @@
+// Plan object shared by the translation units of libpswf_lr (product code, sm_100a).
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <vector>
+
+#include "../../include/pswf_lr.h"
+#include "host_tables.hpp"
+
+namespace pswf {
+
+constexpr int kMaxChannels = 32;
+constexpr int kMaxW = 16;
+constexpr int kMaxWindowDegree = 30;
+constexpr int kMaxKernelDegree = 24;
+constexpr int kProfileRing = 512;
+
+// Parameters of the scale (deconvolve x Green) kernel, passed by value.
+template <class T>
+struct ScaleParams {
+  int M[3];
+  int Mzh;             // Mz/2 + 1
+  int C;               // channels
+  int nslots;          // distinct exponents
+  int slot_p[6];       // exponent of each slot
+  int chan_slot[kMaxChannels];
+  T chan_D0[kMaxChannels];   // multiplier of the m = 0 mode per channel (0 when dropped)
+  T slot_pre[6];       // r_c^(3-p) * constant prefactor of each slot
+  T kfac[3];           // 2 pi / L_d
+  T x_per_k;           // r_c / c
+  T c;                 // mollifier bandwidth
+  T base;              // h_x h_y h_z / M_tot
+  int panels, degree;
+  const T* kcoef;      // [slot][panel][degree+1]
+  const T* invW2[3];   // 1 / W^_d(m)^2 per signed DFT index
+};
+
+// Geometry used by bin/spread/gather kernels.
+template <class T>
+struct GridGeom {
+  int M[3];
+  int w;
+  double invL[3];      // 1 / L_d   (binning is done in double)
+  T dxi_dr[3];         // d xi / d r_d = -2 / h_d
+  int wdeg;            // window polynomial degree
+  const T* wcoef;      // [(wdeg+1)][w]
+  const T* wdcoef;     // [wdeg][w]
+};
+
+}  // namespace pswf
+
+struct pswf_lr_plan {
+  // resolved parameters
+  int precision = 0, w = 0, C = 0, zero_mode = 0, kernel_path = 0;
+  int M[3] = {0, 0, 0};
+  double L[3] = {0, 0, 0}, h[3] = {0, 0, 0};
+  double c = 0, r_c = 0, c_w = 0, eta = 0, poly_eps = 0;
+  int chan_p[pswf::kMaxChannels] = {0};
+  int chan_slot[pswf::kMaxChannels] = {0};
+  std::vector<int> distinct_p;
+  std::vector<double> Phi0;       // per distinct p
+  double What0 = 0;               // W^(0) = prod_d omega_d lambda_0
+  long long modes_in_ball = 0;
+  long long workspace_bytes = 0;
+  // host tables
+  pswf::WindowTable wt;
+  pswf::KernelTable kt;
+  // device tables (plan precision)
+  void* d_wcoef = nullptr;
+  void* d_wdcoef = nullptr;
+  void* d_kcoef = nullptr;
+  void* d_invW2[3] = {nullptr, nullptr, nullptr};
+  // device workspaces
+  void* d_grid = nullptr;         // real  [C][Mx][My][Mz]
+  void* d_spec = nullptr;         // cplx  [C][Mx][My][Mz/2+1]
+  int* d_count = nullptr;         // [Mtot + 1] cell counts -> exclusive starts
+  int* d_blocksums = nullptr;
+  int n_scan_blocks = 0;
+  double* d_Ech = nullptr;        // [C]
+  double* d_Etot = nullptr;       // [1] (execute_host staging)
+  // per-atom workspaces (capacity cap_atoms)
+  int cap_atoms = 0;
+  int* d_key = nullptr;
+  int* d_rank = nullptr;
+  int* d_perm = nullptr;
+  int* d_si0 = nullptr;           // [3][cap] unwrapped first grid index
+  void* d_sdelta = nullptr;       // real [3][cap]
+  void* d_sq = nullptr;           // real [C][cap]
+  void* d_rec = nullptr;          // fast path: per-atom weight records
+  void* d_pos_in = nullptr;       // execute_host staging
+  void* d_q_in = nullptr;
+  void* d_phi_out = nullptr;
+  void* d_F_out = nullptr;
+  int last_n_atoms = 0;
+  // cuFFT
+  cufftHandle fft_fwd = 0, fft_inv = 0;
+  bool have_fft = false;
+  // profiling
+  bool profiling = false;
+  std::vector<cudaEvent_t> events;  // kProfileRing * (N_STAGES + 1)
+  int prof_count = 0;
+  int device = 0;
+  bool host_only = false;
+  int sm_count = 148;
+};

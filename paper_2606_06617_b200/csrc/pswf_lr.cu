@@ -1,0 +1,622 @@
+// C ABI of libpswf_lr: plan creation (host-side PSWF solve + Horner tables + cuFFT plans),
+// execute (bin/sort -> spread -> FFT -> scale+reduce -> inverse FFT -> gather), destroy.
+// See include/pswf_lr.h for the contract and the PAPER.md passages behind each step.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <type_traits>
+
+#include "launch.hpp"
+
+using namespace pswf;
+
+#define CUDA_TRY(expr)                                   \
+  do {                                                   \
+    cudaError_t _e = (expr);                             \
+    if (_e != cudaSuccess) return PSWF_LR_ERR_CUDA;      \
+  } while (0)
+#define CUFFT_TRY(expr)                                  \
+  do {                                                   \
+    cufftResult _r = (expr);                             \
+    if (_r != CUFFT_SUCCESS) return PSWF_LR_ERR_CUFFT;   \
+  } while (0)
+
+namespace {
+
+template <class T>
+int upload(void** dst, const std::vector<double>& src, long long* bytes) {
+  std::vector<T> tmp(src.begin(), src.end());
+  size_t nb = sizeof(T) * std::max<size_t>(tmp.size(), 1);
+  if (cudaMalloc(dst, nb) != cudaSuccess) return PSWF_LR_ERR_ALLOC;
+  if (!tmp.empty() && cudaMemcpy(*dst, tmp.data(), sizeof(T) * tmp.size(), cudaMemcpyHostToDevice) != cudaSuccess)
+    return PSWF_LR_ERR_CUDA;
+  *bytes += (long long)nb;
+  return 0;
+}
+
+inline size_t real_size(const pswf_lr_plan* p) { return p->precision == PSWF_LR_F64 ? 8 : 4; }
+
+int dev_alloc(void** ptr, size_t bytes, long long* total) {
+  if (cudaMalloc(ptr, std::max<size_t>(bytes, 16)) != cudaSuccess) {
+    *ptr = nullptr;
+    return PSWF_LR_ERR_ALLOC;
+  }
+  *total += (long long)bytes;
+  return 0;
+}
+
+void free_atoms(pswf_lr_plan* p) {
+  void** ptrs[] = {(void**)&p->d_key, (void**)&p->d_rank, (void**)&p->d_perm, (void**)&p->d_si0, &p->d_sdelta,
+                   &p->d_sq,          &p->d_rec,          &p->d_pos_in,       &p->d_q_in,        &p->d_phi_out,
+                   &p->d_F_out};
+  for (void** q : ptrs) {
+    if (*q) cudaFree(*q);
+    *q = nullptr;
+  }
+}
+
+int ensure_capacity(pswf_lr_plan* p, int n) {
+  if (n <= p->cap_atoms) return 0;
+  // growing: wait for everything in flight, then reallocate (documented in the header)
+  if (cudaDeviceSynchronize() != cudaSuccess) return PSWF_LR_ERR_CUDA;
+  free_atoms(p);
+  int cap = std::max(n, std::max(p->cap_atoms * 2, 1024));
+  const size_t rs = real_size(p);
+  long long b = 0;
+  int rc = 0;
+  rc |= dev_alloc((void**)&p->d_key, sizeof(int) * (size_t)cap, &b);
+  rc |= dev_alloc((void**)&p->d_rank, sizeof(int) * (size_t)cap, &b);
+  rc |= dev_alloc((void**)&p->d_perm, sizeof(int) * (size_t)cap, &b);
+  rc |= dev_alloc((void**)&p->d_si0, sizeof(int) * 3 * (size_t)cap, &b);
+  rc |= dev_alloc(&p->d_sdelta, rs * 3 * (size_t)cap, &b);
+  rc |= dev_alloc(&p->d_sq, rs * (size_t)p->C * cap, &b);
+  p->cap_atoms = cap;
+  size_t recb = fast_path_supported(p) ? fast_record_bytes(p) * (size_t)cap : 0;
+  if (recb) rc |= dev_alloc(&p->d_rec, recb, &b);
+  if (rc) {
+    free_atoms(p);
+    p->cap_atoms = 0;
+    return PSWF_LR_ERR_ALLOC;
+  }
+  p->workspace_bytes += b;
+  return 0;
+}
+
+int ensure_host_staging(pswf_lr_plan* p) {
+  if (p->d_pos_in) return 0;
+  const size_t rs = real_size(p);
+  long long b = 0;
+  int rc = 0;
+  rc |= dev_alloc(&p->d_pos_in, rs * 3 * (size_t)p->cap_atoms, &b);
+  rc |= dev_alloc(&p->d_q_in, rs * (size_t)p->C * p->cap_atoms, &b);
+  rc |= dev_alloc(&p->d_phi_out, rs * (size_t)p->C * p->cap_atoms, &b);
+  rc |= dev_alloc(&p->d_F_out, rs * 3 * (size_t)p->cap_atoms, &b);
+  if (rc) return PSWF_LR_ERR_ALLOC;
+  p->workspace_bytes += b;
+  return 0;
+}
+
+template <class T>
+GridGeom<T> make_geom(const pswf_lr_plan* p) {
+  GridGeom<T> g;
+  for (int d = 0; d < 3; ++d) {
+    g.M[d] = p->M[d];
+    g.invL[d] = 1.0 / p->L[d];
+    g.dxi_dr[d] = (T)(-2.0 / p->h[d]);
+  }
+  g.w = p->w;
+  g.wdeg = p->wt.degree;
+  g.wcoef = (const T*)p->d_wcoef;
+  g.wdcoef = (const T*)p->d_wdcoef;
+  return g;
+}
+
+double slot_prefactor(int p, double c, double r_c) {
+  // Phi^_p = r_c^(3-p) S^_p, constants of Theorem 1 folded in (see host_tables.hpp / k_scale)
+  switch (p) {
+    case 1: return 4 * kPi * r_c * r_c;
+    case 2: return 2 * kPi * kPi * r_c;
+    case 3: return 4 * kPi;
+    case 4: return kPi * kPi * c / r_c;
+    case 5: return 2 * kPi * c * c / (3 * r_c * r_c);
+    default: return kPi * kPi * c * c * c / (12 * r_c * r_c * r_c);
+  }
+}
+
+template <class T>
+ScaleParams<T> make_scale(const pswf_lr_plan* p) {
+  ScaleParams<T> P;
+  memset(&P, 0, sizeof(P));
+  double hv = 1, mt = 1;
+  for (int d = 0; d < 3; ++d) {
+    P.M[d] = p->M[d];
+    P.kfac[d] = (T)(2 * kPi / p->L[d]);
+    P.invW2[d] = (const T*)p->d_invW2[d];
+    hv *= p->h[d];
+    mt *= p->M[d];
+  }
+  P.Mzh = p->M[2] / 2 + 1;
+  P.C = p->C;
+  P.nslots = (int)p->distinct_p.size();
+  for (int s = 0; s < P.nslots; ++s) {
+    P.slot_p[s] = p->distinct_p[s];
+    P.slot_pre[s] = (T)slot_prefactor(p->distinct_p[s], p->c, p->r_c);
+  }
+  for (int a = 0; a < p->C; ++a) {
+    P.chan_slot[a] = p->chan_slot[a];
+    double d0 = p->zero_mode == 0 ? (hv / mt) * p->Phi0[p->chan_slot[a]] / (p->What0 * p->What0) : 0.0;
+    P.chan_D0[a] = (T)d0;
+  }
+  P.x_per_k = (T)(p->r_c / p->c);
+  P.c = (T)p->c;
+  P.base = (T)(hv / mt);
+  P.panels = p->kt.panels;
+  P.degree = p->kt.degree;
+  P.kcoef = (const T*)p->d_kcoef;
+  return P;
+}
+
+template <class T>
+int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* phi, T* F, cudaStream_t st) {
+  constexpr bool kIsF32 = std::is_same<T, float>::value;
+  const bool fast = kIsF32 && (p->kernel_path == 0) && fast_path_supported(p);
+  GridGeom<T> g = make_geom<T>(p);
+  ScaleParams<T> P = make_scale<T>(p);
+  cudaEvent_t* ev = nullptr;
+  if (p->profiling && p->prof_count < kProfileRing)
+    ev = p->events.data() + (size_t)p->prof_count * (PSWF_LR_N_STAGES + 1);
+  if (ev) cudaEventRecord(ev[0], st);
+  // a0
+  launch_bin_sort<T>(p, n, pos, q, g, st);
+  if constexpr (kIsF32) {
+    if (fast) launch_fast_prepare(p, n, pos, q, g, st);
+  }
+  if (ev) cudaEventRecord(ev[1], st);
+  // a1
+  if constexpr (kIsF32) {
+    if (fast) launch_fast_spread(p, n, g, st);
+  }
+  if (!fast) launch_spread_ref<T>(p, n, g, st);
+  if (ev) cudaEventRecord(ev[2], st);
+  // a2
+  CUFFT_TRY(cufftSetStream(p->fft_fwd, st));
+  if (sizeof(T) == 4)
+    CUFFT_TRY(cufftExecR2C(p->fft_fwd, (cufftReal*)p->d_grid, (cufftComplex*)p->d_spec));
+  else
+    CUFFT_TRY(cufftExecD2Z(p->fft_fwd, (cufftDoubleReal*)p->d_grid, (cufftDoubleComplex*)p->d_spec));
+  if (ev) cudaEventRecord(ev[3], st);
+  // a3
+  cudaMemsetAsync(p->d_Ech, 0, sizeof(double) * p->C, st);
+  launch_scale<T>(p, P, true, st);
+  if (E) launch_finalize_energy(p, E, st);
+  if (ev) cudaEventRecord(ev[4], st);
+  if (phi || F) {
+    // a4
+    CUFFT_TRY(cufftSetStream(p->fft_inv, st));
+    if (sizeof(T) == 4)
+      CUFFT_TRY(cufftExecC2R(p->fft_inv, (cufftComplex*)p->d_spec, (cufftReal*)p->d_grid));
+    else
+      CUFFT_TRY(cufftExecZ2D(p->fft_inv, (cufftDoubleComplex*)p->d_spec, (cufftDoubleReal*)p->d_grid));
+    if (ev) cudaEventRecord(ev[5], st);
+    // a5
+    if constexpr (kIsF32) {
+      if (fast) launch_fast_gather(p, n, g, phi, F, st);
+    }
+    if (!fast) launch_gather_ref<T>(p, n, g, phi, F, st);
+    if (ev) cudaEventRecord(ev[6], st);
+  } else if (ev) {
+    cudaEventRecord(ev[5], st);
+    cudaEventRecord(ev[6], st);
+  }
+  if (ev) p->prof_count++;
+  p->last_n_atoms = n;
+  CUDA_TRY(cudaGetLastError());
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* pswf_lr_version(void) { return "pswf_lr 0.1 (sm_100a)"; }
+
+const char* pswf_lr_error_string(int code) {
+  switch (code) {
+    case PSWF_LR_OK: return "ok";
+    case PSWF_LR_ERR_INVALID_ARG: return "invalid argument";
+    case PSWF_LR_ERR_UNSUPPORTED_EXPONENT: return "unsupported exponent (p must be 1..6)";
+    case PSWF_LR_ERR_GRID_TOO_COARSE: return "grid too coarse for (c, r_c, w, c_window)";
+    case PSWF_LR_ERR_ALLOC: return "device allocation failed";
+    case PSWF_LR_ERR_CUDA: return "CUDA error (no usable device, or a kernel/launch failed)";
+    case PSWF_LR_ERR_CUFFT: return "cuFFT error";
+  }
+  return "unknown error";
+}
+
+int pswf_lr_plan_create(pswf_lr_plan** plan, const double box[3], const int grid[3], int w, double c,
+                        const int* exponents, int n_channels) {
+  return pswf_lr_plan_create_ex(plan, box, grid, w, c, exponents, n_channels, nullptr);
+}
+
+int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int grid[3], int w, double c,
+                           const int* exponents, int n_channels, const pswf_lr_opts* opts) {
+  if (!plan) return PSWF_LR_ERR_INVALID_ARG;
+  *plan = nullptr;
+  if (!box || !grid || !exponents) return PSWF_LR_ERR_INVALID_ARG;
+  if (n_channels < 1 || n_channels > kMaxChannels) return PSWF_LR_ERR_INVALID_ARG;
+  if (w < 2 || w > kMaxW || (w % 2) != 0) return PSWF_LR_ERR_INVALID_ARG;
+  if (!(c >= 2.0 && c <= 60.0)) return PSWF_LR_ERR_INVALID_ARG;
+  double mtot = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (!(box[d] > 0) || grid[d] < 1) return PSWF_LR_ERR_INVALID_ARG;
+    mtot *= grid[d];
+  }
+  if (mtot >= 2147483647.0) return PSWF_LR_ERR_INVALID_ARG;
+  for (int a = 0; a < n_channels; ++a)
+    if (exponents[a] < 1 || exponents[a] > 6) return PSWF_LR_ERR_UNSUPPORTED_EXPONENT;
+  for (int d = 0; d < 3; ++d)
+    if (grid[d] < w) return PSWF_LR_ERR_GRID_TOO_COARSE;
+  pswf_lr_opts o;
+  memset(&o, 0, sizeof(o));
+  if (opts) o = *opts;
+  if (o.precision != PSWF_LR_F32 && o.precision != PSWF_LR_F64) return PSWF_LR_ERR_INVALID_ARG;
+  if (o.r_c < 0 || o.c_window < 0 || o.max_atoms < 0 || o.poly_eps < 0) return PSWF_LR_ERR_INVALID_ARG;
+
+  if (!o.host_only) {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return PSWF_LR_ERR_CUDA;  // no CPU fallback
+  }
+
+  pswf_lr_plan* p = new (std::nothrow) pswf_lr_plan();
+  if (!p) return PSWF_LR_ERR_ALLOC;
+  int rc = 0;
+  try {
+    p->host_only = o.host_only != 0;
+    if (!p->host_only) {
+      cudaGetDevice(&p->device);
+      cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
+    }
+    p->precision = o.precision;
+    p->w = w;
+    p->C = n_channels;
+    p->c = c;
+    p->zero_mode = o.zero_mode;
+    p->kernel_path = o.kernel_path;
+    double hmax = 0;
+    for (int d = 0; d < 3; ++d) {
+      p->M[d] = grid[d];
+      p->L[d] = box[d];
+      p->h[d] = box[d] / grid[d];
+      hmax = std::max(hmax, p->h[d]);
+    }
+    // reading R2: default r_c puts eta = 0.5 in Eq. (29)
+    p->r_c = o.r_c > 0 ? o.r_c : c * hmax / (0.5 * kPi);
+    p->eta = c * hmax / (kPi * p->r_c);
+    if (p->eta > 1.0 + 1e-12) rc = PSWF_LR_ERR_GRID_TOO_COARSE;  // Eq. (29): h <= eta pi r_c / c, eta <= 1
+    // reading R3: window bandwidth
+    p->c_w = o.c_window > 0 ? o.c_window : w * (3.55 - 1.55 * p->eta);
+    p->poly_eps = o.poly_eps > 0 ? o.poly_eps : (p->precision == PSWF_LR_F64 ? 1e-12 : 1e-7);
+
+    // distinct exponents, slots
+    for (int a = 0; a < n_channels; ++a) p->chan_p[a] = exponents[a];
+    for (int pp = 1; pp <= 6; ++pp)
+      for (int a = 0; a < n_channels; ++a)
+        if (exponents[a] == pp) {
+          p->distinct_p.push_back(pp);
+          break;
+        }
+    for (int a = 0; a < n_channels; ++a)
+      for (size_t s = 0; s < p->distinct_p.size(); ++s)
+        if (p->distinct_p[s] == exponents[a]) p->chan_slot[a] = (int)s;
+
+    std::vector<double> invW2[3];
+    if (!rc) {
+      // window: psi_0^{c_w}, panel polynomials, W^ tables (Eq. (21)-(22))
+      Pswf0 psi_w(p->c_w);
+      p->wt = fit_window(psi_w, w, p->poly_eps, kMaxWindowDegree);
+      p->What0 = 1;
+      const double kc = c / p->r_c;
+      for (int d = 0; d < 3; ++d) {
+        const int M = p->M[d];
+        const double omega = 0.5 * w * p->h[d];
+        p->What0 *= omega * psi_w.lambda0;
+        invW2[d].assign(M, 0.0);
+        for (int i = 0; i < M; ++i) {
+          int f = i <= M / 2 ? i : i - M;
+          double kd = 2 * kPi * f / p->L[d];
+          double arg = omega * kd / p->c_w;  // = pi w f / (M c_w)
+          bool nyq = (M % 2 == 0) && i == M / 2;
+          if (std::fabs(kd) < kc && !nyq) {
+            if (std::fabs(arg) > 1.0) {
+              rc = PSWF_LR_ERR_GRID_TOO_COARSE;  // W^ needed outside its band
+              break;
+            }
+            double Wh = omega * psi_w.lambda0 * psi_w.eval(arg);
+            invW2[d][i] = 1.0 / (Wh * Wh);
+          }
+        }
+      }
+    }
+    if (!rc) {
+      // mollifier: psi_0^c, T_p tables, zero-mode constants
+      Pswf0 psi(c);
+      KernelMath km(psi);
+      const int panels = p->precision == PSWF_LR_F64 ? 32 : 16;
+      p->kt = fit_kernels(km, p->distinct_p, panels, p->poly_eps, kMaxKernelDegree);
+      for (int pp : p->distinct_p) p->Phi0.push_back(km.Phi0(pp, p->r_c));
+      // count modes in the ball (half spectrum), for info / roofline bytes
+      long long cnt = 0;
+      const double kc2 = (c / p->r_c) * (c / p->r_c);
+      for (int ix = 0; ix < p->M[0]; ++ix) {
+        int fx = ix <= p->M[0] / 2 ? ix : ix - p->M[0];
+        if ((p->M[0] % 2 == 0) && ix == p->M[0] / 2) continue;
+        double kx = 2 * kPi * fx / p->L[0];
+        for (int iy = 0; iy < p->M[1]; ++iy) {
+          int fy = iy <= p->M[1] / 2 ? iy : iy - p->M[1];
+          if ((p->M[1] % 2 == 0) && iy == p->M[1] / 2) continue;
+          double ky = 2 * kPi * fy / p->L[1];
+          double rem = kc2 - kx * kx - ky * ky;
+          if (rem <= 0) continue;
+          for (int iz = 0; iz <= p->M[2] / 2; ++iz) {
+            if ((p->M[2] % 2 == 0) && iz == p->M[2] / 2) continue;
+            double kz = 2 * kPi * iz / p->L[2];
+            if (kz * kz < rem) ++cnt;
+          }
+        }
+      }
+      p->modes_in_ball = cnt;
+    }
+    if (!rc && !p->host_only) {
+      long long b = 0;
+      if (p->precision == PSWF_LR_F64) {
+        rc |= upload<double>(&p->d_wcoef, p->wt.coef, &b);
+        rc |= upload<double>(&p->d_wdcoef, p->wt.dcoef, &b);
+        rc |= upload<double>(&p->d_kcoef, p->kt.coef, &b);
+        for (int d = 0; d < 3; ++d) rc |= upload<double>(&p->d_invW2[d], invW2[d], &b);
+      } else {
+        rc |= upload<float>(&p->d_wcoef, p->wt.coef, &b);
+        rc |= upload<float>(&p->d_wdcoef, p->wt.dcoef, &b);
+        rc |= upload<float>(&p->d_kcoef, p->kt.coef, &b);
+        for (int d = 0; d < 3; ++d) rc |= upload<float>(&p->d_invW2[d], invW2[d], &b);
+      }
+      const size_t rs = real_size(p);
+      const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
+      const size_t Mhalf = (size_t)p->M[0] * p->M[1] * (p->M[2] / 2 + 1);
+      if (!rc) rc = dev_alloc(&p->d_grid, rs * Mtot * p->C, &b);
+      if (!rc) rc = dev_alloc(&p->d_spec, 2 * rs * Mhalf * p->C, &b);
+      if (!rc) rc = dev_alloc((void**)&p->d_count, sizeof(int) * (Mtot + 1), &b);
+      p->n_scan_blocks = (int)((Mtot + 4095) / 4096);
+      if (!rc) rc = dev_alloc((void**)&p->d_blocksums, sizeof(int) * (size_t)p->n_scan_blocks, &b);
+      if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
+      if (!rc) rc = dev_alloc((void**)&p->d_Etot, sizeof(double), &b);
+      p->workspace_bytes += b;
+    }
+    if (!rc && !p->host_only) {
+      int n[3] = {p->M[0], p->M[1], p->M[2]};
+      const bool f64 = p->precision == PSWF_LR_F64;
+      size_t ws = 0;
+      if (cufftCreate(&p->fft_fwd) != CUFFT_SUCCESS || cufftCreate(&p->fft_inv) != CUFFT_SUCCESS)
+        rc = PSWF_LR_ERR_CUFFT;
+      p->have_fft = true;
+      if (!rc && cufftMakePlanMany(p->fft_fwd, 3, n, nullptr, 1, 0, nullptr, 1, 0, f64 ? CUFFT_D2Z : CUFFT_R2C,
+                                   p->C, &ws) != CUFFT_SUCCESS)
+        rc = PSWF_LR_ERR_CUFFT;
+      p->workspace_bytes += (long long)ws;
+      if (!rc && cufftMakePlanMany(p->fft_inv, 3, n, nullptr, 1, 0, nullptr, 1, 0, f64 ? CUFFT_Z2D : CUFFT_C2R,
+                                   p->C, &ws) != CUFFT_SUCCESS)
+        rc = PSWF_LR_ERR_CUFFT;
+      p->workspace_bytes += (long long)ws;
+    }
+    if (!rc && !p->host_only) rc = ensure_capacity(p, o.max_atoms > 0 ? o.max_atoms : 1024);
+  } catch (const std::bad_alloc&) {
+    rc = PSWF_LR_ERR_ALLOC;
+  } catch (...) {
+    rc = PSWF_LR_ERR_INVALID_ARG;
+  }
+  if (rc) {
+    pswf_lr_destroy(p);
+    return rc;
+  }
+  *plan = p;
+  return 0;
+}
+
+int pswf_lr_execute(pswf_lr_plan* p, int n_atoms, const void* pos, const void* q, void* E, void* phi, void* F,
+                    void* stream) {
+  if (!p || n_atoms < 0) return PSWF_LR_ERR_INVALID_ARG;
+  if (n_atoms > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;  // a tables-only plan cannot execute
+  int rc = ensure_capacity(p, n_atoms);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (p->precision == PSWF_LR_F64)
+    return execute_t<double>(p, n_atoms, (const double*)pos, (const double*)q, (double*)E, (double*)phi,
+                             (double*)F, st);
+  return execute_t<float>(p, n_atoms, (const float*)pos, (const float*)q, (double*)E, (float*)phi, (float*)F, st);
+}
+
+int pswf_lr_execute_host(pswf_lr_plan* p, int n, const void* pos, const void* q, double* E, void* phi, void* F,
+                         void* stream) {
+  if (!p || n < 0) return PSWF_LR_ERR_INVALID_ARG;
+  if (n > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  int rc = ensure_capacity(p, n);
+  if (rc) return rc;
+  rc = ensure_host_staging(p);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t rs = real_size(p);
+  if (n > 0) {
+    CUDA_TRY(cudaMemcpyAsync(p->d_pos_in, pos, rs * 3 * (size_t)n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(p->d_q_in, q, rs * (size_t)p->C * n, cudaMemcpyHostToDevice, st));
+  }
+  rc = pswf_lr_execute(p, n, p->d_pos_in, p->d_q_in, E ? p->d_Etot : nullptr, phi ? p->d_phi_out : nullptr,
+                       F ? p->d_F_out : nullptr, stream);
+  if (rc) return rc;
+  if (E) CUDA_TRY(cudaMemcpyAsync(E, p->d_Etot, sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (phi && n > 0)
+    CUDA_TRY(cudaMemcpyAsync(phi, p->d_phi_out, rs * (size_t)p->C * n, cudaMemcpyDeviceToHost, st));
+  if (F && n > 0) CUDA_TRY(cudaMemcpyAsync(F, p->d_F_out, rs * 3 * (size_t)n, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return 0;
+}
+
+int pswf_lr_channel_energies(pswf_lr_plan* p, void* E_channels, void* stream) {
+  if (!p || !E_channels) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  CUDA_TRY(cudaMemcpyAsync(E_channels, p->d_Ech, sizeof(double) * p->C, cudaMemcpyDeviceToDevice,
+                           (cudaStream_t)stream));
+  return 0;
+}
+
+int pswf_lr_get_info(const pswf_lr_plan* p, pswf_lr_info* info) {
+  if (!p || !info) return PSWF_LR_ERR_INVALID_ARG;
+  memset(info, 0, sizeof(*info));
+  info->r_c = p->r_c;
+  info->c = p->c;
+  info->c_window = p->c_w;
+  info->eta = p->eta;
+  info->w = p->w;
+  info->precision = p->precision;
+  info->n_channels = p->C;
+  info->n_distinct_p = (int)p->distinct_p.size();
+  for (int d = 0; d < 3; ++d) info->grid[d] = p->M[d];
+  info->window_degree = p->wt.degree;
+  info->kernel_degree = p->kt.degree;
+  info->kernel_panels = p->kt.panels;
+  info->modes_in_ball = p->modes_in_ball;
+  info->workspace_bytes = p->workspace_bytes;
+  return 0;
+}
+
+int pswf_lr_set_profiling(pswf_lr_plan* p, int enabled) {
+  if (!p) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  if (enabled && p->events.empty()) {
+    p->events.resize((size_t)kProfileRing * (PSWF_LR_N_STAGES + 1));
+    for (auto& e : p->events) CUDA_TRY(cudaEventCreate(&e));
+  }
+  p->profiling = enabled != 0;
+  p->prof_count = 0;
+  return 0;
+}
+
+int pswf_lr_stage_ms(pswf_lr_plan* p, double ms[PSWF_LR_N_STAGES], int* n_executes) {
+  if (!p || !ms) return PSWF_LR_ERR_INVALID_ARG;
+  for (int s = 0; s < PSWF_LR_N_STAGES; ++s) ms[s] = 0;
+  int n = p->prof_count;
+  if (n_executes) *n_executes = n;
+  if (n == 0) return 0;
+  cudaEvent_t* last = p->events.data() + (size_t)(n - 1) * (PSWF_LR_N_STAGES + 1);
+  CUDA_TRY(cudaEventSynchronize(last[PSWF_LR_N_STAGES]));
+  for (int i = 0; i < n; ++i) {
+    cudaEvent_t* ev = p->events.data() + (size_t)i * (PSWF_LR_N_STAGES + 1);
+    for (int s = 0; s < PSWF_LR_N_STAGES; ++s) {
+      float t = 0;
+      CUDA_TRY(cudaEventElapsedTime(&t, ev[s], ev[s + 1]));
+      ms[s] += t;
+    }
+  }
+  for (int s = 0; s < PSWF_LR_N_STAGES; ++s) ms[s] /= n;
+  p->prof_count = 0;
+  return 0;
+}
+
+int pswf_lr_debug_copy(pswf_lr_plan* p, int what, void* dst, void* stream) {
+  if (!p || !dst) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  const size_t rs = real_size(p);
+  const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
+  const size_t Mhalf = (size_t)p->M[0] * p->M[1] * (p->M[2] / 2 + 1);
+  const void* src = nullptr;
+  size_t nb = 0;
+  if (what == 0 || what == 2) {
+    src = p->d_grid;
+    nb = rs * Mtot * p->C;
+  } else if (what == 1) {
+    src = p->d_spec;
+    nb = 2 * rs * Mhalf * p->C;
+  } else {
+    return PSWF_LR_ERR_INVALID_ARG;
+  }
+  CUDA_TRY(cudaMemcpyAsync(dst, src, nb, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return 0;
+}
+
+int pswf_lr_eval_window(const pswf_lr_plan* p, int n, const double* z, double* W, double* dW) {
+  if (!p || n < 0 || (n > 0 && (!z || !W))) return PSWF_LR_ERR_INVALID_ARG;
+  const int w = p->w, deg = p->wt.degree;
+  for (int i = 0; i < n; ++i) {
+    double s = 0.5 * w * (z[i] + 1.0);  // t + delta
+    int t = (int)std::floor(s);
+    if (t < 0 || t >= w) {
+      W[i] = 0;
+      if (dW) dW[i] = 0;
+      continue;
+    }
+    double xi = 2 * (s - t) - 1;
+    double v = p->wt.coef[(size_t)deg * w + t];
+    for (int m = deg - 1; m >= 0; --m) v = v * xi + p->wt.coef[(size_t)m * w + t];
+    W[i] = v;
+    if (dW) {
+      double dv = p->wt.dcoef[(size_t)(deg - 1) * w + t];
+      for (int m = deg - 2; m >= 0; --m) dv = dv * xi + p->wt.dcoef[(size_t)m * w + t];
+      dW[i] = dv * w;  // d xi / d z = w
+    }
+  }
+  return 0;
+}
+
+int pswf_lr_eval_kernel(const pswf_lr_plan* p, int pe, int n, const double* k, double* Phi) {
+  if (!p || n < 0 || (n > 0 && (!k || !Phi))) return PSWF_LR_ERR_INVALID_ARG;
+  int slot = -1;
+  for (size_t s = 0; s < p->distinct_p.size(); ++s)
+    if (p->distinct_p[s] == pe) slot = (int)s;
+  if (slot < 0) return PSWF_LR_ERR_UNSUPPORTED_EXPONENT;
+  const int deg = p->kt.degree, panels = p->kt.panels;
+  for (int i = 0; i < n; ++i) {
+    double kappa = k[i] * p->r_c, x = kappa / p->c;
+    if (!(x > 0) || x >= 1) {
+      Phi[i] = 0;
+      continue;
+    }
+    int j = std::min((int)(x * panels), panels - 1);
+    double xi = 2 * (x * panels - j) - 1;
+    const double* cf = &p->kt.coef[((size_t)slot * panels + j) * (deg + 1)];
+    double t = cf[deg];
+    for (int m = deg - 1; m >= 0; --m) t = t * xi + cf[m];
+    double s;
+    switch (pe) {
+      case 1: s = t / (kappa * kappa); break;
+      case 2: s = t / kappa; break;
+      case 3: s = t - std::log(x); break;
+      case 5: s = t + x * x * std::log(x); break;
+      default: s = t; break;
+    }
+    Phi[i] = s * slot_prefactor(pe, p->c, p->r_c);
+  }
+  return 0;
+}
+
+int pswf_lr_destroy(pswf_lr_plan* p) {
+  if (!p) return 0;
+  if (p->host_only) {
+    delete p;
+    return 0;
+  }
+  cudaDeviceSynchronize();
+  free_atoms(p);
+  void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
+                  p->d_grid,  p->d_spec,    p->d_count,    p->d_blocksums, p->d_Ech,      p->d_Etot};
+  for (void* q : ptrs)
+    if (q) cudaFree(q);
+  if (p->have_fft) {
+    if (p->fft_fwd) cufftDestroy(p->fft_fwd);
+    if (p->fft_inv) cufftDestroy(p->fft_inv);
+  }
+  for (auto& e : p->events) cudaEventDestroy(e);
+  delete p;
+  return 0;
+}
+
+}  // extern "C"

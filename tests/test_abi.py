@@ -1,0 +1,139 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/pswf_lr.h declares,
+validates arguments, refuses to compute without a device (no CPU fallback), and its host-side
+tables (window and kernel Horner polynomials, resolved defaults) agree with the oracle.
+No compute call is made here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import gridded as G
+from oracle.kernels import Mollifier
+from oracle.pswf import PSWF0
+from paper_2606_06617_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    build.build()
+
+
+def test_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "pswf_lr.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(pswf_lr_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(binding.EXPORTS)
+    L = ctypes.CDLL(binding.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert b"sm_100a" in binding.lib().pswf_lr_version()
+
+
+def test_argument_validation_codes():
+    ok = dict(box=[10.0] * 3, grid=[16] * 3, w=6, c=12.024, exponents=[1], host_only=True)
+
+    def code(**kw):
+        args = dict(ok)
+        args.update(kw)
+        try:
+            binding.Plan(**args).destroy()
+            return 0
+        except binding.PswfLrError as e:
+            return e.code
+    assert code() == 0
+    assert code(w=7) == binding.ERR_INVALID_ARG
+    assert code(w=18) == binding.ERR_INVALID_ARG
+    assert code(c=1.0) == binding.ERR_INVALID_ARG
+    assert code(box=[10.0, -1.0, 10.0]) == binding.ERR_INVALID_ARG
+    assert code(exponents=[7]) == binding.ERR_UNSUPPORTED_EXPONENT
+    assert code(exponents=[0]) == binding.ERR_UNSUPPORTED_EXPONENT
+    assert code(grid=[16, 4, 16]) == binding.ERR_GRID_TOO_COARSE          # w > M_d
+    assert code(r_c=2.0) == binding.ERR_GRID_TOO_COARSE                   # eta = 1.2 > 1, Eq. (29)
+    assert code(w=16, c_window=5.0, r_c=2.5) == binding.ERR_GRID_TOO_COARSE  # W^ outside its band
+    assert code(exponents=[1] * 33) == binding.ERR_INVALID_ARG
+    assert "exponent" in binding.lib().pswf_lr_error_string(-2).decode()
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks behaviour on a box without a GPU")
+def test_no_cpu_fallback_without_device():
+    with pytest.raises(binding.PswfLrError) as e:
+        binding.Plan([10.0] * 3, [16] * 3, 6, 12.024, [1])
+    assert e.value.code == binding.ERR_CUDA
+    # a tables-only plan exists but cannot compute
+    p = binding.Plan([10.0] * 3, [16] * 3, 6, 12.024, [1], host_only=True)
+    with pytest.raises(binding.PswfLrError) as e:
+        p.execute(0, None, None)
+    assert e.value.code == binding.ERR_CUDA
+    with pytest.raises(binding.PswfLrError):
+        p.set_profiling(True)
+
+
+def test_resolved_defaults_match_readings():
+    """Readings R2 (eta = 0.5) and R3 (c_w = w (3.55 - 1.55 eta)); SURVEY.md §8(c) quotes r_c = 4.78 A
+    and c_w = 16.65 for config 1."""
+    p = binding.Plan([10.0] * 3, [16] * 3, 6, 12.024, [1], host_only=True)
+    i = p.info()
+    assert i["r_c"] == pytest.approx(G.default_r_c([10.0] * 3, [16] * 3, 12.024), rel=1e-14)
+    assert i["r_c"] == pytest.approx(4.78, abs=5e-3)
+    assert i["eta"] == pytest.approx(0.5, rel=1e-12)
+    assert i["c_window"] == pytest.approx(G.default_c_w(6), rel=1e-14)
+    assert i["c_window"] == pytest.approx(16.65, abs=1e-9)
+    # half-spectrum modes (m_z >= 0) inside the ball |k| r_c < c, the m = 0 mode included
+    m = np.array([[a, b, c] for a in range(-7, 8) for b in range(-7, 8) for c in range(0, 8)])
+    inside = ((2 * np.pi * m / 10.0) ** 2).sum(1) ** 0.5 * i["r_c"] < 12.024
+    assert i["modes_in_ball"] == int(inside.sum())
+
+
+@pytest.mark.parametrize("precision,w,tol", [("f32", 6, 3e-7), ("f32", 8, 3e-7), ("f64", 6, 5e-14),
+                                             ("f64", 16, 5e-14)])
+def test_window_tables_match_oracle_pswf(precision, w, tol):
+    """Panel polynomials vs the Legendre-series psi_0^{c_w} of the oracle."""
+    p = binding.Plan([10.0] * 3, [32] * 3, w, 12.024, [1], precision=precision, host_only=True)
+    i = p.info()
+    psi = PSWF0(i["c_window"])
+    z = np.linspace(-1, 1, 4001)[:-1]
+    W, dW = p.eval_window(z)
+    assert np.max(np.abs(W - psi(z))) < tol
+    # derivative of the same polynomial; in f64 the comparison is limited to ~2e-11
+    # by the differentiated series on both sides (error budget)
+    assert np.max(np.abs(dW - psi.deriv(z, 1))) < (tol * 60 if precision == "f32" else 1e-10)
+    assert 4 <= i["window_degree"] <= (12 if precision == "f32" else 20)
+    assert np.all(p.eval_window(np.array([-1.2, 1.0, 3.0]))[0] == 0.0)
+
+
+@pytest.mark.parametrize("precision,tol", [("f32", 2e-7), ("f64", 2e-13)])
+def test_kernel_tables_match_oracle_theorem1(precision, tol):
+    """Phi^_p(k) from 'bare transform + smooth Horner part' vs oracle Theorem-1 quadratures."""
+    p = binding.Plan([31.0] * 3, [32] * 3, 6, 12.024, [1, 2, 3, 4, 5, 6], precision=precision,
+                     host_only=True)
+    i = p.info()
+    moll = Mollifier(i["c"], i["r_c"])
+    kc = i["c"] / i["r_c"]
+    k = np.concatenate([np.linspace(2 * np.pi / 31.0, kc * 0.9999, 300), [kc * 0.25, kc * 1.0001, 2 * kc]])
+    for pe in range(1, 7):
+        got = p.eval_kernel(pe, k)
+        ref = moll.Phi_hat(pe, k)
+        # error relative to the kernel's size at the smallest k of the box
+        scale = np.abs(ref).max()
+        assert np.max(np.abs(got - ref)) < tol * scale, pe
+        assert got[-1] == 0.0 and got[-2] == 0.0
+
+
+def test_workloads_are_seeded_and_shaped():
+    from paper_2606_06617_b200 import workloads
+    a, b = workloads.make(2), workloads.make(2)
+    assert np.array_equal(a["pos"], b["pos"]) and np.array_equal(a["q"], b["q"])
+    assert a["pos"].shape == (3000, 3) and a["q"].shape == (2, 3000)
+    assert abs(a["q"][0].sum()) < 1e-4                       # neutral water charges
+    d = np.linalg.norm(a["pos"][1] - a["pos"][0])
+    assert min(d, abs(d - 31.0)) == pytest.approx(0.96, abs=1e-4) or d > 15   # O-H bond (mod wrap)
+    c3 = workloads.make(3, n_atoms=500)
+    assert c3["q"].shape == (8, 500) and np.abs(c3["q"].sum(1)).max() < 1e-4
+    c5 = workloads.make(5, n_atoms=1000)
+    assert c5["pos"][:, 2].min() >= 100.0 and c5["pos"][:, 2].max() < 200.0
+    assert np.all(a["pos"].astype(np.float32).astype(np.float64) == a["pos"])

@@ -1,0 +1,325 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Tolerances are north_star's: fp32 relative energy error <= 1e-5, relative
+force RMS <= 1e-4 (against oracle A, the direct k-sum); fp64 <= 1e-10 (against oracle B at the
+specified w, and against oracle A at w = 16 -- DESIGN.md reading R1).  Error definitions are the
+paper's (S80)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import gridded as G
+from oracle.direct import direct_sums, direct_sums_c
+from paper_2606_06617_b200 import binding, workloads
+from gpu_util import make_plan, rel, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+TOL_E32, TOL_F32 = 1e-5, 1e-4
+TOL_64 = 1e-10
+
+
+def oracle_A(wl, r_c, subset=None):
+    fn = direct_sums if len(wl["pos"]) <= 200 else direct_sums_c
+    return fn(wl["pos"], wl["q"], wl["exponents"], wl["box"], wl["c"], r_c, grid=wl["grid"], subset=subset)
+
+
+def check_vs(out, ref, tolE, tolF, subset=None, label=""):
+    E, Ech, phi, F = ref
+    gphi, gF = out["phi"], out["F"]
+    if subset is not None:
+        gphi, gF = gphi[:, subset], gF[subset]
+    eE = abs(out["E"] - E) / abs(E)
+    eF = rel(gF, F)
+    ephi = max(rel(gphi[a], phi[a]) for a in range(len(phi)))
+    ech = np.max(np.abs(out["E_channels"] - Ech) / np.abs(E))
+    print("%s eps_E=%.3e eps_F=%.3e eps_phi=%.3e eps_Ech=%.3e" % (label, eE, eF, ephi, ech))
+    assert eE <= tolE, (label, eE)
+    assert ech <= tolE, (label, ech)
+    assert eF <= tolF, (label, eF)
+    assert ephi <= tolF, (label, ephi)
+
+
+# ---- config 1: fp64 ---------------------------------------------------------------------------
+
+@pytest.mark.parametrize("kernel_path", [0, 1])
+def test_cfg1_fp64_vs_oracle_B(kernel_path):
+    """Gate (i): fp64 GPU equals the same discretisation computed on the CPU to 1e-10."""
+    wl = workloads.make(1)
+    out = run_gpu(wl, kernel_path=kernel_path)
+    i = out["info"]
+    ref = G.gridded(wl["pos"], wl["q"], wl["exponents"], wl["box"], wl["grid"], wl["w"], wl["c"],
+                    i["r_c"], i["c_window"])
+    check_vs(out, ref, TOL_64, TOL_64, label="cfg1 f64 vs B")
+
+
+def test_cfg1_fp64_w16_vs_oracle_A():
+    """Gate (ii): with a window wide enough to remove aliasing (w = 16) the fp64 GPU result equals the
+    DEFINITION (direct k-sum) to 1e-10."""
+    wl = workloads.make(1)
+    wl["w"] = 16
+    out = run_gpu(wl)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), TOL_64, TOL_64, label="cfg1 f64 w16 vs A")
+
+
+def test_cfg1_fp32_vs_oracle_A():
+    wl = workloads.make(1)
+    wl["precision"] = "f32"
+    wl["pos"] = wl["pos"].astype(np.float32).astype(np.float64)
+    out = run_gpu(wl)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), TOL_E32, TOL_F32, label="cfg1 f32 vs A")
+
+
+def test_all_exponents_fp64_vs_oracle_A():
+    """p = 1..6 with charged channels (every zero-mode convention), non-cubic box, odd grid sizes."""
+    rng = np.random.default_rng(77)
+    box, grid = [11.0, 12.5, 10.0], [18, 21, 16]
+    N = 50
+    wl = dict(pos=rng.uniform(0, 1, (N, 3)) * box, q=rng.normal(0, 0.5, (6, N)), exponents=[1, 2, 3, 4, 5, 6],
+              box=box, grid=grid, w=16, c=12.024, precision="f64")
+    out = run_gpu(wl)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), 1e-9, 1e-9, label="p=1..6 f64 vs A")
+
+
+# ---- configs 2, 3, 5: fp32 vs the definition ---------------------------------------------------
+
+@pytest.mark.parametrize("kernel_path", [0, 1])
+def test_cfg2_fp32_vs_oracle_A(kernel_path):
+    wl = workloads.make(2)
+    out = run_gpu(wl, kernel_path=kernel_path)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), TOL_E32, TOL_F32, label="cfg2 f32 vs A path%d" % kernel_path)
+
+
+@pytest.mark.parametrize("kernel_path", [0, 1])
+def test_cfg3_fp32_vs_oracle_A(kernel_path):
+    wl = workloads.make(3)
+    out = run_gpu(wl, kernel_path=kernel_path)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), TOL_E32, TOL_F32, label="cfg3 f32 vs A path%d" % kernel_path)
+
+
+def test_cfg5_slab_fp32_vs_oracle_A():
+    """Anisotropic box, two thirds vacuum.  The oracle evaluates E over all 200,000 atoms and phi/F on
+    a seeded sample of 2,000 atoms (outputs it can compute one by one)."""
+    wl = workloads.make(5)
+    out = run_gpu(wl)
+    sub = np.sort(np.random.default_rng(5).choice(len(wl["pos"]), 2000, replace=False))
+    check_vs(out, oracle_A(wl, out["info"]["r_c"], subset=sub), TOL_E32, TOL_F32, subset=sub,
+             label="cfg5 f32 vs A")
+
+
+@pytest.mark.slow
+def test_cfg4_full_size_fp32_vs_oracle_A():
+    """BASELINE.json's headline configuration at FULL size (N = 1,000,000, 128^3, w = 8, 4 channels),
+    same plan parameters bench.py times.  rho(k) runs over all atoms (6.9e10 atom-mode pairs); phi
+    and F are compared on a seeded sample of 1,000 atoms."""
+    wl = workloads.make(4)
+    out = run_gpu(wl)
+    sub = np.sort(np.random.default_rng(4).choice(len(wl["pos"]), 1000, replace=False))
+    check_vs(out, oracle_A(wl, out["info"]["r_c"], subset=sub), TOL_E32, TOL_F32, subset=sub,
+             label="cfg4 f32 vs A (full size)")
+    # properties that hold at any size
+    Fn = out["F"]
+    assert np.abs(Fn.sum(0)).max() < 1e-3 * np.sqrt((Fn ** 2).sum())     # net force at aliasing level
+    E_gather = 0.5 * float(np.sum(wl["q"] * out["phi"]))
+    assert abs(E_gather - out["E"]) < 2e-6 * abs(out["E"])               # Eq. (26) == 1/2 sum q phi
+
+
+def test_cfg4_shape_reduced_fp32_vs_oracle_A():
+    """Config 4's box/grid/channels with 60,000 atoms (seconds of oracle time)."""
+    wl = workloads.make(4, n_atoms=60000)
+    out = run_gpu(wl)
+    sub = np.arange(0, 60000, 30)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"], subset=sub), TOL_E32, TOL_F32, subset=sub,
+             label="cfg4-shape 60k f32 vs A")
+
+
+# ---- per-kernel parity against oracle B's intermediate arrays ----------------------------------
+
+@pytest.mark.parametrize("precision,tol", [("f64", 1e-12), ("f32", 2e-6)])
+def test_intermediates_vs_oracle_B(precision, tol):
+    wl = workloads.make(2, n_atoms=600)
+    wl["precision"] = precision
+    wl["grid"] = [20, 24, 16]
+    plan = make_plan(wl)
+    i = plan.info()
+    dev = torch.device("cuda:0")
+    dt = torch.float64 if precision == "f64" else torch.float32
+    ref = G.gridded(wl["pos"], wl["q"], wl["exponents"], wl["box"], wl["grid"], wl["w"], wl["c"], i["r_c"],
+                    i["c_window"], intermediates=True)[4]
+    M = wl["grid"]
+    # energy-only execute keeps the real grid after spreading and the scaled spectrum
+    run_gpu(wl, plan=plan, want=("E",))
+    rho = torch.empty((2, *M), dtype=dt, device=dev)
+    plan.debug_copy(0, rho)
+    spec = torch.empty((2, M[0], M[1], M[2] // 2 + 1, 2), dtype=dt, device=dev)
+    plan.debug_copy(1, spec)
+    torch.cuda.synchronize()
+    assert rel(rho.cpu().numpy(), ref["rho"]) < tol
+    sc = ref["scaled"][..., : M[2] // 2 + 1]
+    # cuFFT's forward sign is e^{-i}, numpy's too: same convention, compare directly
+    got = spec.cpu().numpy()[..., 0] + 1j * spec.cpu().numpy()[..., 1]
+    assert np.linalg.norm(got - sc) / np.linalg.norm(sc) < 5 * tol
+    out = run_gpu(wl, plan=plan)
+    phig = torch.empty((2, *M), dtype=dt, device=dev)
+    plan.debug_copy(2, phig)
+    torch.cuda.synchronize()
+    assert rel(phig.cpu().numpy(), ref["phig"]) < 5 * tol
+    assert np.allclose(out["E_channels"], ref["E_spec"], rtol=10 * tol)
+    plan.destroy()
+
+
+# ---- edge cases --------------------------------------------------------------------------------
+
+def test_empty_input_is_legal():
+    wl = workloads.make(1)
+    plan = make_plan(wl)
+    dev = torch.device("cuda:0")
+    E = torch.full((1,), float("nan"), dtype=torch.float64, device=dev)
+    plan.execute(0, None, None, E, None, None, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert E.item() == 0.0
+    out = run_gpu(wl, plan=plan)       # the plan still works afterwards
+    assert np.isfinite(out["E"])
+    plan.destroy()
+
+
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_boundary_positions_and_wrapping(precision):
+    """Atoms exactly on grid points, at 0 and (numerically) at L, far outside the box, and many
+    atoms in one cell: GPU vs oracle B on the wrapped positions; images give identical results."""
+    rng = np.random.default_rng(9)
+    box, grid, w = [10.0, 12.0, 8.0], [16, 20, 12], 6
+    h = np.array(box) / np.array(grid)
+    pos = np.concatenate([
+        np.array([[0.0, 0.0, 0.0], [h[0] * 3, h[1] * 7, h[2] * 11], [np.nextafter(10.0, 0), 0.5, 7.999999],
+                  [5.0, 6.0, 4.0]]),
+        np.array([2.2, 3.3, 4.4]) + rng.uniform(0, 1, (20, 3)) * h,      # 20 atoms in one cell
+        rng.uniform(0, 1, (8, 3)) * box])
+    if precision == "f32":
+        pos = pos.astype(np.float32).astype(np.float64)
+    q = rng.normal(0, 1, (2, len(pos)))
+    wl = dict(pos=pos, q=q, exponents=[1, 4], box=box, grid=grid, w=w, c=12.024, precision=precision)
+    plan = make_plan(wl)
+    i = plan.info()
+    out = run_gpu(wl, plan=plan)
+    ref = G.gridded(pos, q, wl["exponents"], box, grid, w, wl["c"], i["r_c"], i["c_window"])
+    tol = 1e-10 if precision == "f64" else 2e-5
+    check_vs(out, ref, tol, tol, label="boundary %s" % precision)
+    if precision == "f64":
+        shifted = pos + np.array(box) * rng.integers(-3, 4, size=pos.shape)
+        out2 = run_gpu(wl, plan=plan, pos=shifted)
+        assert abs(out2["E"] - out["E"]) < 1e-10 * abs(out["E"])
+        assert rel(out2["F"], out["F"]) < 1e-9
+    plan.destroy()
+
+
+@pytest.mark.parametrize("w,grid", [(4, [16, 16, 16]), (6, [15, 17, 21]), (8, [24, 16, 40]), (10, [20, 20, 20]),
+                                    (12, [16, 16, 16])])
+def test_window_widths_and_ragged_grids_fp32(w, grid):
+    """Several window widths, odd / non-multiple-of-tile grid sizes, fast path vs reference path vs B."""
+    rng = np.random.default_rng(w)
+    box = [13.0, 14.0, 16.0]
+    N = 700
+    pos = (rng.uniform(0, 1, (N, 3)) * box).astype(np.float32).astype(np.float64)
+    q = rng.normal(0, 0.5, (3, N)).astype(np.float32).astype(np.float64)
+    wl = dict(pos=pos, q=q, exponents=[1, 3, 6], box=box, grid=grid, w=w, c=12.024, precision="f32")
+    a = run_gpu(wl, kernel_path=0)
+    b = run_gpu(wl, kernel_path=1)
+    i = a["info"]
+    ref = G.gridded(pos, q, wl["exponents"], box, grid, w, wl["c"], i["r_c"], i["c_window"])
+    check_vs(a, ref, 5e-6, 2e-5, label="w=%d fast vs B" % w)
+    check_vs(b, ref, 5e-6, 2e-5, label="w=%d ref vs B" % w)
+
+
+@pytest.mark.parametrize("C", [1, 2, 3, 5, 8, 11])
+def test_channel_counts_fp32(C):
+    rng = np.random.default_rng(C)
+    box, grid = [12.0] * 3, [24] * 3
+    N = 500
+    pos = (rng.uniform(0, 12, (N, 3))).astype(np.float32).astype(np.float64)
+    q = rng.normal(0, 0.5, (C, N)).astype(np.float32).astype(np.float64)
+    ex = [(1, 6, 3, 2, 4, 5)[a % 6] for a in range(C)]
+    wl = dict(pos=pos, q=q, exponents=ex, box=box, grid=grid, w=8, c=12.024, precision="f32")
+    out = run_gpu(wl)
+    i = out["info"]
+    ref = G.gridded(pos, q, ex, box, grid, 8, wl["c"], i["r_c"], i["c_window"])
+    check_vs(out, ref, 5e-6, 2e-5, label="C=%d" % C)
+
+
+def test_energy_only_path_and_repeatability():
+    wl = workloads.make(2)
+    plan = make_plan(wl)
+    full = run_gpu(wl, plan=plan)
+    eo = run_gpu(wl, plan=plan, want=("E",))
+    assert abs(eo["E"] - full["E"]) < 2e-6 * abs(full["E"])     # fp32 atomics: order may differ
+    again = run_gpu(wl, plan=plan)
+    assert abs(again["E"] - full["E"]) < 2e-6 * abs(full["E"])
+    assert rel(again["F"], full["F"]) < 1e-5
+    plan.destroy()
+
+
+def test_execute_host_matches_execute():
+    wl = workloads.make(2)
+    plan = make_plan(wl)
+    dev_out = run_gpu(wl, plan=plan)
+    n, C = len(wl["pos"]), 2
+    pos = torch.as_tensor(wl["pos"], dtype=torch.float32).pin_memory()
+    q = torch.as_tensor(wl["q"], dtype=torch.float32).pin_memory()
+    E = torch.zeros(1, dtype=torch.float64).pin_memory()
+    phi = torch.zeros((C, n), dtype=torch.float32).pin_memory()
+    F = torch.zeros((n, 3), dtype=torch.float32).pin_memory()
+    plan.execute_host(n, pos, q, E, phi, F, torch.cuda.current_stream().cuda_stream)
+    assert abs(E.item() - dev_out["E"]) < 2e-6 * abs(dev_out["E"])
+    assert rel(F.double().numpy(), dev_out["F"]) < 1e-5
+    assert rel(phi.double().numpy(), dev_out["phi"]) < 1e-5
+    plan.destroy()
+
+
+def test_capacity_growth_and_plan_reuse():
+    small = workloads.make(2, n_atoms=300)
+    big = workloads.make(2)
+    plan = make_plan(big, max_atoms=16)
+    a = run_gpu(small, plan=plan)
+    b = run_gpu(big, plan=plan)
+    c = run_gpu(small, plan=plan)
+    assert abs(a["E"] - c["E"]) < 2e-6 * abs(a["E"])
+    ref = run_gpu(big)
+    assert abs(b["E"] - ref["E"]) < 2e-6 * abs(ref["E"])
+    plan.destroy()
+
+
+def test_gridded_invariants_on_gpu():
+    """Forces are the gradient of the discrete energy (central differences through the GPU path, fp64),
+    net force and translation invariance at the aliasing level (reading R12)."""
+    wl = workloads.make(1)
+    plan = make_plan(wl)
+    out = run_gpu(wl, plan=plan)
+    hh = 1e-5
+    for i, d in ((3, 0), (40, 2)):
+        pp, pm = wl["pos"].copy(), wl["pos"].copy()
+        pp[i, d] += hh
+        pm[i, d] -= hh
+        fd = -(run_gpu(wl, plan=plan, pos=pp, want=("E",))["E"] - run_gpu(wl, plan=plan, pos=pm, want=("E",))["E"]) / (2 * hh)
+        assert abs(fd - out["F"][i, d]) < 2e-8 * np.abs(out["F"]).max()
+    assert abs(0.5 * np.sum(wl["q"] * out["phi"]) - out["E"]) < 1e-12 * abs(out["E"])
+    E2 = run_gpu(wl, plan=plan, pos=wl["pos"] + np.array([0.21, -0.4, 0.13]), want=("E",))["E"]
+    assert abs(E2 - out["E"]) < 1e-5 * abs(out["E"])
+    plan.destroy()
+
+
+def test_zero_mode_option():
+    wl = workloads.make(2)           # the p = 6 channel has Q_net != 0
+    a = run_gpu(wl)
+    b = run_gpu(wl, zero_mode=1)
+    i = a["info"]
+    from oracle.kernels import Mollifier
+    V = float(np.prod(wl["box"]))
+    E0 = Mollifier(i["c"], i["r_c"]).Phi0(6) * wl["q"][1].sum() ** 2 / (2 * V)
+    assert abs((a["E_channels"][1] - b["E_channels"][1]) - E0) < 1e-5 * abs(E0)
+    assert abs(a["E_channels"][0] - b["E_channels"][0]) < 1e-6 * abs(a["E_channels"][0])
+
+
+def test_native_library_is_loaded():
+    """The product path is the CUDA library: the shared object is mapped into this process."""
+    binding.lib()
+    maps = open("/proc/self/maps").read()
+    assert "libpswf_lr.so" in maps and "libcufft" in maps
