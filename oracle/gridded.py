@@ -9,7 +9,8 @@ PAPER.md:76, 1099).  The window is evaluated from the Legendre series of psi_0^{
 
   R3  the window bandwidth c_w is a parameter separate from the mollifier's c;
   R4  u = r_d/h_d with r wrapped into [0,L); i0 = ceil(u - w/2); the atom touches grid points
-      i0 .. i0+w-1 (mod M_d); window argument z_t = (i0 + t - u)/(w/2) in [-1, 1);
+      i0 .. i0+w-1 (mod M_d); window argument z_t = (i0 + t - u)/(w/2) in [-1, 1) (the order of the
+      float64 operations that decide i0 is fixed in stencil());
   R10 D_p(m) = (h_x h_y h_z / M_tot) Phi^_p(|k_m|) / W^(k_m)^2 with unnormalised forward and
       inverse DFTs, so that 1/2 sum_m D |rho^|^2 = 1/2 sum_i q_i phi_i;
   R11 multiplier zero on Nyquist planes and for |k| r_c >= c; the m = 0 entry carries the
@@ -21,17 +22,24 @@ from .kernels import Mollifier
 
 
 def stencil(pos, box, grid, w):
-    """(i0 (N,3) int, z (N,3,w) float): first grid index and window arguments (reading R4)."""
+    """(i0 (N,3) int, z (N,3,w) float): first grid index and window arguments (reading R4).
+
+    R4 fixes the arithmetic that decides the integer i0 (so that the oracle and the kernel take
+    the same decision for atoms sitting exactly on a grid point): s = x * (1/L); s -= floor(s);
+    u' = s * M - w/2;  i0 = ceil(u');  delta = i0 - u';  z_t = (t + delta) / (w/2) - 1, each
+    operation rounded to float64 separately."""
     pos = np.asarray(pos, dtype=np.float64)
     box = np.asarray(box, dtype=np.float64)
     grid = np.asarray(grid)
-    h = box / grid
-    r = pos - np.floor(pos / box) * box           # wrap into [0, L)
-    r = np.where(r >= box, 0.0, r)                # guard the rounding case r == L
-    u = r / h
-    i0 = np.ceil(u - w / 2.0).astype(np.int64)
+    s = pos * (1.0 / box)
+    s = s - np.floor(s)                           # wrap into [0, 1)
+    s = np.where(s >= 1.0, 0.0, s)                # guard the rounding case s == 1
+    u = s * grid.astype(np.float64) - w / 2.0
+    cu = np.ceil(u)
+    i0 = cu.astype(np.int64)
+    delta = cu - u                                # in [0, 1)
     t = np.arange(w)
-    z = (i0[:, :, None] + t[None, None, :] - u[:, :, None]) / (w / 2.0)
+    z = (t[None, None, :] + delta[:, :, None]) / (w / 2.0) - 1.0
     return i0, z
 
 

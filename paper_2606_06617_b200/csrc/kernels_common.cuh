@@ -11,13 +11,15 @@ namespace pswf {
 // window argument of point t is z_t = 2 (t + delta) / w - 1.  Done in double for both precisions
 // so that no bits of the in-cell offset are lost at u ~ M (a handful of DP ops per atom).
 __device__ __forceinline__ void stencil_1d(double x, double invL, int M, int w, int& i0, double& delta) {
-  double s = x * invL;
-  s -= floor(s);
+  // explicit _rn intrinsics: no FMA contraction, so the integer decision i0 = ceil(u) is taken
+  // with exactly the roundings DESIGN.md reading R4 states (and the oracle reproduces)
+  double s = __dmul_rn(x, invL);
+  s = __dsub_rn(s, floor(s));
   if (s >= 1.0) s = 0.0;
-  double u = s * (double)M - 0.5 * (double)w;
+  double u = __dsub_rn(__dmul_rn(s, (double)M), 0.5 * (double)w);
   double cu = ceil(u);
   i0 = (int)cu;
-  delta = cu - u;
+  delta = __dsub_rn(cu, u);
 }
 
 __device__ __forceinline__ int wrap_index(int i, int M) {

@@ -76,6 +76,7 @@ struct pswf_lr_plan {
   void* d_spec = nullptr;         // cplx  [C][Mx][My][Mz/2+1]
   int* d_count = nullptr;         // [Mtot + 1] cell counts -> exclusive starts
   int* d_blocksums = nullptr;
+  int* d_colcount = nullptr;      // [My*Mz] atoms per stencil-cell column (fast gather)
   int n_scan_blocks = 0;
   double* d_Ech = nullptr;        // [C]
   double* d_Etot = nullptr;       // [1] (execute_host staging)
