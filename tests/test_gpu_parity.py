@@ -212,7 +212,7 @@ def test_boundary_positions_and_wrapping(precision):
     plan.destroy()
 
 
-@pytest.mark.parametrize("w,grid", [(4, [16, 16, 16]), (6, [15, 17, 21]), (8, [24, 16, 40]), (10, [20, 20, 20]),
+@pytest.mark.parametrize("w,grid", [(4, [16, 16, 16]), (6, [15, 17, 21]), (8, [24, 16, 40]), (8, [24, 40, 56]), (8, [32, 28, 24]), (10, [20, 20, 20]),
                                     (12, [16, 16, 16])])
 def test_window_widths_and_ragged_grids_fp32(w, grid):
     """Several window widths, odd / non-multiple-of-tile grid sizes, fast path vs reference path vs B."""
