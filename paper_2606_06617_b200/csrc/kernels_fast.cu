@@ -29,34 +29,8 @@ namespace {
 constexpr int FW = 8;     // window width handled by the fast path
 constexpr int PY = 4;     // patch rows (y) per warp
 constexpr int PZ = 8;     // patch columns (z) per warp, contiguous in memory
-constexpr int SPREAD_TX = 32;
 constexpr int GATHER_TX = 32;
 
-__host__ __device__ inline int rec_floats(int C) { return 3 * FW + 4 + ((C + 3) / 4) * 4; }
-
-// ------------------------------------------------------------------------------------------------
-// records: one warp per atom, lane t writes float t of the record (coalesced 128 B stores)
-// ------------------------------------------------------------------------------------------------
-__global__ void k_fast_records(int n, int C, int cap, int recf, GridGeom<float> g, const int* __restrict__ si0,
-                               const float* __restrict__ sdelta, const float* __restrict__ sq,
-                               float* __restrict__ rec) {
-  const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  if (j >= n) return;
-  for (int t = lane; t < recf; t += 32) {
-    float v = 0.f;
-    if (t < 3 * FW) {
-      int d = t / FW, tt = t - d * FW;
-      float xi = 2.f * sdelta[(size_t)d * cap + j] - 1.f;
-      v = horner_panel(g.wcoef, FW, tt, g.wdeg, xi);
-    } else if (t == 3 * FW) {
-      v = __int_as_float(wrap_index(si0[2 * (size_t)cap + j], g.M[2]));
-    } else if (t >= 3 * FW + 4 && t < 3 * FW + 4 + C) {
-      v = sq[(size_t)(t - 3 * FW - 4) * cap + j];
-    }
-    rec[(size_t)j * recf + t] = v;
-  }
-}
 
 // occupancy of each (s_y, s_z) column of stencil cells, from the cell starts (gather skips vacuum)
 __global__ void k_colcount(int Mx, int My, int Mz, const int* __restrict__ start, int* __restrict__ colcount) {
@@ -68,121 +42,6 @@ __global__ void k_colcount(int Mx, int My, int Mz, const int* __restrict__ start
     cnt += __ldg(start + k + 1) - __ldg(start + k);
   }
   colcount[col] = cnt;
-}
-
-// ------------------------------------------------------------------------------------------------
-// spread
-// ------------------------------------------------------------------------------------------------
-
-template <int CB>
-__device__ __forceinline__ void load_q(const float* __restrict__ r, float (&q)[CB]) {
-  if constexpr (CB % 4 == 0) {
-#pragma unroll
-    for (int i = 0; i < CB / 4; ++i) {
-      float4 t = __ldg(reinterpret_cast<const float4*>(r) + i);
-      q[4 * i] = t.x; q[4 * i + 1] = t.y; q[4 * i + 2] = t.z; q[4 * i + 3] = t.w;
-    }
-  } else if constexpr (CB == 2) {
-    float2 t = __ldg(reinterpret_cast<const float2*>(r));
-    q[0] = t.x; q[1] = t.y;
-  } else {
-#pragma unroll
-    for (int i = 0; i < CB; ++i) q[i] = __ldg(r + i);
-  }
-}
-
-template <int CB>
-__global__ void __launch_bounds__(256) k_spread_tiled(int Mx, int My, int Mz, int recf, int cb0, int ntz,
-                                                      int nty, const int* __restrict__ start,
-                                                      const float* __restrict__ rec, float* __restrict__ grid) {
-  // block -> (x segment, 16 x 16 (y,z) tile); warp -> 4 x 8 patch; lane -> one grid column
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  int bid = blockIdx.x;
-  const int tz = bid % ntz; bid /= ntz;
-  const int ty = bid % nty; bid /= nty;
-  const int X0 = bid * SPREAD_TX;
-  const int X1 = min(X0 + SPREAD_TX, Mx);
-  const int Y0 = ty * 16 + (wid >> 1) * PY;
-  const int Z0 = tz * 16 + (wid & 1) * PZ;
-  if (Y0 >= My || Z0 >= Mz) return;
-  const int ly = lane >> 3, lz = lane & 7;
-  const int iy = Y0 + ly, iz = Z0 + lz;
-  const bool lane_ok = iy < My && iz < Mz;
-  const size_t Mtot = (size_t)Mx * My * Mz;
-
-  // z range of stencil cells whose footprint meets the patch: [Z0-7, Z0+7], wrapped into <= 2 runs
-  int zlo = Z0 - (FW - 1), zhi = min(Z0 + PZ - 1, Mz - 1);
-  int zlo2 = 0, zhi2 = -1;          // second run (after wrapping), empty by default
-  if (zlo < 0) {
-    zlo2 = zlo + Mz; zhi2 = Mz - 1; zlo = 0;
-  }
-
-  float acc[FW][CB];
-#pragma unroll
-  for (int a = 0; a < FW; ++a)
-#pragma unroll
-    for (int c = 0; c < CB; ++c) acc[a][c] = 0.f;
-
-  auto process_run = [&](int sx, int sy, int za, int zb, int r, auto& accu, auto slot_of) {
-    // atoms of cells (sx, sy, za..zb): one contiguous run in the cell-sorted order
-    const int kbase = (sx * My + sy) * Mz;
-    const int jlo = __ldg(start + kbase + za), jhi = __ldg(start + kbase + zb + 1);
-    const int dy = ly + FW - 1 - r;                 // y offset of this lane's column in the footprint
-    const bool y_ok = lane_ok && dy >= 0 && dy < FW;
-    for (int j = jlo; j < jhi; ++j) {
-      const float* rj = rec + (size_t)j * recf;
-      const int sz = __float_as_int(__ldg(rj + 3 * FW));
-      int t = iz - sz;
-      if (t < 0) t += Mz;
-      const bool ok = y_ok && t < FW;
-      float wy = 0.f, wz = 0.f;
-      if (ok) {
-        wy = __ldg(rj + FW + dy);
-        wz = __ldg(rj + 2 * FW + t);
-      }
-      const float v = wy * wz;
-      float q[CB];
-      load_q<CB>(rj + 3 * FW + 4 + cb0, q);
-      const float4 wa = __ldg(reinterpret_cast<const float4*>(rj));
-      const float4 wb = __ldg(reinterpret_cast<const float4*>(rj) + 1);
-      const float wx[FW] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-#pragma unroll
-      for (int c = 0; c < CB; ++c) {
-        const float vq = v * q[c];
-#pragma unroll
-        for (int a = 0; a < FW; ++a) slot_of(accu, a, c) = fmaf(wx[a], vq, slot_of(accu, a, c));
-      }
-    }
-  };
-
-  // planes s = X0-8 .. X1-1 in groups of 8 (static register rotation); plane s holds the atoms whose
-  // first x-point is s; after it, x-point s is complete and leaves the window.
-  for (int s0 = X0 - FW; s0 < X1; s0 += FW) {
-#pragma unroll
-    for (int u = 0; u < FW; ++u) {
-      const int s = s0 + u;
-      if (s < X1 && s > X0 - FW) {
-        const int sx = s < 0 ? s + Mx : s;
-        auto slot = [u](auto& A, int a, int c) -> float& { return A[(u + a) % FW][c]; };
-        for (int r = 0; r < PY + FW - 1; ++r) {
-          int sy = Y0 - (FW - 1) + r;
-          if (sy < 0) sy += My;
-          if (sy >= My) sy -= My;
-          process_run(sx, sy, zlo, zhi, r, acc, slot);
-          if (zhi2 >= zlo2) process_run(sx, sy, zlo2, zhi2, r, acc, slot);
-        }
-      }
-      if (s >= X0 && s < X1) {
-        if (lane_ok) {
-          const size_t gi = ((size_t)s * My + iy) * Mz + iz;
-#pragma unroll
-          for (int c = 0; c < CB; ++c) grid[(size_t)(cb0 + c) * Mtot + gi] = acc[u][c];
-        }
-      }
-#pragma unroll
-      for (int c = 0; c < CB; ++c) acc[u][c] = 0.f;
-    }
-  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -361,48 +220,11 @@ bool fast_path_supported(const pswf_lr_plan* p) {
   return true;
 }
 
-size_t fast_record_bytes(const pswf_lr_plan* p) { return sizeof(float) * rec_floats(p->C); }
-
-void launch_fast_prepare(pswf_lr_plan* p, int n, const float*, const float*, const GridGeom<float>& g,
+void launch_fast_prepare(pswf_lr_plan* p, int n, const float*, const float*, const GridGeom<float>&,
                          cudaStream_t st) {
+  (void)n;
   const int ncol = p->M[1] * p->M[2];
   k_colcount<<<(ncol + 255) / 256, 256, 0, st>>>(p->M[0], p->M[1], p->M[2], p->d_count, p->d_colcount);
-  if (n <= 0) return;
-  const int recf = rec_floats(p->C);
-  const long long threads = (long long)n * 32;
-  k_fast_records<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(n, p->C, p->cap_atoms, recf, g, p->d_si0,
-                                                                   (const float*)p->d_sdelta,
-                                                                   (const float*)p->d_sq, (float*)p->d_rec);
-}
-
-void launch_fast_spread(pswf_lr_plan* p, int n, const GridGeom<float>&, cudaStream_t st) {
-  (void)n;
-  const int Mx = p->M[0], My = p->M[1], Mz = p->M[2];
-  const int ntz = (Mz + 15) / 16, nty = (My + 15) / 16, nseg = (Mx + SPREAD_TX - 1) / SPREAD_TX;
-  const unsigned blocks = (unsigned)(ntz * nty * nseg);
-  const int recf = rec_floats(p->C);
-  const float* rec = (const float*)p->d_rec;
-  float* grid = (float*)p->d_grid;
-  int cb0 = 0;
-  while (cb0 < p->C) {
-    const int left = p->C - cb0;
-    if (left >= 8) {
-      k_spread_tiled<8><<<blocks, 256, 0, st>>>(Mx, My, Mz, recf, cb0, ntz, nty, p->d_count, rec, grid);
-      cb0 += 8;
-    } else if (left >= 4) {
-      k_spread_tiled<4><<<blocks, 256, 0, st>>>(Mx, My, Mz, recf, cb0, ntz, nty, p->d_count, rec, grid);
-      cb0 += 4;
-    } else if (left == 3) {
-      k_spread_tiled<3><<<blocks, 256, 0, st>>>(Mx, My, Mz, recf, cb0, ntz, nty, p->d_count, rec, grid);
-      cb0 += 3;
-    } else if (left == 2) {
-      k_spread_tiled<2><<<blocks, 256, 0, st>>>(Mx, My, Mz, recf, cb0, ntz, nty, p->d_count, rec, grid);
-      cb0 += 2;
-    } else {
-      k_spread_tiled<1><<<blocks, 256, 0, st>>>(Mx, My, Mz, recf, cb0, ntz, nty, p->d_count, rec, grid);
-      cb0 += 1;
-    }
-  }
 }
 
 void launch_fast_gather(pswf_lr_plan* p, int n, const GridGeom<float>& g, float* phi, float* F, cudaStream_t st) {

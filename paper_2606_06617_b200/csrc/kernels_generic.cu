@@ -337,7 +337,8 @@ __global__ void k_gather_ref(int n, int C, int cap, GridGeom<T> g, const int* __
 // host launchers
 // ------------------------------------------------------------------------------------------------
 template <class T>
-void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, cudaStream_t st) {
+void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, bool scatter,
+                     cudaStream_t st) {
   const int Mtot = p->M[0] * p->M[1] * p->M[2];
   cudaMemsetAsync(p->d_count, 0, sizeof(int) * ((size_t)Mtot + 1), st);
   if (n > 0)
@@ -345,7 +346,7 @@ void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const Gri
   k_scan_blocks<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_blocksums);
   k_scan_sums<<<1, 1024, 0, st>>>(p->n_scan_blocks, p->d_blocksums);
   k_scan_add<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_blocksums, Mtot, n);
-  if (n > 0)
+  if (n > 0 && scatter)
     k_scatter<T><<<(n + 255) / 256, 256, 0, st>>>(n, p->C, p->cap_atoms, pos, q, g, p->d_count, p->d_key,
                                                    p->d_rank, p->d_perm, p->d_si0, (T*)p->d_sdelta,
                                                    (T*)p->d_sq);
@@ -380,7 +381,7 @@ void launch_gather_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, T* phi, T* 
 }
 
 #define PSWF_INSTANTIATE(T)                                                                               \
-  template void launch_bin_sort<T>(pswf_lr_plan*, int, const T*, const T*, const GridGeom<T>&, cudaStream_t); \
+  template void launch_bin_sort<T>(pswf_lr_plan*, int, const T*, const T*, const GridGeom<T>&, bool, cudaStream_t); \
   template void launch_spread_ref<T>(pswf_lr_plan*, int, const GridGeom<T>&, cudaStream_t);              \
   template void launch_scale<T>(pswf_lr_plan*, const ScaleParams<T>&, bool, cudaStream_t);               \
   template void launch_gather_ref<T>(pswf_lr_plan*, int, const GridGeom<T>&, T*, T*, cudaStream_t);

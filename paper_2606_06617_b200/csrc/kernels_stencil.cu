@@ -1,0 +1,438 @@
+// Fast fp32 stencil kernels for sm_100a: spread (a1) and the per-atom weight records it consumes.
+//
+// Spread, Eq. (20)-(21),(24), is rho_g^a = sum_j q_j^a wx_j(g_x) wy_j(g_y) wz_j(g_z):
+// w^3 C FMAs per atom and ~0.5 atoms per grid cell, i.e. bound by FP32 issue, not by HBM.  Shared-
+// memory float atomics are CAS loops on sm_100a, so the kernel is OUTPUT-STATIONARY AT THREAD LEVEL
+// and atomic-free:
+//
+//  * a thread owns two adjacent grid columns (y, z0) and (y, z0+1) and sweeps x; its accumulators
+//    acc[8][2][CB] live in registers, slot k holding the plane x == k (mod 8);
+//  * atoms are cell-sorted; for every cell plane s_x the CTA stages the weight records of the cells
+//    (s_y, s_z) that can touch its 8WY x 8WZ patch into shared memory with TMA bulk copies
+//    (cp.async.bulk + mbarrier, double buffered, one contiguous run per cell row);
+//  * every thread then walks ITS OWN list of atoms -- the 8 x 9 cells whose footprint covers its
+//    two columns, read through a per-plane table of cell boundaries -- so nearly all lanes do
+//    useful FMAs (a warp-wide broadcast of each atom would keep only 64/165 of them busy);
+//  * the record holds the three weight vectors ROTATED by the atom's cell index mod 8, so a thread
+//    reads wy at offset (y & 7), wz at (z0 & 7) and multiplies slot k by wxr[k]: no per-atom index
+//    arithmetic, no register rotation, no unrolled plane loop;
+//  * when a plane leaves the window its slot is stored once with plain coalesced stores: no
+//    zero-fill of the grid, no atomics, deterministic summation order.
+//
+// Requirements of this path (host-checked): fp32, even w <= 8 (narrower windows are zero padded to 8
+// slots), M_d a multiple of 8 and >= 16.
+#include <cstdint>
+
+#include "kernels_common.cuh"
+#include "launch.hpp"
+
+namespace pswf {
+
+namespace {
+
+constexpr int SW = 8;  // stencil slots per dimension
+
+// ------------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + TMA bulk copy (global -> shared)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// scatter into cell-sorted order + per-atom weight records
+// record (recf floats): wxr[8] | wyc[8] | wzc[8] | q[C padded to 4]; wxr[k] = wx[(k - s_x) & 7] etc.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_scatter_records(int n, int C, int cap, int recf, const float* __restrict__ pos,
+                                                         const float* __restrict__ q, GridGeom<float> g,
+                                                         const int* __restrict__ start, const int* __restrict__ key,
+                                                         const int* __restrict__ rank, int* __restrict__ perm,
+                                                         int* __restrict__ si0, float* __restrict__ sdelta,
+                                                         float* __restrict__ sq, float* __restrict__ rec) {
+  __shared__ float s_coef[(kMaxWindowDegree + 1) * SW];
+  const int w = g.w, deg = g.wdeg;
+  for (int i = threadIdx.x; i < (deg + 1) * w; i += blockDim.x) s_coef[i] = g.wcoef[i];
+  __syncthreads();
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int dst = start[key[i]] + rank[i];
+  perm[dst] = i;
+  float* r = rec + (size_t)dst * recf;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    int i0;
+    double delta;
+    stencil_1d((double)pos[3 * (size_t)i + d], g.invL[d], g.M[d], w, i0, delta);
+    si0[(size_t)d * cap + dst] = i0;
+    const float df = (float)delta;
+    sdelta[(size_t)d * cap + dst] = df;
+    const int s = wrap_index(i0, g.M[d]);
+    const float xi = 2.f * df - 1.f;
+    float v[SW];
+#pragma unroll
+    for (int k = 0; k < SW; ++k) {
+      const int t = (k - s) & (SW - 1);
+      float a = 0.f;
+      if (t < w) {
+        a = s_coef[deg * w + t];
+        for (int m = deg - 1; m >= 0; --m) a = fmaf(a, xi, s_coef[m * w + t]);
+      }
+      v[k] = a;
+    }
+    reinterpret_cast<float4*>(r)[2 * d] = make_float4(v[0], v[1], v[2], v[3]);
+    reinterpret_cast<float4*>(r)[2 * d + 1] = make_float4(v[4], v[5], v[6], v[7]);
+  }
+  for (int c0 = 0; c0 < recf - 3 * SW; c0 += 4) {
+    float qq[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int c = c0 + u;
+      float t = 0.f;
+      if (c < C) {
+        t = q[(size_t)c * n + i];
+        sq[(size_t)c * cap + dst] = t;
+      }
+      qq[u] = t;
+    }
+    reinterpret_cast<float4*>(r + 3 * SW)[c0 >> 2] = make_float4(qq[0], qq[1], qq[2], qq[3]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// spread
+// ------------------------------------------------------------------------------------------------
+struct RoundDesc {
+  int p;      // cell plane index within the segment sweep (0 .. NP-1); NP = finished
+  int r0, r1; // rows of the plane handled by this round
+  int total;  // atoms staged
+  int slow;   // 1: a single row larger than the staging buffer, read from global memory
+};
+
+template <int WY, int WZ>
+struct SpreadShape {
+  static constexpr int TY = 8 * WY, TZ = 8 * WZ;
+  static constexpr int NROW = TY + 7, NCELL = TZ + 7, NB = TZ + 8;
+  static constexpr int NT = 32 * WY * WZ;
+  static constexpr int kHeader = 64 + 2 * 32 * 4 + 3 * 32 * 16;  // mbar+desc | rowoff | rowinfo
+  static constexpr int kTables = 3 * NROW * NB * 4;
+  static_assert(NROW <= 32, "one lane per row in the round builder");
+};
+
+// One thread's walk over its atoms of a round: rows [r, r_hi) of the plane table; per row the cells
+// s_z = z0-7 .. z0+1 are one contiguous run [a.x, b.y) of staged records; atoms of the first cell miss
+// column z0+1 (j < a.y) and atoms of the last cell miss column z0 (j >= b.x).
+// GLOBAL = false: records in shared memory (LDS); true: the round's single row read from global memory.
+template <int CB, bool GLOBAL>
+__device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], int r, const int r_hi, const int* Lp, const int NB,
+                                           const int* ro, const float* rbase, const int recf, const int cb0,
+                                           const int oy, const int oz, const int4 srow) {
+  int j = 0, jend = 0, ja = 0, jb = 0;
+  for (;;) {
+    bool more = true;
+    while (j >= jend) {
+      if (r >= r_hi) { more = false; break; }
+      const int2 a = *reinterpret_cast<const int2*>(Lp + r * NB);
+      const int2 b = *reinterpret_cast<const int2*>(Lp + r * NB + SW);
+      const int off = GLOBAL ? 0 : ro[r];
+      j = off + a.x; ja = off + a.y; jb = off + b.x; jend = off + b.y;
+      ++r;
+    }
+    if (!more) break;
+    const float* rp;
+    if constexpr (GLOBAL) {
+      const int gj = j < srow.y ? srow.x + j : srow.z + (j - srow.y);
+      rp = rbase + (size_t)gj * recf;
+    } else {
+      rp = rbase + j * recf;
+    }
+    const float4 wa = *reinterpret_cast<const float4*>(rp);
+    const float4 wb = *reinterpret_cast<const float4*>(rp + 4);
+    float qv[CB];
+    if constexpr (CB >= 3) {
+      const float4 t = *reinterpret_cast<const float4*>(rp + 3 * SW + cb0);
+      qv[0] = t.x; qv[1] = t.y; qv[2] = t.z;
+      if constexpr (CB == 4) qv[3] = t.w;
+    } else if constexpr (CB == 2) {
+      const float2 t = *reinterpret_cast<const float2*>(rp + 3 * SW + cb0);
+      qv[0] = t.x; qv[1] = t.y;
+    } else {
+      qv[0] = rp[3 * SW + cb0];
+    }
+    const float wyv = rp[oy];
+    const float2 wzv = *reinterpret_cast<const float2*>(rp + oz);
+    const float p0 = j < jb ? wyv * wzv.x : 0.f;
+    const float p1 = j >= ja ? wyv * wzv.y : 0.f;
+    const float wx[SW] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+#pragma unroll
+    for (int c = 0; c < CB; ++c) {
+      const float v0 = p0 * qv[c], v1 = p1 * qv[c];
+#pragma unroll
+      for (int k = 0; k < SW; ++k) {
+        acc[k][0][c] = fmaf(wx[k], v0, acc[k][0][c]);
+        acc[k][1][c] = fmaf(wx[k], v1, acc[k][1][c]);
+      }
+    }
+    ++j;
+  }
+}
+
+template <int WY, int WZ, int CB>
+__global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 4 ? 3 : 2)))
+    k_spread_os(int Mx, int My, int Mz, int XS, int npy, int npz, int cap, int recf, int cb0,
+                const int* __restrict__ start, const float* __restrict__ rec, float* __restrict__ grid) {
+  using S = SpreadShape<WY, WZ>;
+  constexpr int NROW = S::NROW, NB = S::NB, NT = S::NT;
+  extern __shared__ __align__(128) unsigned char smem[];
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem);                 // [2]
+  RoundDesc* s_desc = reinterpret_cast<RoundDesc*>(smem + 16);        // [2]
+  int* s_rowoff = reinterpret_cast<int*>(smem + 64);                  // [2][32]
+  int4* s_row = reinterpret_cast<int4*>(smem + 64 + 256);             // [3][32]  {gA0, nA, gB0, nB}
+  int* s_L = reinterpret_cast<int*>(smem + S::kHeader);               // [3][NROW][NB]
+  float* s_rec = reinterpret_cast<float*>(smem + S::kHeader + S::kTables);  // [2][cap * recf]
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  int bid = blockIdx.x;
+  const int pz = bid % npz; bid /= npz;
+  const int py = bid % npy; bid /= npy;
+  const int X0 = bid * XS, X1 = min(X0 + XS, Mx);
+  const int NP = X1 - X0 + (SW - 1);
+  const int Y0 = py * S::TY, Z0 = pz * S::TZ;
+  // cells of a row: sz_u = Z0-7 .. Z0+TZ-1; those below 0 wrap to the end of the row (run A)
+  const int nAc = Z0 < SW - 1 ? SW - 1 - Z0 : 0;
+  const int zb0 = Z0 - (SW - 1) + nAc;
+  const int nBc = min(S::NCELL - nAc, Mz - zb0);
+  const int ncell = nAc + nBc;
+
+  // this thread's two columns
+  const int wy_ = warp / WZ, wz_ = warp % WZ;
+  const int ly = lane >> 2, lzp = lane & 3;
+  const int y = Y0 + wy_ * 8 + ly, z0 = Z0 + wz_ * 8 + 2 * lzp;
+  const bool lane_ok = y < My && z0 < Mz;
+  const int rlo = wy_ * 8 + ly;          // first of the 8 rows (s_y = y-7 .. y) this thread reads
+  const int clo = wz_ * 8 + 2 * lzp;     // boundary index of cell s_z = z0-7
+  const int oy = SW + (y & 7), oz = 2 * SW + (z0 & 7);
+  const size_t Mtot = (size_t)Mx * My * Mz;
+
+  auto build_plane = [&](int pl) {
+    const int tb = pl % 3;
+    const int sxu = X0 - (SW - 1) + pl;
+    const int sx = sxu < 0 ? sxu + Mx : sxu;
+    for (int t = tid; t < NROW * NB; t += NT) {
+      const int r = t / NB, b = t - r * NB;
+      const int syu = Y0 - (SW - 1) + r;
+      int val = 0;
+      int4 ri = make_int4(0, 0, 0, 0);
+      if (syu < My) {
+        const int sy = syu < 0 ? syu + My : syu;
+        const int* rs = start + ((size_t)sx * My + sy) * Mz;
+        const int gA0 = nAc ? __ldg(rs + Mz - nAc) : 0;
+        const int nA = nAc ? __ldg(rs + Mz) - gA0 : 0;
+        const int gB0 = __ldg(rs + zb0);
+        if (b < nAc) {
+          val = __ldg(rs + Mz - nAc + b) - gA0;
+        } else {
+          const int bb = min(b, ncell) - nAc;
+          val = nA + __ldg(rs + zb0 + bb) - gB0;
+        }
+        if (b == 0) ri = make_int4(gA0, nA, gB0, __ldg(rs + zb0 + nBc) - gB0);
+      }
+      s_L[(tb * NROW + r) * NB + b] = val;
+      if (b == 0) s_row[tb * 32 + r] = ri;
+    }
+  };
+
+  // round builder (warp 0): rows [rn0, r1n) of plane pn whose atoms fit the staging buffer
+  auto build_round = [&](int pn, int rn0, int nb) {
+    RoundDesc nd;
+    nd.p = pn; nd.r0 = rn0; nd.r1 = NROW; nd.total = 0; nd.slow = 0;
+    if (pn < NP) {
+      const int tb = pn % 3;
+      const bool mine = lane >= rn0 && lane < NROW;
+      const int tot = mine ? s_L[(tb * NROW + lane) * NB + NB - 1] : 0;
+      int cum = tot;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, cum, o);
+        if (lane >= o) cum += t;
+      }
+      int nr = __popc(__ballot_sync(0xffffffffu, mine && cum <= cap));
+      if (nr == 0) { nr = 1; nd.slow = 1; }
+      nd.r1 = rn0 + nr;
+      nd.total = __shfl_sync(0xffffffffu, cum, nd.r1 - 1);
+      const bool in_round = lane >= rn0 && lane < nd.r1;
+      if (in_round) s_rowoff[nb * 32 + lane] = cum - tot;
+      if (!nd.slow && nd.total > 0) {
+        if (lane == 0) mbar_arrive_expect_tx(&mbar[nb], (uint32_t)nd.total * recf * 4u);
+        __syncwarp();
+        if (in_round && tot > 0) {
+          const int4 ri = s_row[tb * 32 + lane];
+          float* dst = s_rec + (size_t)nb * cap * recf + (size_t)(cum - tot) * recf;
+          if (ri.y > 0) bulk_g2s(dst, rec + (size_t)ri.x * recf, (uint32_t)ri.y * recf * 4u, &mbar[nb]);
+          if (ri.w > 0)
+            bulk_g2s(dst + (size_t)ri.y * recf, rec + (size_t)ri.z * recf, (uint32_t)ri.w * recf * 4u, &mbar[nb]);
+        }
+      }
+    }
+    if (lane == 0) s_desc[nb] = nd;
+  };
+
+  if (tid == 0) {
+    mbar_init(&mbar[0], 1);
+    mbar_init(&mbar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  build_plane(0);
+  if (NP > 1) build_plane(1);
+  __syncthreads();
+  if (warp == 0) build_round(0, 0, 0);
+
+  float acc[SW][2][CB];
+#pragma unroll
+  for (int k = 0; k < SW; ++k)
+#pragma unroll
+    for (int u = 0; u < 2; ++u)
+#pragma unroll
+      for (int c = 0; c < CB; ++c) acc[k][u][c] = 0.f;
+
+  uint32_t phase0 = 0, phase1 = 0;
+  for (int it = 0;; ++it) {
+    __syncthreads();
+    const int cur = it & 1;
+    const RoundDesc d = s_desc[cur];
+    if (d.p >= NP) break;
+    if (warp == 0) {
+      const bool last = d.r1 >= NROW;
+      build_round(last ? d.p + 1 : d.p, last ? 0 : d.r1, cur ^ 1);
+    }
+    if (d.r0 == 0 && d.p + 2 < NP) build_plane(d.p + 2);
+    if (!d.slow && d.total > 0) {
+      if (cur == 0) { mbar_wait(&mbar[0], phase0); phase0 ^= 1; }
+      else          { mbar_wait(&mbar[1], phase1); phase1 ^= 1; }
+    }
+    // ---- this thread's atoms of the round ----
+    {
+      const int tb = d.p % 3;
+      const int r_beg = max(rlo, d.r0);
+      const int r_hi = lane_ok ? min(rlo + SW, d.r1) : r_beg;
+      const int* Lp = s_L + (size_t)tb * NROW * NB + clo;
+      if (!d.slow)
+        walk_atoms<CB, false>(acc, r_beg, r_hi, Lp, NB, s_rowoff + cur * 32, s_rec + (size_t)cur * cap * recf, recf,
+                              cb0, oy, oz, make_int4(0, 0, 0, 0));
+      else   // a single row larger than the staging buffer: records straight from global memory
+        walk_atoms<CB, true>(acc, r_beg, r_hi, Lp, NB, nullptr, rec, recf, cb0, oy, oz, s_row[tb * 32 + d.r0]);
+    }
+    // ---- plane complete: store its slot once, clear it ----
+    if (d.r1 >= NROW) {
+      const int sxu = X0 - (SW - 1) + d.p;
+      const bool st = lane_ok && sxu >= X0;
+      float* gp = grid + (size_t)cb0 * Mtot + ((size_t)max(sxu, 0) * My + y) * Mz + z0;
+      switch (sxu & 7) {
+#define PSWF_FLUSH(K)                                                                                   \
+  case K:                                                                                               \
+    _Pragma("unroll") for (int c = 0; c < CB; ++c) {                                                    \
+      if (st) *reinterpret_cast<float2*>(gp + (size_t)c * Mtot) = make_float2(acc[K][0][c], acc[K][1][c]); \
+      acc[K][0][c] = 0.f;                                                                               \
+      acc[K][1][c] = 0.f;                                                                               \
+    }                                                                                                   \
+    break;
+        PSWF_FLUSH(0) PSWF_FLUSH(1) PSWF_FLUSH(2) PSWF_FLUSH(3)
+        PSWF_FLUSH(4) PSWF_FLUSH(5) PSWF_FLUSH(6) PSWF_FLUSH(7)
+#undef PSWF_FLUSH
+      }
+    }
+  }
+}
+
+template <int WY, int WZ>
+struct SpreadLaunch {
+  using S = SpreadShape<WY, WZ>;
+  static size_t smem_bytes(int cap, int recf) { return S::kHeader + S::kTables + 2 * (size_t)cap * recf * 4; }
+
+  template <int CB>
+  static void run(pswf_lr_plan* p, int XS, int cap, int recf, int cb0, cudaStream_t st) {
+    const int Mx = p->M[0], My = p->M[1], Mz = p->M[2];
+    const int npy = (My + S::TY - 1) / S::TY, npz = (Mz + S::TZ - 1) / S::TZ, nseg = (Mx + XS - 1) / XS;
+    const size_t sm = smem_bytes(cap, recf);
+    auto kern = k_spread_os<WY, WZ, CB>;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    kern<<<(unsigned)(npy * npz * nseg), S::NT, sm, st>>>(Mx, My, Mz, XS, npy, npz, cap, recf, cb0, p->d_count,
+                                                         (const float*)p->d_rec, (float*)p->d_grid);
+  }
+};
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+int stencil_rec_floats(int C) {
+  int f = 3 * SW + ((C + 3) / 4) * 4;
+  if (((f / 4) & 1) == 0) f += 4;   // odd number of 16-byte quads: consecutive records hit distinct banks
+  return f;
+}
+
+bool stencil_path_supported(const pswf_lr_plan* p) {
+  if (p->precision != PSWF_LR_F32 || p->w > SW) return false;
+  for (int d = 0; d < 3; ++d)
+    if (p->M[d] % SW != 0 || p->M[d] < 2 * SW) return false;
+  return true;
+}
+
+size_t stencil_record_bytes(const pswf_lr_plan* p) { return sizeof(float) * stencil_rec_floats(p->C); }
+
+void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
+                            cudaStream_t st) {
+  if (n <= 0) return;
+  k_scatter_records<<<(n + 255) / 256, 256, 0, st>>>(n, p->C, p->cap_atoms, stencil_rec_floats(p->C), pos, q, g,
+                                                     p->d_count, p->d_key, p->d_rank, p->d_perm, p->d_si0,
+                                                     (float*)p->d_sdelta, (float*)p->d_sq, (float*)p->d_rec);
+}
+
+void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {
+  (void)n;
+  using L = SpreadLaunch<2, 2>;
+  const int recf = stencil_rec_floats(p->C);
+  // staging capacity: three CTAs per SM
+  const size_t budget = 74 * 1024;
+  int cap = (int)((budget - L::S::kHeader - L::S::kTables) / (2 * (size_t)recf * 4));
+  cap &= ~7;
+  // x segments: enough CTAs to fill the machine, as long as possible (each segment re-reads 7 halo planes)
+  const int Mx = p->M[0];
+  const int npatch = ((p->M[1] + L::S::TY - 1) / L::S::TY) * ((p->M[2] + L::S::TZ - 1) / L::S::TZ);
+  int XS = Mx;
+  while (XS > 16 && npatch * ((Mx + XS - 1) / XS) < 2 * p->sm_count) XS = ((XS / 2 + 7) / 8) * 8;
+  int cb0 = 0;
+  while (cb0 < p->C) {
+    const int left = p->C - cb0;
+    if (left >= 4) { L::run<4>(p, XS, cap, recf, cb0, st); cb0 += 4; }
+    else if (left == 3) { L::run<3>(p, XS, cap, recf, cb0, st); cb0 += 3; }
+    else if (left == 2) { L::run<2>(p, XS, cap, recf, cb0, st); cb0 += 2; }
+    else { L::run<1>(p, XS, cap, recf, cb0, st); cb0 += 1; }
+  }
+}
+
+}  // namespace pswf

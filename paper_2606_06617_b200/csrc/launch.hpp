@@ -5,7 +5,8 @@
 namespace pswf {
 
 template <class T>
-void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, cudaStream_t st);
+void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, bool scatter,
+                     cudaStream_t st);
 template <class T>
 void launch_spread_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, cudaStream_t st);
 template <class T>
@@ -16,11 +17,16 @@ void launch_gather_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, T* phi, T* 
 
 // fast fp32 path (kernels_fast.cu)
 bool fast_path_supported(const pswf_lr_plan* p);
-size_t fast_record_bytes(const pswf_lr_plan* p);
 void launch_fast_prepare(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
                          cudaStream_t st);
-void launch_fast_spread(pswf_lr_plan* p, int n, const GridGeom<float>& g, cudaStream_t st);
 void launch_fast_gather(pswf_lr_plan* p, int n, const GridGeom<float>& g, float* phi, float* F,
                         cudaStream_t st);
+
+// stencil fp32 path (kernels_stencil.cu)
+bool stencil_path_supported(const pswf_lr_plan* p);
+size_t stencil_record_bytes(const pswf_lr_plan* p);
+void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
+                            cudaStream_t st);
+void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st);
 
 }  // namespace pswf

@@ -71,7 +71,7 @@ int ensure_capacity(pswf_lr_plan* p, int n) {
   rc |= dev_alloc(&p->d_sdelta, rs * 3 * (size_t)cap, &b);
   rc |= dev_alloc(&p->d_sq, rs * (size_t)p->C * cap, &b);
   p->cap_atoms = cap;
-  size_t recb = fast_path_supported(p) ? fast_record_bytes(p) * (size_t)cap : 0;
+  size_t recb = stencil_path_supported(p) ? stencil_record_bytes(p) * (size_t)cap : 0;
   if (recb) rc |= dev_alloc(&p->d_rec, recb, &b);
   if (rc) {
     free_atoms(p);
@@ -159,7 +159,8 @@ ScaleParams<T> make_scale(const pswf_lr_plan* p) {
 template <class T>
 int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* phi, T* F, cudaStream_t st) {
   constexpr bool kIsF32 = std::is_same<T, float>::value;
-  const bool fast = kIsF32 && (p->kernel_path == 0) && fast_path_supported(p);
+  const bool stencil = kIsF32 && (p->kernel_path == 0) && stencil_path_supported(p);
+  const bool fast = stencil && fast_path_supported(p);
   GridGeom<T> g = make_geom<T>(p);
   ScaleParams<T> P = make_scale<T>(p);
   cudaEvent_t* ev = nullptr;
@@ -167,16 +168,17 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
     ev = p->events.data() + (size_t)p->prof_count * (PSWF_LR_N_STAGES + 1);
   if (ev) cudaEventRecord(ev[0], st);
   // a0
-  launch_bin_sort<T>(p, n, pos, q, g, st);
+  launch_bin_sort<T>(p, n, pos, q, g, !stencil, st);
   if constexpr (kIsF32) {
+    if (stencil) launch_scatter_records(p, n, pos, q, g, st);
     if (fast) launch_fast_prepare(p, n, pos, q, g, st);
   }
   if (ev) cudaEventRecord(ev[1], st);
   // a1
   if constexpr (kIsF32) {
-    if (fast) launch_fast_spread(p, n, g, st);
+    if (stencil) launch_stencil_spread(p, n, st);
   }
-  if (!fast) launch_spread_ref<T>(p, n, g, st);
+  if (!stencil) launch_spread_ref<T>(p, n, g, st);
   if (ev) cudaEventRecord(ev[2], st);
   // a2
   CUFFT_TRY(cufftSetStream(p->fft_fwd, st));
