@@ -66,22 +66,28 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // ------------------------------------------------------------------------------------------------
 // scatter into cell-sorted order + per-atom weight records
 // record (recf floats): wxr[8] | wyc[8] | wzc[8] | q[C padded to 4]; wxr[k] = wx[(k - s_x) & 7] etc.
+// derivative record (24 floats, gather only): dxr[8] | dyc[8] | dzc[8], d/dr_d of the same weights
+// (derivative of the SAME panel polynomials), rotated the same way.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_scatter_records(int n, int C, int cap, int recf, const float* __restrict__ pos,
                                                          const float* __restrict__ q, GridGeom<float> g,
                                                          const int* __restrict__ start, const int* __restrict__ key,
                                                          const int* __restrict__ rank, int* __restrict__ perm,
                                                          int* __restrict__ si0, float* __restrict__ sdelta,
-                                                         float* __restrict__ sq, float* __restrict__ rec) {
+                                                         float* __restrict__ sq, float* __restrict__ rec,
+                                                         float* __restrict__ drec) {
   __shared__ float s_coef[(kMaxWindowDegree + 1) * SW];
+  __shared__ float s_dcoef[kMaxWindowDegree * SW];
   const int w = g.w, deg = g.wdeg;
   for (int i = threadIdx.x; i < (deg + 1) * w; i += blockDim.x) s_coef[i] = g.wcoef[i];
+  for (int i = threadIdx.x; i < deg * w; i += blockDim.x) s_dcoef[i] = g.wdcoef[i];
   __syncthreads();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int dst = start[key[i]] + rank[i];
   perm[dst] = i;
   float* r = rec + (size_t)dst * recf;
+  float* dr = drec + (size_t)dst * (3 * SW);
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     int i0;
@@ -92,19 +98,27 @@ __global__ void __launch_bounds__(256) k_scatter_records(int n, int C, int cap, 
     sdelta[(size_t)d * cap + dst] = df;
     const int s = wrap_index(i0, g.M[d]);
     const float xi = 2.f * df - 1.f;
-    float v[SW];
+    float v[SW], dv[SW];
 #pragma unroll
     for (int k = 0; k < SW; ++k) {
       const int t = (k - s) & (SW - 1);
-      float a = 0.f;
+      float a = 0.f, b = 0.f;
       if (t < w) {
         a = s_coef[deg * w + t];
-        for (int m = deg - 1; m >= 0; --m) a = fmaf(a, xi, s_coef[m * w + t]);
+        b = s_dcoef[(deg - 1) * w + t];
+        for (int m = deg - 1; m >= 1; --m) {
+          a = fmaf(a, xi, s_coef[m * w + t]);
+          b = fmaf(b, xi, s_dcoef[(m - 1) * w + t]);
+        }
+        a = fmaf(a, xi, s_coef[t]);
       }
       v[k] = a;
+      dv[k] = b * g.dxi_dr[d];
     }
     reinterpret_cast<float4*>(r)[2 * d] = make_float4(v[0], v[1], v[2], v[3]);
     reinterpret_cast<float4*>(r)[2 * d + 1] = make_float4(v[4], v[5], v[6], v[7]);
+    reinterpret_cast<float4*>(dr)[2 * d] = make_float4(dv[0], dv[1], dv[2], dv[3]);
+    reinterpret_cast<float4*>(dr)[2 * d + 1] = make_float4(dv[4], dv[5], dv[6], dv[7]);
   }
   for (int c0 = 0; c0 < recf - 3 * SW; c0 += 4) {
     float qq[4];
@@ -403,13 +417,15 @@ bool stencil_path_supported(const pswf_lr_plan* p) {
 }
 
 size_t stencil_record_bytes(const pswf_lr_plan* p) { return sizeof(float) * stencil_rec_floats(p->C); }
+size_t stencil_drecord_bytes(const pswf_lr_plan*) { return sizeof(float) * 3 * SW; }
 
 void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
                             cudaStream_t st) {
   if (n <= 0) return;
   k_scatter_records<<<(n + 255) / 256, 256, 0, st>>>(n, p->C, p->cap_atoms, stencil_rec_floats(p->C), pos, q, g,
                                                      p->d_count, p->d_key, p->d_rank, p->d_perm, p->d_si0,
-                                                     (float*)p->d_sdelta, (float*)p->d_sq, (float*)p->d_rec);
+                                                     (float*)p->d_sdelta, (float*)p->d_sq, (float*)p->d_rec,
+                                                     (float*)p->d_drec);
 }
 
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {

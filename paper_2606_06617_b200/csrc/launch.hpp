@@ -15,16 +15,13 @@ void launch_finalize_energy(pswf_lr_plan* p, double* E, cudaStream_t st);
 template <class T>
 void launch_gather_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, T* phi, T* F, cudaStream_t st);
 
-// fast fp32 path (kernels_fast.cu)
-bool fast_path_supported(const pswf_lr_plan* p);
-void launch_fast_prepare(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
-                         cudaStream_t st);
-void launch_fast_gather(pswf_lr_plan* p, int n, const GridGeom<float>& g, float* phi, float* F,
-                        cudaStream_t st);
-
-// stencil fp32 path (kernels_stencil.cu)
+// fast fp32 path: per-atom weight records + output-stationary spread (kernels_stencil.cu),
+// register-window gather (kernels_gather.cu)
 bool stencil_path_supported(const pswf_lr_plan* p);
+int stencil_rec_floats(int C);
 size_t stencil_record_bytes(const pswf_lr_plan* p);
+size_t stencil_drecord_bytes(const pswf_lr_plan* p);
+void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream_t st);
 void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
                             cudaStream_t st);
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st);

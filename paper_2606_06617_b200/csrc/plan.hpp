@@ -76,7 +76,6 @@ struct pswf_lr_plan {
   void* d_spec = nullptr;         // cplx  [C][Mx][My][Mz/2+1]
   int* d_count = nullptr;         // [Mtot + 1] cell counts -> exclusive starts
   int* d_blocksums = nullptr;
-  int* d_colcount = nullptr;      // [My*Mz] atoms per stencil-cell column (fast gather)
   int n_scan_blocks = 0;
   double* d_Ech = nullptr;        // [C]
   double* d_Etot = nullptr;       // [1] (execute_host staging)
@@ -89,6 +88,7 @@ struct pswf_lr_plan {
   void* d_sdelta = nullptr;       // real [3][cap]
   void* d_sq = nullptr;           // real [C][cap]
   void* d_rec = nullptr;          // fast path: per-atom weight records
+  void* d_drec = nullptr;         // fast path: per-atom derivative-weight records (gather)
   void* d_pos_in = nullptr;       // execute_host staging
   void* d_q_in = nullptr;
   void* d_phi_out = nullptr;

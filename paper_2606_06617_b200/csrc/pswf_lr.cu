@@ -47,7 +47,7 @@ int dev_alloc(void** ptr, size_t bytes, long long* total) {
 
 void free_atoms(pswf_lr_plan* p) {
   void** ptrs[] = {(void**)&p->d_key, (void**)&p->d_rank, (void**)&p->d_perm, (void**)&p->d_si0, &p->d_sdelta,
-                   &p->d_sq,          &p->d_rec,          &p->d_pos_in,       &p->d_q_in,        &p->d_phi_out,
+                   &p->d_sq,          &p->d_rec,          &p->d_drec,         &p->d_pos_in,       &p->d_q_in,        &p->d_phi_out,
                    &p->d_F_out};
   for (void** q : ptrs) {
     if (*q) cudaFree(*q);
@@ -73,6 +73,7 @@ int ensure_capacity(pswf_lr_plan* p, int n) {
   p->cap_atoms = cap;
   size_t recb = stencil_path_supported(p) ? stencil_record_bytes(p) * (size_t)cap : 0;
   if (recb) rc |= dev_alloc(&p->d_rec, recb, &b);
+  if (recb) rc |= dev_alloc(&p->d_drec, stencil_drecord_bytes(p) * (size_t)cap, &b);
   if (rc) {
     free_atoms(p);
     p->cap_atoms = 0;
@@ -160,7 +161,6 @@ template <class T>
 int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* phi, T* F, cudaStream_t st) {
   constexpr bool kIsF32 = std::is_same<T, float>::value;
   const bool stencil = kIsF32 && (p->kernel_path == 0) && stencil_path_supported(p);
-  const bool fast = stencil && fast_path_supported(p);
   GridGeom<T> g = make_geom<T>(p);
   ScaleParams<T> P = make_scale<T>(p);
   cudaEvent_t* ev = nullptr;
@@ -171,7 +171,6 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   launch_bin_sort<T>(p, n, pos, q, g, !stencil, st);
   if constexpr (kIsF32) {
     if (stencil) launch_scatter_records(p, n, pos, q, g, st);
-    if (fast) launch_fast_prepare(p, n, pos, q, g, st);
   }
   if (ev) cudaEventRecord(ev[1], st);
   // a1
@@ -202,9 +201,9 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
     if (ev) cudaEventRecord(ev[5], st);
     // a5
     if constexpr (kIsF32) {
-      if (fast) launch_fast_gather(p, n, g, phi, F, st);
+      if (stencil) launch_fast_gather(p, n, phi, F, st);
     }
-    if (!fast) launch_gather_ref<T>(p, n, g, phi, F, st);
+    if (!stencil) launch_gather_ref<T>(p, n, g, phi, F, st);
     if (ev) cudaEventRecord(ev[6], st);
   } else if (ev) {
     cudaEventRecord(ev[5], st);
@@ -389,7 +388,6 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       if (!rc) rc = dev_alloc((void**)&p->d_count, sizeof(int) * (Mtot + 1), &b);
       p->n_scan_blocks = (int)((Mtot + 4095) / 4096);
       if (!rc) rc = dev_alloc((void**)&p->d_blocksums, sizeof(int) * (size_t)p->n_scan_blocks, &b);
-      if (!rc) rc = dev_alloc((void**)&p->d_colcount, sizeof(int) * (size_t)p->M[1] * p->M[2], &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Etot, sizeof(double), &b);
       p->workspace_bytes += b;
@@ -610,8 +608,7 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   cudaDeviceSynchronize();
   free_atoms(p);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
-                  p->d_grid,  p->d_spec,    p->d_count,    p->d_blocksums, p->d_Ech,      p->d_Etot,
-                  p->d_colcount};
+                  p->d_grid,  p->d_spec,    p->d_count,    p->d_blocksums, p->d_Ech,      p->d_Etot};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   if (p->have_fft) {
