@@ -13,8 +13,11 @@
 //    ROTATED by the atom's cell index mod 8, so the x contraction is sum_k wxr[k] * win[k] with static
 //    register indices: one copy of the atom code, no unrolled window rotation (the first tiled
 //    kernel's 118 KB of SASS thrashed the instruction cache, profiles/r1a);
-//  * one coalesced plane load per x step refreshes the slot that left the window (served by L1:
-//    neighbouring columns of the CTA share 7/8 of their footprint);
+//  * the potential grid is first copied from cuFFT's planar layout [C][M] into a channel-interleaved
+//    one [M][CB] (k_interleave, L2-resident, ~10 us), so that one 16-byte load per footprint point
+//    refreshes the slot that left the window for all channels (with planar loads the address
+//    arithmetic of 8 scalar loads per x step was a third of all instructions, profiles/r1c);
+//    the loads are served by L1: neighbouring columns of the CTA share 7/8 of their footprint;
 //  * the lanes of a segment fetch the cell boundaries of its 32 cells at once, prefetch the
 //    records of the non-empty cells to L2, skip leading / trailing empty cells and return at once
 //    when the segment holds no atoms (vacuum of configuration 5);
@@ -31,6 +34,32 @@ namespace {
 constexpr int SW = 8;        // stencil slots per dimension
 constexpr int XSEG = 32;     // cells per x segment: one lane per cell boundary pair
 constexpr int GBY = 2, GBZ = 4;   // cell columns per CTA (y x z): 8 warps
+
+template <int CB> struct VecOf;
+template <> struct VecOf<1> { using type = float; };
+template <> struct VecOf<2> { using type = float2; };
+template <> struct VecOf<4> { using type = float4; };
+
+template <int CB>
+__device__ __forceinline__ void unpack(const typename VecOf<CB>::type& v, float (&o)[CB]) {
+  if constexpr (CB == 1) { o[0] = v; }
+  else if constexpr (CB == 2) { o[0] = v.x; o[1] = v.y; }
+  else { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+}
+
+// planar [C][M] -> interleaved [M][CB] for the channels cb0 .. cb0+CB-1 (missing channels read as 0)
+template <int CB>
+__global__ void __launch_bounds__(256) k_interleave(size_t Mtot, int nch, const float* __restrict__ planar,
+                                                    typename VecOf<CB>::type* __restrict__ out) {
+  const size_t m = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= Mtot) return;
+  float v[CB];
+#pragma unroll
+  for (int c = 0; c < CB; ++c) v[c] = c < nch ? __ldg(planar + (size_t)c * Mtot + m) : 0.f;
+  if constexpr (CB == 1) out[m] = v[0];
+  else if constexpr (CB == 2) out[m] = make_float2(v[0], v[1]);
+  else out[m] = make_float4(v[0], v[1], v[2], v[3]);
+}
 
 // 9-shuffle transpose-reduce of 8 values over the 32 lanes; on return lane l holds in v[0] the full
 // sum of input index  ((l >> 4) & 1) * 4 + ((l >> 3) & 1) * 2 + ((l >> 2) & 1).
@@ -68,8 +97,9 @@ template <int CB>
 __global__ void __launch_bounds__(32 * GBY * GBZ, 2)
     k_gather_cols(int n, int C, int cb0, int Mx, int My, int Mz, int nseg, int nby, int nbz, int recf,
                   const int* __restrict__ start, const float* __restrict__ rec, const float* __restrict__ drec,
-                  const int* __restrict__ perm, const float* __restrict__ grid, float* __restrict__ phi,
-                  float* __restrict__ Facc, int accumulate_F) {
+                  const int* __restrict__ perm, const typename VecOf<CB>::type* __restrict__ gridi,
+                  float* __restrict__ phi, float* __restrict__ Facc, int accumulate_F) {
+  using V = typename VecOf<CB>::type;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   // block -> (segment, y block, z block); consecutive blocks walk z, then y: CTAs resident on an SM
   // at the same time share most of their footprints in L1
@@ -103,25 +133,21 @@ __global__ void __launch_bounds__(32 * GBY * GBZ, 2)
   int iz = sz + c_off; if (iz >= Mz) iz -= Mz;
   int iy0 = sy + b0;      if (iy0 >= My) iy0 -= My;
   int iy1 = sy + b0 + 4;  if (iy1 >= My) iy1 -= My;
-  const size_t Mtot = (size_t)Mx * My * Mz;
-  const size_t plane = (size_t)My * Mz;
-  const float* g0 = grid + (size_t)cb0 * Mtot + (size_t)iy0 * Mz + iz;
-  const float* g1 = grid + (size_t)cb0 * Mtot + (size_t)iy1 * Mz + iz;
+  const unsigned plane = (unsigned)My * Mz;
+  const V* g0 = gridi + (size_t)iy0 * Mz + iz;
+  const V* g1 = gridi + (size_t)iy1 * Mz + iz;
   // record offsets of this lane's (y,z) weights (records are rotated by the cell index mod 8)
   const int oy0 = SW + ((sy + b0) & 7), oy1 = SW + ((sy + b0 + 4) & 7), oz = 2 * SW + ((sz + c_off) & 7);
 
   float win[SW][2][CB];
   auto load_plane = [&](int xs) {
     int x = xs; if (x >= Mx) x -= Mx;
-    const float* p0 = g0 + (size_t)x * plane;
-    const float* p1 = g1 + (size_t)x * plane;
-    switch (xs & 7) {
-#define PSWF_LOAD(K)                                        \
-  case K:                                                   \
-    _Pragma("unroll") for (int c = 0; c < CB; ++c) {        \
-      win[K][0][c] = __ldg(p0 + (size_t)c * Mtot);          \
-      win[K][1][c] = __ldg(p1 + (size_t)c * Mtot);          \
-    }                                                       \
+    const unsigned off = (unsigned)x * plane;
+    switch (xs & 7) {     // the loads sit inside the cases so that they write the slot registers directly
+#define PSWF_LOAD(K)                         \
+  case K:                                    \
+    unpack<CB>(__ldg(g0 + off), win[K][0]);  \
+    unpack<CB>(__ldg(g1 + off), win[K][1]);  \
     break;
       PSWF_LOAD(0) PSWF_LOAD(1) PSWF_LOAD(2) PSWF_LOAD(3)
       PSWF_LOAD(4) PSWF_LOAD(5) PSWF_LOAD(6) PSWF_LOAD(7)
@@ -208,29 +234,47 @@ __global__ void __launch_bounds__(32 * GBY * GBZ, 2)
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
+size_t gather_grid_bytes(const pswf_lr_plan* p) {
+  // interleaved copy of the potential grid: channel groups of 4 (last group 1, 2 or 4 wide)
+  const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
+  size_t fl = 0;
+  for (int cb0 = 0; cb0 < p->C; cb0 += 4) {
+    const int left = p->C - cb0;
+    fl += Mtot * (left >= 3 ? 4 : left);
+  }
+  return fl * sizeof(float);
+}
+
 void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream_t st) {
   if (n <= 0) return;
   const int Mx = p->M[0], My = p->M[1], Mz = p->M[2];
+  const size_t Mtot = (size_t)Mx * My * Mz;
   const int nseg = (Mx + XSEG - 1) / XSEG;
   const int nby = (My + GBY - 1) / GBY, nbz = (Mz + GBZ - 1) / GBZ;
   const unsigned blocks = (unsigned)(nseg * nby * nbz);
+  const unsigned iblocks = (unsigned)((Mtot + 255) / 256);
   const int recf = stencil_rec_floats(p->C);
-  int cb0 = 0;
+  float* gi = (float*)p->d_gridi;
   int pass = 0;
-  while (cb0 < p->C) {
+  for (int cb0 = 0; cb0 < p->C; cb0 += 4, ++pass) {
     const int left = p->C - cb0;
     const int acc = pass > 0 ? 1 : 0;
-#define PSWF_GATHER(CBV)                                                                                    \
-  k_gather_cols<CBV><<<blocks, 32 * GBY * GBZ, 0, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nby, nbz, recf,     \
-                                                        p->d_count, (const float*)p->d_rec,                 \
-                                                        (const float*)p->d_drec, p->d_perm,                 \
-                                                        (const float*)p->d_grid, phi, F, acc)
-    if (left >= 4) { PSWF_GATHER(4); cb0 += 4; }
-    else if (left == 3) { PSWF_GATHER(3); cb0 += 3; }
-    else if (left == 2) { PSWF_GATHER(2); cb0 += 2; }
-    else { PSWF_GATHER(1); cb0 += 1; }
+    const float* planar = (const float*)p->d_grid + (size_t)cb0 * Mtot;
+#define PSWF_GATHER(CBV, NCH)                                                                               \
+  do {                                                                                                      \
+    using V = typename VecOf<CBV>::type;                                                                    \
+    k_interleave<CBV><<<iblocks, 256, 0, st>>>(Mtot, NCH, planar, (V*)gi);                                  \
+    k_gather_cols<CBV><<<blocks, 32 * GBY * GBZ, 0, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nby, nbz, recf,   \
+                                                          p->d_count, (const float*)p->d_rec,               \
+                                                          (const float*)p->d_drec, p->d_perm,               \
+                                                          (const V*)gi, phi, F, acc);                       \
+    gi += Mtot * CBV;                                                                                       \
+  } while (0)
+    if (left >= 4) PSWF_GATHER(4, 4);
+    else if (left == 3) PSWF_GATHER(4, 3);
+    else if (left == 2) PSWF_GATHER(2, 2);
+    else PSWF_GATHER(1, 1);
 #undef PSWF_GATHER
-    ++pass;
   }
 }
 

@@ -21,6 +21,7 @@ bool stencil_path_supported(const pswf_lr_plan* p);
 int stencil_rec_floats(int C);
 size_t stencil_record_bytes(const pswf_lr_plan* p);
 size_t stencil_drecord_bytes(const pswf_lr_plan* p);
+size_t gather_grid_bytes(const pswf_lr_plan* p);
 void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream_t st);
 void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
                             cudaStream_t st);

@@ -73,6 +73,7 @@ struct pswf_lr_plan {
   void* d_invW2[3] = {nullptr, nullptr, nullptr};
   // device workspaces
   void* d_grid = nullptr;         // real  [C][Mx][My][Mz]
+  void* d_gridi = nullptr;        // real  [M][CB] channel-interleaved copy of the potential grid (fast gather)
   void* d_spec = nullptr;         // cplx  [C][Mx][My][Mz/2+1]
   int* d_count = nullptr;         // [Mtot + 1] cell counts -> exclusive starts
   int* d_blocksums = nullptr;

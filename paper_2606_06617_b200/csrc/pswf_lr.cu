@@ -385,6 +385,7 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       const size_t Mhalf = (size_t)p->M[0] * p->M[1] * (p->M[2] / 2 + 1);
       if (!rc) rc = dev_alloc(&p->d_grid, rs * Mtot * p->C, &b);
       if (!rc) rc = dev_alloc(&p->d_spec, 2 * rs * Mhalf * p->C, &b);
+      if (!rc && stencil_path_supported(p)) rc = dev_alloc(&p->d_gridi, gather_grid_bytes(p), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_count, sizeof(int) * (Mtot + 1), &b);
       p->n_scan_blocks = (int)((Mtot + 4095) / 4096);
       if (!rc) rc = dev_alloc((void**)&p->d_blocksums, sizeof(int) * (size_t)p->n_scan_blocks, &b);
@@ -608,7 +609,8 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   cudaDeviceSynchronize();
   free_atoms(p);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
-                  p->d_grid,  p->d_spec,    p->d_count,    p->d_blocksums, p->d_Ech,      p->d_Etot};
+                  p->d_grid,  p->d_spec,    p->d_count,    p->d_blocksums, p->d_Ech,      p->d_Etot,
+                  p->d_gridi};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   if (p->have_fft) {
