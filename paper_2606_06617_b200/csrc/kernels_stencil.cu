@@ -69,71 +69,93 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // derivative record (24 floats, gather only): dxr[8] | dyc[8] | dzc[8], d/dr_d of the same weights
 // (derivative of the SAME panel polynomials), rotated the same way.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_scatter_records(int n, int C, int cap, int recf, const float* __restrict__ pos,
-                                                         const float* __restrict__ q, GridGeom<float> g,
-                                                         const int* __restrict__ start, const int* __restrict__ key,
-                                                         const int* __restrict__ rank, int* __restrict__ perm,
-                                                         int* __restrict__ si0, float* __restrict__ sdelta,
-                                                         float* __restrict__ sq, float* __restrict__ rec,
-                                                         float* __restrict__ drec) {
-  __shared__ float s_coef[(kMaxWindowDegree + 1) * SW];
-  __shared__ float s_dcoef[kMaxWindowDegree * SW];
-  const int w = g.w, deg = g.wdeg;
-  for (int i = threadIdx.x; i < (deg + 1) * w; i += blockDim.x) s_coef[i] = g.wcoef[i];
-  for (int i = threadIdx.x; i < deg * w; i += blockDim.x) s_dcoef[i] = g.wdcoef[i];
-  __syncthreads();
+// rotate right by s: out[k] = v[(k - s) & 7], three conditional stages (24 selects)
+__device__ __forceinline__ void rotate8(float (&v)[SW], int s) {
+  float t[SW];
+  const bool r4 = s & 4, r2 = s & 2, r1 = s & 1;
+#pragma unroll
+  for (int k = 0; k < SW; ++k) t[k] = r4 ? v[(k + 4) & 7] : v[k];
+#pragma unroll
+  for (int k = 0; k < SW; ++k) v[k] = r2 ? t[(k + 6) & 7] : t[k];
+#pragma unroll
+  for (int k = 0; k < SW; ++k) t[k] = r1 ? v[(k + 7) & 7] : v[k];
+#pragma unroll
+  for (int k = 0; k < SW; ++k) v[k] = t[k];
+}
+
+// perm[sorted slot] = atom: the only scattered write of the sort (4 bytes per atom).
+__global__ void __launch_bounds__(256) k_perm(int n, const int* __restrict__ start, const int* __restrict__ key,
+                                              const int* __restrict__ rank, int* __restrict__ perm) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const int dst = start[key[i]] + rank[i];
-  perm[dst] = i;
-  float* r = rec + (size_t)dst * recf;
-  float* dr = drec + (size_t)dst * (3 * SW);
+  if (i < n) perm[__ldg(start + __ldg(key + i)) + __ldg(rank + i)] = i;
+}
+
+// One thread per SORTED slot j: gathers pos / q of atom perm[j] (random 32-byte reads out of L2; the
+// inputs fit it), builds the records and leaves them through shared memory so that the CTA writes
+// 128 consecutive records with fully coalesced 16-byte stores.  (Scattering finished records from
+// atom order cost 300 us: 17 partially written sectors per atom; profiles/r1b.)
+//
+// The panel polynomials arrive BY VALUE (kernel parameter space = constant bank): with the panel
+// index and the power static, every Horner step is one FFMA with a constant-bank operand and no
+// coefficient load.  The rotation by the cell index is done on the finished weights in registers.
+constexpr int kRecThreads = 128;
+
+__global__ void __launch_bounds__(kRecThreads) k_records(int n, int C, int recf, const float* __restrict__ pos,
+                                                         const float* __restrict__ q, GridGeom<float> g,
+                                                         const __grid_constant__ WindowPoly P,
+                                                         const int* __restrict__ perm, float* __restrict__ rec,
+                                                         float* __restrict__ drec) {
+  extern __shared__ __align__(16) float s_stage[];   // [kRecThreads][recf] | [kRecThreads][24]
+  float* s_rec = s_stage;
+  float* s_drec = s_stage + kRecThreads * recf;
+  const int j0 = blockIdx.x * kRecThreads;
+  const int j = j0 + threadIdx.x;
+  if (j < n) {
+    const int i = __ldg(perm + j);
+    float* r = s_rec + threadIdx.x * recf;
+    float* dr = s_drec + threadIdx.x * (3 * SW);
+    const float px[3] = {__ldg(pos + 3 * (size_t)i), __ldg(pos + 3 * (size_t)i + 1), __ldg(pos + 3 * (size_t)i + 2)};
+    for (int c0 = 0; c0 < recf - 3 * SW; c0 += 4) {
+      float qq[4];
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    int i0;
-    double delta;
-    stencil_1d((double)pos[3 * (size_t)i + d], g.invL[d], g.M[d], w, i0, delta);
-    si0[(size_t)d * cap + dst] = i0;
-    const float df = (float)delta;
-    sdelta[(size_t)d * cap + dst] = df;
-    const int s = wrap_index(i0, g.M[d]);
-    const float xi = 2.f * df - 1.f;
-    float v[SW], dv[SW];
+      for (int u = 0; u < 4; ++u) qq[u] = c0 + u < C ? __ldg(q + (size_t)(c0 + u) * n + i) : 0.f;
+      reinterpret_cast<float4*>(r + 3 * SW)[c0 >> 2] = make_float4(qq[0], qq[1], qq[2], qq[3]);
+    }
 #pragma unroll
-    for (int k = 0; k < SW; ++k) {
-      const int t = (k - s) & (SW - 1);
-      float a = 0.f, b = 0.f;
-      if (t < w) {
-        a = s_coef[deg * w + t];
-        b = s_dcoef[(deg - 1) * w + t];
-        for (int m = deg - 1; m >= 1; --m) {
-          a = fmaf(a, xi, s_coef[m * w + t]);
-          b = fmaf(b, xi, s_dcoef[(m - 1) * w + t]);
+    for (int d = 0; d < 3; ++d) {
+      int i0;
+      double delta;
+      stencil_1d((double)px[d], g.invL[d], g.M[d], g.w, i0, delta);
+      const int s = wrap_index(i0, g.M[d]);
+      const float xi = 2.f * (float)delta - 1.f;
+      float v[SW], dv[SW];
+#pragma unroll
+      for (int t = 0; t < SW; ++t) {
+        float a = P.c[kFastWindowDegree][t], b = P.d[kFastWindowDegree - 1][t];
+#pragma unroll
+        for (int m = kFastWindowDegree - 1; m >= 1; --m) {
+          a = fmaf(a, xi, P.c[m][t]);
+          b = fmaf(b, xi, P.d[m - 1][t]);
         }
-        a = fmaf(a, xi, s_coef[t]);
+        a = fmaf(a, xi, P.c[0][t]);
+        v[t] = a;
+        dv[t] = b * g.dxi_dr[d];
       }
-      v[k] = a;
-      dv[k] = b * g.dxi_dr[d];
+      rotate8(v, s);
+      rotate8(dv, s);
+      reinterpret_cast<float4*>(r)[2 * d] = make_float4(v[0], v[1], v[2], v[3]);
+      reinterpret_cast<float4*>(r)[2 * d + 1] = make_float4(v[4], v[5], v[6], v[7]);
+      reinterpret_cast<float4*>(dr)[2 * d] = make_float4(dv[0], dv[1], dv[2], dv[3]);
+      reinterpret_cast<float4*>(dr)[2 * d + 1] = make_float4(dv[4], dv[5], dv[6], dv[7]);
     }
-    reinterpret_cast<float4*>(r)[2 * d] = make_float4(v[0], v[1], v[2], v[3]);
-    reinterpret_cast<float4*>(r)[2 * d + 1] = make_float4(v[4], v[5], v[6], v[7]);
-    reinterpret_cast<float4*>(dr)[2 * d] = make_float4(dv[0], dv[1], dv[2], dv[3]);
-    reinterpret_cast<float4*>(dr)[2 * d + 1] = make_float4(dv[4], dv[5], dv[6], dv[7]);
   }
-  for (int c0 = 0; c0 < recf - 3 * SW; c0 += 4) {
-    float qq[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int c = c0 + u;
-      float t = 0.f;
-      if (c < C) {
-        t = q[(size_t)c * n + i];
-        sq[(size_t)c * cap + dst] = t;
-      }
-      qq[u] = t;
-    }
-    reinterpret_cast<float4*>(r + 3 * SW)[c0 >> 2] = make_float4(qq[0], qq[1], qq[2], qq[3]);
-  }
+  __syncthreads();
+  const int nrec = min(kRecThreads, n - j0);
+  const int rq = recf >> 2;
+  float4* grec = reinterpret_cast<float4*>(rec + (size_t)j0 * recf);
+  float4* gdrec = reinterpret_cast<float4*>(drec + (size_t)j0 * (3 * SW));
+  for (int t = threadIdx.x; t < nrec * rq; t += kRecThreads) grec[t] = reinterpret_cast<const float4*>(s_rec)[t];
+  for (int t = threadIdx.x; t < nrec * 6; t += kRecThreads) gdrec[t] = reinterpret_cast<const float4*>(s_drec)[t];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -410,7 +432,7 @@ int stencil_rec_floats(int C) {
 }
 
 bool stencil_path_supported(const pswf_lr_plan* p) {
-  if (p->precision != PSWF_LR_F32 || p->w > SW) return false;
+  if (p->precision != PSWF_LR_F32 || p->w > SW || p->wt.degree > kFastWindowDegree) return false;
   for (int d = 0; d < 3; ++d)
     if (p->M[d] % SW != 0 || p->M[d] < 2 * SW) return false;
   return true;
@@ -422,10 +444,16 @@ size_t stencil_drecord_bytes(const pswf_lr_plan*) { return sizeof(float) * 3 * S
 void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
                             cudaStream_t st) {
   if (n <= 0) return;
-  k_scatter_records<<<(n + 255) / 256, 256, 0, st>>>(n, p->C, p->cap_atoms, stencil_rec_floats(p->C), pos, q, g,
-                                                     p->d_count, p->d_key, p->d_rank, p->d_perm, p->d_si0,
-                                                     (float*)p->d_sdelta, (float*)p->d_sq, (float*)p->d_rec,
-                                                     (float*)p->d_drec);
+  const int recf = stencil_rec_floats(p->C);
+  k_perm<<<(n + 255) / 256, 256, 0, st>>>(n, p->d_count, p->d_key, p->d_rank, p->d_perm);
+  const size_t sm = sizeof(float) * kRecThreads * (size_t)(recf + 3 * SW);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_records, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    attr_set = true;
+  }
+  k_records<<<(n + kRecThreads - 1) / kRecThreads, kRecThreads, sm, st>>>(n, p->C, recf, pos, q, g, p->wpoly, p->d_perm,
+                                                                        (float*)p->d_rec, (float*)p->d_drec);
 }
 
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {
@@ -436,11 +464,16 @@ void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {
   const size_t budget = 74 * 1024;
   int cap = (int)((budget - L::S::kHeader - L::S::kTables) / (2 * (size_t)recf * 4));
   cap &= ~7;
-  // x segments: enough CTAs to fill the machine, as long as possible (each segment re-reads 7 halo planes)
+  // x segments: ONE wave of CTAs (3 resident per SM).  Every segment re-reads 7 halo planes, so the
+  // segments are as long as a single wave allows; a second, partly filled wave costs a full segment
+  // time (512 CTAs on 444 slots ran 2 x 23 planes instead of 1 x 29; profiles/r1b).
   const int Mx = p->M[0];
   const int npatch = ((p->M[1] + L::S::TY - 1) / L::S::TY) * ((p->M[2] + L::S::TZ - 1) / L::S::TZ);
-  int XS = Mx;
-  while (XS > 16 && npatch * ((Mx + XS - 1) / XS) < 2 * p->sm_count) XS = ((XS / 2 + 7) / 8) * 8;
+  const int slots = 3 * p->sm_count;
+  int nseg = slots / npatch;
+  if (nseg < 1) nseg = 1;
+  int XS = (Mx + nseg - 1) / nseg;
+  if (XS < 8) XS = 8;
   int cb0 = 0;
   while (cb0 < p->C) {
     const int left = p->C - cb0;

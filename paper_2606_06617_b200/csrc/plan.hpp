@@ -15,6 +15,14 @@ constexpr int kMaxW = 16;
 constexpr int kMaxWindowDegree = 30;
 constexpr int kMaxKernelDegree = 24;
 constexpr int kProfileRing = 512;
+constexpr int kFastWindowDegree = 12;   // fast fp32 path: panel polynomials zero-padded to this degree
+
+// Window panel polynomials of the fast fp32 path, passed to kernels by value (constant bank):
+// c[m][t] = coefficient of xi^m of panel t (zero for t >= w or m > degree); d = d/dxi of the same.
+struct WindowPoly {
+  float c[kFastWindowDegree + 1][8];
+  float d[kFastWindowDegree][8];
+};
 
 // Parameters of the scale (deconvolve x Green) kernel, passed by value.
 template <class T>
@@ -66,6 +74,7 @@ struct pswf_lr_plan {
   // host tables
   pswf::WindowTable wt;
   pswf::KernelTable kt;
+  pswf::WindowPoly wpoly;         // fast path copy of wt (float, zero padded)
   // device tables (plan precision)
   void* d_wcoef = nullptr;
   void* d_wdcoef = nullptr;

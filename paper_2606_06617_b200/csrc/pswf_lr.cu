@@ -315,6 +315,12 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       // window: psi_0^{c_w}, panel polynomials, W^ tables (Eq. (21)-(22))
       Pswf0 psi_w(p->c_w);
       p->wt = fit_window(psi_w, w, p->poly_eps, kMaxWindowDegree);
+      memset(&p->wpoly, 0, sizeof(p->wpoly));
+      if (w <= 8 && p->wt.degree <= kFastWindowDegree)
+        for (int t = 0; t < w; ++t) {
+          for (int m = 0; m <= p->wt.degree; ++m) p->wpoly.c[m][t] = (float)p->wt.coef[(size_t)m * w + t];
+          for (int m = 0; m < p->wt.degree; ++m) p->wpoly.d[m][t] = (float)p->wt.dcoef[(size_t)m * w + t];
+        }
       p->What0 = 1;
       const double kc = c / p->r_c;
       for (int d = 0; d < 3; ++d) {
