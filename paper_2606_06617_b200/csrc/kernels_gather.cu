@@ -4,26 +4,32 @@
 // derivative of the SAME panel polynomials),  F_i = - sum_a q_i^a grad phi_i^a.
 // 4 w^3 C flops per atom and ~0.5 atoms per grid cell: bound by FP32 issue, not by HBM.
 //
-// Design: INPUT-STATIONARY IN REGISTERS, one warp per column of stencil cells.
-//  * a warp owns the cells (s_x, s_y, s_z), s_x in one x segment, of one (s_y, s_z) column.  Every
-//    atom of those cells reads the same 8 x 8 (y,z) footprint, two points per lane, so all 32 lanes
-//    work on every atom and the per-atom sums are a warp shuffle reduction (no atomics);
-//  * the 8 x-planes an atom can touch live in a register window win[8][2][CB]; slot k holds the plane
-//    x == k (mod 8).  The per-atom weight records written by k_scatter_records hold wx and dwx/dx
-//    ROTATED by the atom's cell index mod 8, so the x contraction is sum_k wxr[k] * win[k] with static
-//    register indices: one copy of the atom code, no unrolled window rotation (the first tiled
-//    kernel's 118 KB of SASS thrashed the instruction cache, profiles/r1a);
-//  * the potential grid is first copied from cuFFT's planar layout [C][M] into a channel-interleaved
-//    one [M][CB] (k_interleave, L2-resident, ~10 us), so that one 16-byte load per footprint point
-//    refreshes the slot that left the window for all channels (with planar loads the address
-//    arithmetic of 8 scalar loads per x step was a third of all instructions, profiles/r1c);
-//    the loads are served by L1: neighbouring columns of the CTA share 7/8 of their footprint;
-//  * the lanes of a segment fetch the cell boundaries of its 32 cells at once, prefetch the
-//    records of the non-empty cells to L2, skip leading / trailing empty cells and return at once
-//    when the segment holds no atoms (vacuum of configuration 5);
-//  * per atom: x contraction with value and derivative weights in one pass (2 x 8 x 2 FFMA per
-//    channel per lane), combination with the (y,z) weights, 9-shuffle transpose-reduce of
+// Design: INPUT-STATIONARY IN REGISTERS, one warp per ROW of stencil cells, swept
+// along z -- the direction in which the cell-sorted atoms are contiguous.
+//  * a warp owns the cells (s_x, s_y, s_z), s_z in one 32-cell segment.  Their atoms are ONE
+//    contiguous run of the sorted arrays, so records and permutation entries stream through L1
+//    (prefetched a few atoms ahead) instead of costing an L2 round trip per atom (v2, profiles/r1b:
+//    a quarter of the kernel time was spent waiting for per-atom record loads);
+//  * every atom of those cells reads the same 8 x 8 (x,y) footprint, two points per lane, so all 32
+//    lanes work on every atom and the per-atom sums are a warp shuffle reduction (no atomics);
+//  * the 8 z-planes an atom can touch live in a register window win[8][2][CB]; slot k holds the plane
+//    z == k (mod 8).  The weight records hold wz and dwz/dz ROTATED by the atom's cell index mod 8,
+//    so the z contraction is sum_k wzr[k] * win[k] with static register indices: one copy of the
+//    atom code, no unrolled window rotation;
+//  * the potential grid is first copied from cuFFT's planar layout [C][x][y][z] into a transposed,
+//    channel-interleaved one [z][x][y][CB] (k_interleave_t, L2-resident), so that a z-plane is
+//    contiguous and one 16-byte load per footprint point refreshes the slot that left the window
+//    for all channels.  The plane of the NEXT step is loaded one step ahead into scratch registers
+//    and the one after that is touched in L1, so that empty cells do not expose load latency;
+//    neighbouring rows of the CTA share 7/8 of their footprint in L1;
+//  * the lanes of a segment fetch the cell boundaries of its 32 cells at once, skip leading /
+//    trailing empty cells and return at once when the segment holds no atoms (vacuum of
+//    configuration 5);
+//  * per atom: z contraction with value and derivative weights in one pass (2 x 8 x 2 FFMA per
+//    channel per lane), combination with the (x,y) weights, 9-shuffle transpose-reduce of
 //    (phi_a, F_x, F_y, F_z), scattered store to the caller's atom order.
+#include <cstdlib>
+
 #include "kernels_common.cuh"
 #include "launch.hpp"
 
@@ -32,8 +38,8 @@ namespace pswf {
 namespace {
 
 constexpr int SW = 8;        // stencil slots per dimension
-constexpr int XSEG = 32;     // cells per x segment: one lane per cell boundary pair
-constexpr int GBY = 2, GBZ = 4;   // cell columns per CTA (y x z): 8 warps
+constexpr int ZSEG = 32;     // cells per z segment: one lane per cell boundary pair
+constexpr int GBX = 2, GBY = 4;   // cell rows per CTA (x by y): 8 warps
 
 template <int CB> struct VecOf;
 template <> struct VecOf<1> { using type = float; };
@@ -47,18 +53,38 @@ __device__ __forceinline__ void unpack(const typename VecOf<CB>::type& v, float 
   else { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
 }
 
-// planar [C][M] -> interleaved [M][CB] for the channels cb0 .. cb0+CB-1 (missing channels read as 0)
+// planar [C][x][y][z] -> transposed + interleaved [z][x][y][CB] for the channels cb0 .. cb0+CB-1
+// (missing channels read as 0).  One CTA per (x, 32 x 32 tile of (y,z)); reads coalesced along z,
+// writes coalesced along y.
 template <int CB>
-__global__ void __launch_bounds__(256) k_interleave(size_t Mtot, int nch, const float* __restrict__ planar,
-                                                    typename VecOf<CB>::type* __restrict__ out) {
-  const size_t m = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (m >= Mtot) return;
-  float v[CB];
+__global__ void __launch_bounds__(256) k_interleave_t(int Mx, int My, int Mz, int nch, const float* __restrict__ planar,
+                                                      typename VecOf<CB>::type* __restrict__ out) {
+  __shared__ float tile[CB][32][33];
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const int z0 = blockIdx.x * 32, y0 = blockIdx.y * 32, x = blockIdx.z;
+  const size_t Mtot = (size_t)Mx * My * Mz;
 #pragma unroll
-  for (int c = 0; c < CB; ++c) v[c] = c < nch ? __ldg(planar + (size_t)c * Mtot + m) : 0.f;
-  if constexpr (CB == 1) out[m] = v[0];
-  else if constexpr (CB == 2) out[m] = make_float2(v[0], v[1]);
-  else out[m] = make_float4(v[0], v[1], v[2], v[3]);
+  for (int c = 0; c < CB; ++c)
+#pragma unroll
+    for (int yy = ty; yy < 32; yy += 8) {
+      float v = 0.f;
+      if (c < nch && y0 + yy < My && z0 + tx < Mz)
+        v = __ldg(planar + (size_t)c * Mtot + ((size_t)x * My + (y0 + yy)) * Mz + z0 + tx);
+      tile[c][yy][tx] = v;
+    }
+  __syncthreads();
+#pragma unroll
+  for (int zz = ty; zz < 32; zz += 8) {
+    if (y0 + tx < My && z0 + zz < Mz) {
+      float v[CB];
+#pragma unroll
+      for (int c = 0; c < CB; ++c) v[c] = tile[c][tx][zz];
+      const size_t o = ((size_t)(z0 + zz) * Mx + x) * My + y0 + tx;
+      if constexpr (CB == 1) out[o] = v[0];
+      else if constexpr (CB == 2) out[o] = make_float2(v[0], v[1]);
+      else out[o] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+  }
 }
 
 // 9-shuffle transpose-reduce of 8 values over the 32 lanes; on return lane l holds in v[0] the full
@@ -89,144 +115,206 @@ __device__ __forceinline__ float reduce8(float (&v)[8], int lane) {
   return v[0];
 }
 
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+__device__ __forceinline__ void prefetch_l1(const void* p) {
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
 }
 
-template <int CB>
-__global__ void __launch_bounds__(32 * GBY * GBZ, 2)
-    k_gather_cols(int n, int C, int cb0, int Mx, int My, int Mz, int nseg, int nby, int nbz, int recf,
+constexpr int kStage = 32;       // atoms staged per warp at a time (one lane per atom for the output pass)
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)),
+               "l"(gsrc)
+               : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// floats of shared memory per warp: kStage records, kStage derivative records, kStage x 8 results
+__host__ __device__ constexpr int gather_warp_floats(int recf) { return kStage * (recf + 3 * SW + 8); }
+
+template <int CB, int PF>
+__global__ void __launch_bounds__(32 * GBX * GBY, 2)
+    k_gather_rows(int n, int C, int cb0, int Mx, int My, int Mz, int nbx, int nby, int recf,
                   const int* __restrict__ start, const float* __restrict__ rec, const float* __restrict__ drec,
-                  const int* __restrict__ perm, const typename VecOf<CB>::type* __restrict__ gridi,
+                  const int* __restrict__ perm, const typename VecOf<CB>::type* __restrict__ gridt,
                   float* __restrict__ phi, float* __restrict__ Facc, int accumulate_F) {
   using V = typename VecOf<CB>::type;
+  extern __shared__ __align__(16) float s_all[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  // block -> (segment, y block, z block); consecutive blocks walk z, then y: CTAs resident on an SM
+  float* s_rec = s_all + (size_t)wid * gather_warp_floats(recf);   // [kStage][recf]
+  float* s_drec = s_rec + kStage * recf;                            // [kStage][24]
+  float* s_out = s_drec + kStage * 3 * SW;                          // [kStage][8]
+  // block -> (z segment, x block, y block); consecutive blocks walk y, then x: CTAs resident on an SM
   // at the same time share most of their footprints in L1
   int bid = blockIdx.x;
-  const int bz = bid % nbz; bid /= nbz;
   const int by = bid % nby; bid /= nby;
+  const int bx = bid % nbx; bid /= nbx;
   const int seg = bid;
-  const int sy = by * GBY + wid / GBZ, sz = bz * GBZ + wid % GBZ;
-  if (sy >= My || sz >= Mz) return;
-  const int X0 = seg * XSEG, X1 = min(X0 + XSEG, Mx);
+  const int sx = bx * GBX + wid / GBY, sy = by * GBY + wid % GBY;
+  if (sx >= Mx || sy >= My) return;
+  const int Z0 = seg * ZSEG, Z1 = min(Z0 + ZSEG, Mz);
 
-  // cell boundaries of the segment: lane l <-> cell X0 + l
+  // cell boundaries of the segment: lane l <-> cell Z0 + l; the atoms of the row are one run
   int jlo_l = 0, jhi_l = 0;
-  if (X0 + lane < X1) {
-    const size_t key = ((size_t)(X0 + lane) * My + sy) * Mz + sz;
+  if (Z0 + lane < Z1) {
+    const size_t key = ((size_t)sx * My + sy) * Mz + Z0 + lane;
     jlo_l = __ldg(start + key);
     jhi_l = __ldg(start + key + 1);
   }
   const unsigned mask = __ballot_sync(0xffffffffu, jhi_l > jlo_l);
-  if (mask == 0u) return;   // no atoms in this segment of the column (vacuum)
-  if (jhi_l > jlo_l) {
-    const float* r = rec + (size_t)jlo_l * recf;
-    prefetch_l2(r);
-    prefetch_l2(r + 32);
-    prefetch_l2(drec + (size_t)jlo_l * (3 * SW));
-  }
+  if (mask == 0u) return;   // no atoms in this segment of the row (vacuum)
   const int first = __ffs(mask) - 1, last = 31 - __clz(mask);
+  const int jbeg = __shfl_sync(0xffffffffu, jlo_l, first), jend = __shfl_sync(0xffffffffu, jhi_l, last);
 
-  // lane -> 2 (b, c) points of the 8 x 8 (y,z) footprint: c = lane & 7, b = (lane >> 3) + 4u
-  const int c_off = lane & 7, b0 = lane >> 3;
-  int iz = sz + c_off; if (iz >= Mz) iz -= Mz;
-  int iy0 = sy + b0;      if (iy0 >= My) iy0 -= My;
-  int iy1 = sy + b0 + 4;  if (iy1 >= My) iy1 -= My;
-  const unsigned plane = (unsigned)My * Mz;
-  const V* g0 = gridi + (size_t)iy0 * Mz + iz;
-  const V* g1 = gridi + (size_t)iy1 * Mz + iz;
-  // record offsets of this lane's (y,z) weights (records are rotated by the cell index mod 8)
-  const int oy0 = SW + ((sy + b0) & 7), oy1 = SW + ((sy + b0 + 4) & 7), oz = 2 * SW + ((sz + c_off) & 7);
-
-  float win[SW][2][CB];
-  auto load_plane = [&](int xs) {
-    int x = xs; if (x >= Mx) x -= Mx;
-    const unsigned off = (unsigned)x * plane;
-    switch (xs & 7) {     // the loads sit inside the cases so that they write the slot registers directly
-#define PSWF_LOAD(K)                         \
-  case K:                                    \
-    unpack<CB>(__ldg(g0 + off), win[K][0]);  \
-    unpack<CB>(__ldg(g1 + off), win[K][1]);  \
-    break;
-      PSWF_LOAD(0) PSWF_LOAD(1) PSWF_LOAD(2) PSWF_LOAD(3)
-      PSWF_LOAD(4) PSWF_LOAD(5) PSWF_LOAD(6) PSWF_LOAD(7)
-#undef PSWF_LOAD
-    }
+  // stage the records of atoms [js, js + kStage) of the run: asynchronous 16-byte copies, one
+  // contiguous stream for rec and one for drec; lane l keeps the permutation entry of atom js + l
+  int js = jbeg, perm_l = 0;
+  auto stage = [&]() {
+    const int cnt = min(kStage, jend - js);
+    const float4* gr = reinterpret_cast<const float4*>(rec + (size_t)js * recf);
+    const float4* gd = reinterpret_cast<const float4*>(drec + (size_t)js * (3 * SW));
+    const int nr = cnt * (recf >> 2), nd = cnt * 6;
+    for (int t = lane; t < nr; t += 32) cp_async16(reinterpret_cast<float4*>(s_rec) + t, gr + t);
+    for (int t = lane; t < nd; t += 32) cp_async16(reinterpret_cast<float4*>(s_drec) + t, gd + t);
+    perm_l = lane < cnt ? __ldg(perm + js + lane) : 0;
   };
+  // write the results of the staged atoms: lane l <-> atom js + l, scattered to the caller's order
+  auto flush = [&](int cnt) {
+    __syncwarp();
+    if (lane < cnt) {
+      const float4 a = *reinterpret_cast<const float4*>(s_out + 8 * lane);
+      const float4 f = *reinterpret_cast<const float4*>(s_out + 8 * lane + 4);
+      const float pv[4] = {a.x, a.y, a.z, a.w};
+      if (phi) {
 #pragma unroll
-  for (int k = 0; k < SW; ++k)
-#pragma unroll
-    for (int u = 0; u < 2; ++u)
-#pragma unroll
-      for (int c = 0; c < CB; ++c) win[k][u][c] = 0.f;
-
-  // warm-up: planes sx0 .. sx0+6 of the first non-empty cell
-  const int sx0 = X0 + first, sx1 = X0 + last;
-  for (int a = 0; a < SW - 1; ++a) load_plane(sx0 + a);
-
-  for (int sx = sx0; sx <= sx1; ++sx) {
-    load_plane(sx + SW - 1);
-    if (!((mask >> (sx - X0)) & 1u)) continue;
-    const int jlo = __shfl_sync(0xffffffffu, jlo_l, sx - X0);
-    const int jhi = __shfl_sync(0xffffffffu, jhi_l, sx - X0);
-    for (int j = jlo; j < jhi; ++j) {
-      const float* r = rec + (size_t)j * recf;
-      const float* dr = drec + (size_t)j * (3 * SW);
-      const float4 xa = __ldg(reinterpret_cast<const float4*>(r));
-      const float4 xb = __ldg(reinterpret_cast<const float4*>(r) + 1);
-      const float4 da = __ldg(reinterpret_cast<const float4*>(dr));
-      const float4 db = __ldg(reinterpret_cast<const float4*>(dr) + 1);
-      const float4 q4 = __ldg(reinterpret_cast<const float4*>(r + 3 * SW) + (cb0 >> 2));
-      const float wy0 = __ldg(r + oy0), wy1 = __ldg(r + oy1), wz = __ldg(r + oz);
-      const float dy0 = __ldg(dr + oy0), dy1 = __ldg(dr + oy1), dz = __ldg(dr + oz);
-      const float wx[SW] = {xa.x, xa.y, xa.z, xa.w, xb.x, xb.y, xb.z, xb.w};
-      const float dx[SW] = {da.x, da.y, da.z, da.w, db.x, db.y, db.z, db.w};
-      const float qv[4] = {q4.x, q4.y, q4.z, q4.w};
-      const float yz[2] = {wy0 * wz, wy1 * wz};
-      const float dyz[2] = {dy0 * wz, dy1 * wz};
-      const float ydz[2] = {wy0 * dz, wy1 * dz};
-      float red[8];
-      float fx = 0.f, fy = 0.f, fz = 0.f;
-#pragma unroll
-      for (int c = 0; c < CB; ++c) {
-        float val = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-          float S0 = 0.f, S1 = 0.f;
-#pragma unroll
-          for (int k = 0; k < SW; ++k) {
-            S0 = fmaf(wx[k], win[k][u][c], S0);
-            S1 = fmaf(dx[k], win[k][u][c], S1);
-          }
-          val = fmaf(yz[u], S0, val);
-          gx = fmaf(yz[u], S1, gx);
-          gy = fmaf(dyz[u], S0, gy);
-          gz = fmaf(ydz[u], S0, gz);
-        }
-        const float qc = qv[c];
-        fx = fmaf(-qc, gx, fx);
-        fy = fmaf(-qc, gy, fy);
-        fz = fmaf(-qc, gz, fz);
-        red[c] = val;
+        for (int c = 0; c < CB; ++c)
+          if (cb0 + c < C) phi[(size_t)(cb0 + c) * n + perm_l] = pv[c];
       }
-#pragma unroll
-      for (int c = CB; c < 4; ++c) red[c] = 0.f;
-      red[4] = fx; red[5] = fy; red[6] = fz; red[7] = 0.f;
-      const float tot = reduce8(red, lane);
-      // lane l with (l & 3) == 0 holds output index (l>>4)*4 + ((l>>3)&1)*2 + ((l>>2)&1)
-      if ((lane & 3) == 0) {
-        const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
-        const int dst = __ldg(perm + j);
-        if (idx < CB) {
-          if (phi && cb0 + idx < C) phi[(size_t)(cb0 + idx) * n + dst] = tot;
-        } else if (idx >= 4 && idx < 7 && Facc) {
-          float* fp = Facc + 3 * (size_t)dst + (idx - 4);
-          *fp = accumulate_F ? (*fp + tot) : tot;
-        }
+      if (Facc) {
+        float* fp = Facc + 3 * (size_t)perm_l;
+        if (accumulate_F) { fp[0] += f.x; fp[1] += f.y; fp[2] += f.z; }
+        else { fp[0] = f.x; fp[1] = f.y; fp[2] = f.z; }
       }
+    }
+    __syncwarp();
+  };
+  stage();
+
+  // lane -> 2 points of the 8 x 8 (x,y) footprint: y offset c = lane & 7, x offsets b and b + 4
+  const int c_off = lane & 7, b0 = lane >> 3;
+  int iy = sy + c_off;      if (iy >= My) iy -= My;
+  int ix0 = sx + b0;        if (ix0 >= Mx) ix0 -= Mx;
+  int ix1 = sx + b0 + 4;    if (ix1 >= Mx) ix1 -= Mx;
+  const unsigned plane = (unsigned)Mx * My, wrap = plane * (unsigned)Mz;
+  const V* g0 = gridt + (size_t)ix0 * My + iy;
+  const V* g1 = gridt + (size_t)ix1 * My + iy;
+  // record offsets of this lane's (x,y) weights (records are rotated by the cell index mod 8)
+  const int ox0 = (sx + b0) & 7, ox1 = ox0 ^ 4, oy = SW + ((sy + c_off) & 7);
+
+  // warm-up: the 8 planes sz0 .. sz0+7 of the first non-empty cell, slot k <- the plane z == k (mod 8)
+  // (static slots: 16 independent loads in flight, straight into the window registers)
+  const int sz0 = Z0 + first, sz1 = Z0 + last;
+  float win[SW][2][CB];
+#pragma unroll
+  for (int k = 0; k < SW; ++k) {
+    int z = sz0 + ((k - sz0) & 7); if (z >= Mz) z -= Mz;
+    const unsigned off = (unsigned)z * plane;
+    unpack<CB>(__ldg(g0 + off), win[k][0]);
+    unpack<CB>(__ldg(g1 + off), win[k][1]);
+  }
+  // offset of the plane that enters the window next, and of the one PF steps further on
+  unsigned off_n = (unsigned)((sz0 + SW) % Mz) * plane;
+  unsigned off_p = (unsigned)((sz0 + SW + PF) % Mz) * plane;
+  if constexpr (PF > 0) {
+#pragma unroll
+    for (int a = 0; a < PF; ++a) {
+      const unsigned off = (unsigned)((sz0 + SW + a) % Mz) * plane;
+      prefetch_l1(g0 + off);
+      prefetch_l1(g1 + off);
     }
   }
+  cp_async_wait_all();
+  __syncwarp();
+
+  for (int sz = sz0; sz <= sz1; ++sz) {
+    if constexpr (PF > 0) {   // touch in L1 the plane that enters the window PF steps from now
+      prefetch_l1(g0 + off_p);
+      prefetch_l1(g1 + off_p);
+      off_p += plane; if (off_p == wrap) off_p = 0u;
+    }
+    if ((mask >> (sz - Z0)) & 1u) {
+      const int jlo = __shfl_sync(0xffffffffu, jlo_l, sz - Z0);
+      const int jhi = __shfl_sync(0xffffffffu, jhi_l, sz - Z0);
+      for (int j = jlo; j < jhi; ++j) {
+        if (j - js >= kStage) {   // staging buffer exhausted (dense rows): write results, stage the next atoms
+          flush(kStage);
+          js += kStage;
+          stage();
+          cp_async_wait_all();
+          __syncwarp();
+        }
+        const float* r = s_rec + (j - js) * recf;
+        const float* dr = s_drec + (j - js) * (3 * SW);
+        const float4 za = *reinterpret_cast<const float4*>(r + 2 * SW);
+        const float4 zb = *reinterpret_cast<const float4*>(r + 2 * SW + 4);
+        const float4 da = *reinterpret_cast<const float4*>(dr + 2 * SW);
+        const float4 db = *reinterpret_cast<const float4*>(dr + 2 * SW + 4);
+        const float4 q4 = *reinterpret_cast<const float4*>(r + 3 * SW + cb0);
+        const float wx0 = r[ox0], wx1 = r[ox1], wy = r[oy];
+        const float dx0 = dr[ox0], dx1 = dr[ox1], dy = dr[oy];
+        const float wz[SW] = {za.x, za.y, za.z, za.w, zb.x, zb.y, zb.z, zb.w};
+        const float dz[SW] = {da.x, da.y, da.z, da.w, db.x, db.y, db.z, db.w};
+        const float qv[4] = {q4.x, q4.y, q4.z, q4.w};
+        const float xy[2] = {wx0 * wy, wx1 * wy};      // value and d/dz
+        const float dxy[2] = {dx0 * wy, dx1 * wy};     // d/dx
+        const float xdy[2] = {wx0 * dy, wx1 * dy};     // d/dy
+        float red[8];
+        float fx = 0.f, fy = 0.f, fz = 0.f;
+#pragma unroll
+        for (int c = 0; c < CB; ++c) {
+          float val = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
+#pragma unroll
+          for (int u = 0; u < 2; ++u) {
+            float S0 = 0.f, S1 = 0.f;
+#pragma unroll
+            for (int k = 0; k < SW; ++k) {
+              S0 = fmaf(wz[k], win[k][u][c], S0);
+              S1 = fmaf(dz[k], win[k][u][c], S1);
+            }
+            val = fmaf(xy[u], S0, val);
+            gz = fmaf(xy[u], S1, gz);
+            gx = fmaf(dxy[u], S0, gx);
+            gy = fmaf(xdy[u], S0, gy);
+          }
+          const float qc = qv[c];
+          fx = fmaf(-qc, gx, fx);
+          fy = fmaf(-qc, gy, fy);
+          fz = fmaf(-qc, gz, fz);
+          red[c] = val;
+        }
+#pragma unroll
+        for (int c = CB; c < 4; ++c) red[c] = 0.f;
+        red[4] = fx; red[5] = fy; red[6] = fz; red[7] = 0.f;
+        const float tot = reduce8(red, lane);
+        // lane l with (l & 3) == 0 holds output index (l>>4)*4 + ((l>>3)&1)*2 + ((l>>2)&1)
+        if ((lane & 3) == 0)
+          s_out[8 * (j - js) + ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)] = tot;
+      }
+    }
+    if (sz < sz1) {   // the plane sz has left the window: its slot takes the plane sz + 8
+      switch (sz & 7) {   // the loads sit inside the cases: they write the slot registers directly
+#define PSWF_SLOT(K)                           \
+  case K:                                      \
+    unpack<CB>(__ldg(g0 + off_n), win[K][0]);  \
+    unpack<CB>(__ldg(g1 + off_n), win[K][1]);  \
+    break;
+        PSWF_SLOT(0) PSWF_SLOT(1) PSWF_SLOT(2) PSWF_SLOT(3)
+        PSWF_SLOT(4) PSWF_SLOT(5) PSWF_SLOT(6) PSWF_SLOT(7)
+#undef PSWF_SLOT
+      }
+      off_n += plane; if (off_n == wrap) off_n = 0u;
+    }
+  }
+  flush(jend - js);
 }
 
 }  // namespace
@@ -249,11 +337,13 @@ void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream
   if (n <= 0) return;
   const int Mx = p->M[0], My = p->M[1], Mz = p->M[2];
   const size_t Mtot = (size_t)Mx * My * Mz;
-  const int nseg = (Mx + XSEG - 1) / XSEG;
-  const int nby = (My + GBY - 1) / GBY, nbz = (Mz + GBZ - 1) / GBZ;
-  const unsigned blocks = (unsigned)(nseg * nby * nbz);
-  const unsigned iblocks = (unsigned)((Mtot + 255) / 256);
+  const int nseg = (Mz + ZSEG - 1) / ZSEG;
+  const int nbx = (Mx + GBX - 1) / GBX, nby = (My + GBY - 1) / GBY;
+  const unsigned blocks = (unsigned)(nseg * nbx * nby);
+  const dim3 iblocks((unsigned)((Mz + 31) / 32), (unsigned)((My + 31) / 32), (unsigned)Mx);
   const int recf = stencil_rec_floats(p->C);
+  const size_t smem = sizeof(float) * GBX * GBY * (size_t)gather_warp_floats(recf);
+  static const bool pf = getenv("PSWF_GATHER_PF") ? atoi(getenv("PSWF_GATHER_PF")) != 0 : false;   // experiment switch: L1 touch of planes ahead (measured: no gain)
   float* gi = (float*)p->d_gridi;
   int pass = 0;
   for (int cb0 = 0; cb0 < p->C; cb0 += 4, ++pass) {
@@ -263,11 +353,12 @@ void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream
 #define PSWF_GATHER(CBV, NCH)                                                                               \
   do {                                                                                                      \
     using V = typename VecOf<CBV>::type;                                                                    \
-    k_interleave<CBV><<<iblocks, 256, 0, st>>>(Mtot, NCH, planar, (V*)gi);                                  \
-    k_gather_cols<CBV><<<blocks, 32 * GBY * GBZ, 0, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nby, nbz, recf,   \
-                                                          p->d_count, (const float*)p->d_rec,               \
-                                                          (const float*)p->d_drec, p->d_perm,               \
-                                                          (const V*)gi, phi, F, acc);                       \
+    k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);                          \
+    auto kern = pf ? k_gather_rows<CBV, 2> : k_gather_rows<CBV, 0>;                                         \
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \
+    kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nbx, nby, recf, p->d_count,        \
+                                               (const float*)p->d_rec, (const float*)p->d_drec, p->d_perm,  \
+                                               (const V*)gi, phi, F, acc);                                  \
     gi += Mtot * CBV;                                                                                       \
   } while (0)
     if (left >= 4) PSWF_GATHER(4, 4);
