@@ -131,7 +131,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // floats of shared memory per warp: kStage records, kStage derivative records, kStage x 8 results
 __host__ __device__ constexpr int gather_warp_floats(int recf) { return kStage * (recf + 3 * SW + 8); }
 
-template <int CB, int PF>
+template <int CB>
 __global__ void __launch_bounds__(32 * GBX * GBY, 2)
     k_gather_rows(int n, int C, int cb0, int Mx, int My, int Mz, int nbx, int nby, int recf,
                   const int* __restrict__ start, const float* __restrict__ rec, const float* __restrict__ drec,
@@ -221,29 +221,17 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
     unpack<CB>(__ldg(g0 + off), win[k][0]);
     unpack<CB>(__ldg(g1 + off), win[k][1]);
   }
-  // offset of the plane that enters the window next, and of the one PF steps further on
-  unsigned off_n = (unsigned)((sz0 + SW) % Mz) * plane;
-  unsigned off_p = (unsigned)((sz0 + SW + PF) % Mz) * plane;
-  if constexpr (PF > 0) {
-#pragma unroll
-    for (int a = 0; a < PF; ++a) {
-      const unsigned off = (unsigned)((sz0 + SW + a) % Mz) * plane;
-      prefetch_l1(g0 + off);
-      prefetch_l1(g1 + off);
-    }
-  }
   cp_async_wait_all();
   __syncwarp();
 
-  for (int sz = sz0; sz <= sz1; ++sz) {
-    if constexpr (PF > 0) {   // touch in L1 the plane that enters the window PF steps from now
-      prefetch_l1(g0 + off_p);
-      prefetch_l1(g1 + off_p);
-      off_p += plane; if (off_p == wrap) off_p = 0u;
-    }
-    if ((mask >> (sz - Z0)) & 1u) {
-      const int jlo = __shfl_sync(0xffffffffu, jlo_l, sz - Z0);
-      const int jhi = __shfl_sync(0xffffffffu, jhi_l, sz - Z0);
+  // walk the non-empty cells of the segment; between two of them the window is refilled in one go
+  int cur = first;            // current cell, relative to Z0
+  unsigned rem = mask;        // non-empty cells not yet visited
+  for (;;) {
+    rem &= rem - 1u;
+    {
+      const int jlo = __shfl_sync(0xffffffffu, jlo_l, cur);
+      const int jhi = __shfl_sync(0xffffffffu, jhi_l, cur);
       for (int j = jlo; j < jhi; ++j) {
         if (j - js >= kStage) {   // staging buffer exhausted (dense rows): write results, stage the next atoms
           flush(kStage);
@@ -300,19 +288,36 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
           s_out[8 * (j - js) + ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)] = tot;
       }
     }
-    if (sz < sz1) {   // the plane sz has left the window: its slot takes the plane sz + 8
-      switch (sz & 7) {   // the loads sit inside the cases: they write the slot registers directly
-#define PSWF_SLOT(K)                           \
-  case K:                                      \
-    unpack<CB>(__ldg(g0 + off_n), win[K][0]);  \
-    unpack<CB>(__ldg(g1 + off_n), win[K][1]);  \
-    break;
-        PSWF_SLOT(0) PSWF_SLOT(1) PSWF_SLOT(2) PSWF_SLOT(3)
-        PSWF_SLOT(4) PSWF_SLOT(5) PSWF_SLOT(6) PSWF_SLOT(7)
-#undef PSWF_SLOT
-      }
-      off_n += plane; if (off_n == wrap) off_n = 0u;
+    if (rem == 0u) break;
+    // advance to the next non-empty cell nxt: the planes max(cur+8, nxt) .. nxt+7 replace the ones that
+    // left the window.  All loads of an advance are issued back to back, straight into their slot
+    // registers (Duff's device over the static slots): no per-plane dispatch, no register moves.
+    const int nxt = __ffs(rem) - 1;
+    int ps = max(cur + SW, nxt);          // first plane to load, relative to Z0
+    int cnt = nxt + SW - ps;              // 1 .. 8 planes
+    int zz = Z0 + ps;
+    while (zz >= Mz) zz -= Mz;
+    unsigned off = (unsigned)zz * plane;
+#define PSWF_SLOT(K)                         \
+  case K:                                    \
+    unpack<CB>(__ldg(g0 + off), win[K][0]);  \
+    unpack<CB>(__ldg(g1 + off), win[K][1]);  \
+    off += plane;                            \
+    if (off == wrap) off = 0u;
+    switch ((Z0 + ps) & 7) {
+      do {
+        PSWF_SLOT(0) if (--cnt == 0) break;
+        PSWF_SLOT(1) if (--cnt == 0) break;
+        PSWF_SLOT(2) if (--cnt == 0) break;
+        PSWF_SLOT(3) if (--cnt == 0) break;
+        PSWF_SLOT(4) if (--cnt == 0) break;
+        PSWF_SLOT(5) if (--cnt == 0) break;
+        PSWF_SLOT(6) if (--cnt == 0) break;
+        PSWF_SLOT(7)
+      } while (--cnt != 0);
     }
+#undef PSWF_SLOT
+    cur = nxt;
   }
   flush(jend - js);
 }
@@ -343,7 +348,6 @@ void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream
   const dim3 iblocks((unsigned)((Mz + 31) / 32), (unsigned)((My + 31) / 32), (unsigned)Mx);
   const int recf = stencil_rec_floats(p->C);
   const size_t smem = sizeof(float) * GBX * GBY * (size_t)gather_warp_floats(recf);
-  static const bool pf = getenv("PSWF_GATHER_PF") ? atoi(getenv("PSWF_GATHER_PF")) != 0 : false;   // experiment switch: L1 touch of planes ahead (measured: no gain)
   float* gi = (float*)p->d_gridi;
   int pass = 0;
   for (int cb0 = 0; cb0 < p->C; cb0 += 4, ++pass) {
@@ -354,7 +358,7 @@ void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream
   do {                                                                                                      \
     using V = typename VecOf<CBV>::type;                                                                    \
     k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);                          \
-    auto kern = pf ? k_gather_rows<CBV, 2> : k_gather_rows<CBV, 0>;                                         \
+    auto kern = k_gather_rows<CBV>;                                                                         \
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \
     kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nbx, nby, recf, p->d_count,        \
                                                (const float*)p->d_rec, (const float*)p->d_drec, p->d_perm,  \
