@@ -129,7 +129,8 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // floats of shared memory per warp: kStage records, kStage derivative records, kStage x 8 results
-__host__ __device__ constexpr int gather_warp_floats(int recf) { return kStage * (recf + 3 * SW + 8); }
+// (+ one spare result row: the sink of the software-pipelined reduction when nothing is pending)
+__host__ __device__ constexpr int gather_warp_floats(int recf) { return kStage * (recf + 3 * SW + 8) + 8; }
 
 template <int CB>
 __global__ void __launch_bounds__(32 * GBX * GBY, 2)
@@ -142,7 +143,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   float* s_rec = s_all + (size_t)wid * gather_warp_floats(recf);   // [kStage][recf]
   float* s_drec = s_rec + kStage * recf;                            // [kStage][24]
-  float* s_out = s_drec + kStage * 3 * SW;                          // [kStage][8]
+  float* s_out = s_drec + kStage * 3 * SW;                          // [kStage + 1][8]
   // block -> (z segment, x block, y block); consecutive blocks walk y, then x: CTAs resident on an SM
   // at the same time share most of their footprints in L1
   int bid = blockIdx.x;
@@ -224,6 +225,19 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
   cp_async_wait_all();
   __syncwarp();
 
+  // The lane sums of an atom are reduced across the warp one atom LATE, inside the next atom's
+  // contraction, so that the five dependent shuffle levels (~150 cycles) overlap its FFMAs.
+  float pend[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) pend[i] = 0.f;
+  // lane l with (l & 3) == 0 ends up with output index (l>>4)*4 + ((l>>3)&1)*2 + ((l>>2)&1)
+  const int out_idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+  int pend_row = kStage;   // result row of the pending atom; kStage = the spare row (nothing pending)
+  auto retire = [&]() {
+    const float tot = reduce8(pend, lane);
+    if ((lane & 3) == 0) s_out[8 * pend_row + out_idx] = tot;
+  };
+
   // walk the non-empty cells of the segment; between two of them the window is refilled in one go
   int cur = first;            // current cell, relative to Z0
   unsigned rem = mask;        // non-empty cells not yet visited
@@ -234,6 +248,8 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
       const int jhi = __shfl_sync(0xffffffffu, jhi_l, cur);
       for (int j = jlo; j < jhi; ++j) {
         if (j - js >= kStage) {   // staging buffer exhausted (dense rows): write results, stage the next atoms
+          retire();
+          pend_row = kStage;
           flush(kStage);
           js += kStage;
           stage();
@@ -255,7 +271,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
         const float xy[2] = {wx0 * wy, wx1 * wy};      // value and d/dz
         const float dxy[2] = {dx0 * wy, dx1 * wy};     // d/dx
         const float xdy[2] = {wx0 * dy, wx1 * dy};     // d/dy
-        float red[8];
+        retire();   // the previous atom's reduction: independent of everything below, interleaved by ptxas
         float fx = 0.f, fy = 0.f, fz = 0.f;
 #pragma unroll
         for (int c = 0; c < CB; ++c) {
@@ -277,15 +293,12 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
           fx = fmaf(-qc, gx, fx);
           fy = fmaf(-qc, gy, fy);
           fz = fmaf(-qc, gz, fz);
-          red[c] = val;
+          pend[c] = val;
         }
 #pragma unroll
-        for (int c = CB; c < 4; ++c) red[c] = 0.f;
-        red[4] = fx; red[5] = fy; red[6] = fz; red[7] = 0.f;
-        const float tot = reduce8(red, lane);
-        // lane l with (l & 3) == 0 holds output index (l>>4)*4 + ((l>>3)&1)*2 + ((l>>2)&1)
-        if ((lane & 3) == 0)
-          s_out[8 * (j - js) + ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)] = tot;
+        for (int c = CB; c < 4; ++c) pend[c] = 0.f;
+        pend[4] = fx; pend[5] = fy; pend[6] = fz; pend[7] = 0.f;
+        pend_row = j - js;
       }
     }
     if (rem == 0u) break;
@@ -319,6 +332,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, 2)
 #undef PSWF_SLOT
     cur = nxt;
   }
+  retire();
   flush(jend - js);
 }
 
