@@ -21,6 +21,8 @@
 //
 // Requirements of this path (host-checked): fp32, even w <= 8 (narrower windows are zero padded to 8
 // slots), M_d a multiple of 8 and >= 16.
+#include <algorithm>
+#include <climits>
 #include <cstdint>
 
 #include "kernels_common.cuh"
@@ -161,11 +163,16 @@ __global__ void __launch_bounds__(kRecThreads) k_records(int n, int C, int recf,
 // ------------------------------------------------------------------------------------------------
 // spread
 // ------------------------------------------------------------------------------------------------
+// A round = the atoms of one cell plane that are staged at once: whole cell rows [r0, r1) of the
+// plane, or -- when a single row holds more atoms than the staging buffer -- the atoms [a0, a1) of
+// the one row r0 (indices local to the row).
 struct RoundDesc {
-  int p;      // cell plane index within the segment sweep (0 .. NP-1); NP = finished
-  int r0, r1; // rows of the plane handled by this round
-  int total;  // atoms staged
-  int slow;   // 1: a single row larger than the staging buffer, read from global memory
+  int p;          // cell plane within the segment (0 .. NP-1); NP = finished
+  int r0, r1;     // rows of the plane handled by this round
+  int a0, a1;     // atom sub-range of a single-row round (0, INT_MAX otherwise)
+  int total;      // atoms staged
+  int flush;      // 1: the plane is complete after this round
+  int np, nr, na; // where the next round starts (plane, row, atom)
 };
 
 template <int WY, int WZ>
@@ -173,38 +180,48 @@ struct SpreadShape {
   static constexpr int TY = 8 * WY, TZ = 8 * WZ;
   static constexpr int NROW = TY + 7, NCELL = TZ + 7, NB = TZ + 8;
   static constexpr int NT = 32 * WY * WZ;
-  static constexpr int kHeader = 64 + 2 * 32 * 4 + 3 * 32 * 16;  // mbar+desc | rowoff | rowinfo
+  static constexpr int kHeader = 128 + 2 * 32 * 4 + 3 * 32 * 16;  // mbar+desc | rowoff | rowinfo
   static constexpr int kTables = 3 * NROW * NB * 4;
   static_assert(NROW <= 32, "one lane per row in the round builder");
+  static_assert(2 * sizeof(RoundDesc) + 16 <= 128, "header");
 };
 
+__device__ __forceinline__ void red_add_v2(float* p, float a, float b) {
+  asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
+}
+
 // One thread's walk over its atoms of a round: rows [r, r_hi) of the plane table; per row the cells
-// s_z = z0-7 .. z0+1 are one contiguous run [a.x, b.y) of staged records; atoms of the first cell miss
-// column z0+1 (j < a.y) and atoms of the last cell miss column z0 (j >= b.x).
-// GLOBAL = false: records in shared memory (LDS); true: the round's single row read from global memory.
-template <int CB, bool GLOBAL>
+// s_z = z0-7 .. z0+1 are one contiguous run [a.x, b.y) of the row's atoms (clipped to the round's
+// [a0, a1)); atoms of the first cell miss column z0+1 (j < ja) and atoms of the last cell miss column
+// z0 (j >= jb).  The run of the NEXT row is fetched while the current one is processed, so that a row
+// change costs a few register moves instead of a dependent shared-memory round trip (in v3 the row
+// changes -- divergent, two LDS latencies deep -- took as long as the FMAs; profiles/r1c).
+template <int CB>
 __device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], int r, const int r_hi, const int* Lp, const int NB,
                                            const int* ro, const float* rbase, const int recf, const int cb0,
-                                           const int oy, const int oz, const int4 srow) {
+                                           const int oy, const int oz, const int a0, const int a1) {
   int j = 0, jend = 0, ja = 0, jb = 0;
+  int nj = 0, njend = 0, nja = 0, njb = 0;
+  bool pending = false;
+  auto fetch = [&](int rr) {
+    const int2 a = *reinterpret_cast<const int2*>(Lp + rr * NB);
+    const int2 b = *reinterpret_cast<const int2*>(Lp + rr * NB + SW);
+    const int off = ro[rr];      // staged position of the row's atom a0
+    nj = off + max(a.x, a0) - a0;
+    njend = off + min(b.y, a1) - a0;
+    nja = off + a.y - a0;
+    njb = off + b.x - a0;
+  };
+  if (r < r_hi) { fetch(r); ++r; pending = true; }
   for (;;) {
-    bool more = true;
-    while (j >= jend) {
-      if (r >= r_hi) { more = false; break; }
-      const int2 a = *reinterpret_cast<const int2*>(Lp + r * NB);
-      const int2 b = *reinterpret_cast<const int2*>(Lp + r * NB + SW);
-      const int off = GLOBAL ? 0 : ro[r];
-      j = off + a.x; ja = off + a.y; jb = off + b.x; jend = off + b.y;
-      ++r;
+    // row change (divergent, register moves only); the lanes reconverge before the atom body
+    while (j >= jend && pending) {
+      j = nj; jend = njend; ja = nja; jb = njb;
+      pending = r < r_hi;
+      if (pending) { fetch(r); ++r; }
     }
-    if (!more) break;
-    const float* rp;
-    if constexpr (GLOBAL) {
-      const int gj = j < srow.y ? srow.x + j : srow.z + (j - srow.y);
-      rp = rbase + (size_t)gj * recf;
-    } else {
-      rp = rbase + j * recf;
-    }
+    if (j >= jend) break;
+    const float* rp = rbase + j * recf;
     const float4 wa = *reinterpret_cast<const float4*>(rp);
     const float4 wb = *reinterpret_cast<const float4*>(rp + 4);
     float qv[CB];
@@ -236,17 +253,17 @@ __device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], int r, const
   }
 }
 
-template <int WY, int WZ, int CB>
-__global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 4 ? 3 : 2)))
-    k_spread_os(int Mx, int My, int Mz, int XS, int npy, int npz, int cap, int recf, int cb0,
+template <int WY, int WZ, int CB, int NCTA>
+__global__ void __launch_bounds__(32 * WY * WZ, NCTA)
+    k_spread_os(int Mx, int My, int Mz, int nseg, int npy, int npz, int cap, int recf, int cb0,
                 const int* __restrict__ start, const float* __restrict__ rec, float* __restrict__ grid) {
   using S = SpreadShape<WY, WZ>;
   constexpr int NROW = S::NROW, NB = S::NB, NT = S::NT;
   extern __shared__ __align__(128) unsigned char smem[];
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem);                 // [2]
   RoundDesc* s_desc = reinterpret_cast<RoundDesc*>(smem + 16);        // [2]
-  int* s_rowoff = reinterpret_cast<int*>(smem + 64);                  // [2][32]
-  int4* s_row = reinterpret_cast<int4*>(smem + 64 + 256);             // [3][32]  {gA0, nA, gB0, nB}
+  int* s_rowoff = reinterpret_cast<int*>(smem + 128);                 // [2][32]
+  int4* s_row = reinterpret_cast<int4*>(smem + 128 + 256);            // [3][32]  {gA0, nA, gB0, nB}
   int* s_L = reinterpret_cast<int*>(smem + S::kHeader);               // [3][NROW][NB]
   float* s_rec = reinterpret_cast<float*>(smem + S::kHeader + S::kTables);  // [2][cap * recf]
 
@@ -254,8 +271,10 @@ __global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 
   int bid = blockIdx.x;
   const int pz = bid % npz; bid /= npz;
   const int py = bid % npy; bid /= npy;
-  const int X0 = bid * XS, X1 = min(X0 + XS, Mx);
-  const int NP = X1 - X0 + (SW - 1);
+  // this CTA's cell planes: the atoms are PARTITIONED over the x segments (no halo is re-read); the
+  // 7 output planes a segment shares with each neighbour are merged in global memory by RED
+  const int X0 = (int)((long long)bid * Mx / nseg), X1 = (int)((long long)(bid + 1) * Mx / nseg);
+  const int NP = X1 - X0;
   const int Y0 = py * S::TY, Z0 = pz * S::TZ;
   // cells of a row: sz_u = Z0-7 .. Z0+TZ-1; those below 0 wrap to the end of the row (run A)
   const int nAc = Z0 < SW - 1 ? SW - 1 - Z0 : 0;
@@ -275,8 +294,7 @@ __global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 
 
   auto build_plane = [&](int pl) {
     const int tb = pl % 3;
-    const int sxu = X0 - (SW - 1) + pl;
-    const int sx = sxu < 0 ? sxu + Mx : sxu;
+    const int sx = X0 + pl;
     for (int t = tid; t < NROW * NB; t += NT) {
       const int r = t / NB, b = t - r * NB;
       const int syu = Y0 - (SW - 1) + r;
@@ -301,35 +319,54 @@ __global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 
     }
   };
 
-  // round builder (warp 0): rows [rn0, r1n) of plane pn whose atoms fit the staging buffer
-  auto build_round = [&](int pn, int rn0, int nb) {
+  // round builder (warp 0): the next round starts at (plane pn, row rn0, atom an0 of that row)
+  auto build_round = [&](int pn, int rn0, int an0, int nb) {
     RoundDesc nd;
-    nd.p = pn; nd.r0 = rn0; nd.r1 = NROW; nd.total = 0; nd.slow = 0;
+    nd.p = pn; nd.r0 = rn0; nd.r1 = NROW; nd.a0 = 0; nd.a1 = INT_MAX; nd.total = 0; nd.flush = 1;
+    nd.np = pn + 1; nd.nr = 0; nd.na = 0;
     if (pn < NP) {
       const int tb = pn % 3;
       const bool mine = lane >= rn0 && lane < NROW;
-      const int tot = mine ? s_L[(tb * NROW + lane) * NB + NB - 1] : 0;
+      int tot = mine ? s_L[(tb * NROW + lane) * NB + NB - 1] : 0;
+      if (lane == rn0) tot -= an0;
       int cum = tot;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
         const int t = __shfl_up_sync(0xffffffffu, cum, o);
         if (lane >= o) cum += t;
       }
-      int nr = __popc(__ballot_sync(0xffffffffu, mine && cum <= cap));
-      if (nr == 0) { nr = 1; nd.slow = 1; }
-      nd.r1 = rn0 + nr;
-      nd.total = __shfl_sync(0xffffffffu, cum, nd.r1 - 1);
+      const int nfit = __popc(__ballot_sync(0xffffffffu, mine && cum <= cap));
+      const int t0 = __shfl_sync(0xffffffffu, tot, rn0);
+      const bool single = an0 > 0 || nfit == 0;
+      int so, cnt;   // this lane's row: staged position of its first atom, atoms staged
+      if (single) {  // (the rest of) one row, at most a buffer full
+        const int take = min(cap, t0);
+        nd.r1 = rn0 + 1; nd.a0 = an0; nd.a1 = an0 + take; nd.total = take;
+        if (t0 > take) { nd.flush = 0; nd.np = pn; nd.nr = rn0; nd.na = an0 + take; }
+        else if (rn0 + 1 < NROW) { nd.flush = 0; nd.np = pn; nd.nr = rn0 + 1; }
+        so = 0; cnt = take;
+      } else {       // whole rows
+        nd.r1 = rn0 + nfit;
+        nd.total = __shfl_sync(0xffffffffu, cum, nd.r1 - 1);
+        if (nd.r1 < NROW) { nd.flush = 0; nd.np = pn; nd.nr = nd.r1; }
+        so = cum - tot; cnt = tot;
+      }
       const bool in_round = lane >= rn0 && lane < nd.r1;
-      if (in_round) s_rowoff[nb * 32 + lane] = cum - tot;
-      if (!nd.slow && nd.total > 0) {
+      if (in_round) s_rowoff[nb * 32 + lane] = so;
+      if (nd.total > 0) {
         if (lane == 0) mbar_arrive_expect_tx(&mbar[nb], (uint32_t)nd.total * recf * 4u);
         __syncwarp();
-        if (in_round && tot > 0) {
-          const int4 ri = s_row[tb * 32 + lane];
-          float* dst = s_rec + (size_t)nb * cap * recf + (size_t)(cum - tot) * recf;
-          if (ri.y > 0) bulk_g2s(dst, rec + (size_t)ri.x * recf, (uint32_t)ri.y * recf * 4u, &mbar[nb]);
-          if (ri.w > 0)
-            bulk_g2s(dst + (size_t)ri.y * recf, rec + (size_t)ri.z * recf, (uint32_t)ri.w * recf * 4u, &mbar[nb]);
+        if (in_round && cnt > 0) {
+          const int4 ri = s_row[tb * 32 + lane];   // the row = run A (ri.y atoms at ri.x) then run B
+          const int lo = nd.a0, hi = nd.a0 + cnt;
+          const int a_lo = min(lo, ri.y), a_hi = min(hi, ri.y);
+          const int b_lo = max(lo, ri.y) - ri.y, b_hi = max(hi, ri.y) - ri.y;
+          float* dst = s_rec + (size_t)nb * cap * recf + (size_t)so * recf;
+          if (a_hi > a_lo)
+            bulk_g2s(dst, rec + (size_t)(ri.x + a_lo) * recf, (uint32_t)(a_hi - a_lo) * recf * 4u, &mbar[nb]);
+          if (b_hi > b_lo)
+            bulk_g2s(dst + (size_t)(a_hi - a_lo) * recf, rec + (size_t)(ri.z + b_lo) * recf,
+                     (uint32_t)(b_hi - b_lo) * recf * 4u, &mbar[nb]);
         }
       }
     }
@@ -344,7 +381,7 @@ __global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 
   build_plane(0);
   if (NP > 1) build_plane(1);
   __syncthreads();
-  if (warp == 0) build_round(0, 0, 0);
+  if (warp == 0) build_round(0, 0, 0, 0);
 
   float acc[SW][2][CB];
 #pragma unroll
@@ -360,12 +397,9 @@ __global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 
     const int cur = it & 1;
     const RoundDesc d = s_desc[cur];
     if (d.p >= NP) break;
-    if (warp == 0) {
-      const bool last = d.r1 >= NROW;
-      build_round(last ? d.p + 1 : d.p, last ? 0 : d.r1, cur ^ 1);
-    }
-    if (d.r0 == 0 && d.p + 2 < NP) build_plane(d.p + 2);
-    if (!d.slow && d.total > 0) {
+    if (warp == 0) build_round(d.np, d.nr, d.na, cur ^ 1);
+    if (d.r0 == 0 && d.a0 == 0 && d.p + 2 < NP) build_plane(d.p + 2);
+    if (d.total > 0) {
       if (cur == 0) { mbar_wait(&mbar[0], phase0); phase0 ^= 1; }
       else          { mbar_wait(&mbar[1], phase1); phase1 ^= 1; }
     }
@@ -374,49 +408,75 @@ __global__ void __launch_bounds__(32 * WY * WZ, (WY * WZ <= 2 ? 6 : (WY * WZ <= 
       const int tb = d.p % 3;
       const int r_beg = max(rlo, d.r0);
       const int r_hi = lane_ok ? min(rlo + SW, d.r1) : r_beg;
-      const int* Lp = s_L + (size_t)tb * NROW * NB + clo;
-      if (!d.slow)
-        walk_atoms<CB, false>(acc, r_beg, r_hi, Lp, NB, s_rowoff + cur * 32, s_rec + (size_t)cur * cap * recf, recf,
-                              cb0, oy, oz, make_int4(0, 0, 0, 0));
-      else   // a single row larger than the staging buffer: records straight from global memory
-        walk_atoms<CB, true>(acc, r_beg, r_hi, Lp, NB, nullptr, rec, recf, cb0, oy, oz, s_row[tb * 32 + d.r0]);
+      walk_atoms<CB>(acc, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32,
+                     s_rec + (size_t)cur * cap * recf, recf, cb0, oy, oz, d.a0, d.a1);
     }
-    // ---- plane complete: store its slot once, clear it ----
-    if (d.r1 >= NROW) {
-      const int sxu = X0 - (SW - 1) + d.p;
-      const bool st = lane_ok && sxu >= X0;
-      float* gp = grid + (size_t)cb0 * Mtot + ((size_t)max(sxu, 0) * My + y) * Mz + z0;
-      switch (sxu & 7) {
-#define PSWF_FLUSH(K)                                                                                   \
-  case K:                                                                                               \
-    _Pragma("unroll") for (int c = 0; c < CB; ++c) {                                                    \
-      if (st) *reinterpret_cast<float2*>(gp + (size_t)c * Mtot) = make_float2(acc[K][0][c], acc[K][1][c]); \
-      acc[K][0][c] = 0.f;                                                                               \
-      acc[K][1][c] = 0.f;                                                                               \
-    }                                                                                                   \
+    // ---- plane complete: its slot leaves the window; after the last cell plane so do the 7 planes
+    //      beyond it.  Planes shared with a neighbouring segment are added (RED), the others stored.
+    if (d.flush && lane_ok) {
+      const int nfl = d.p == NP - 1 ? SW : 1;
+      for (int i = 0; i < nfl; ++i) {
+        const int pl = d.p + i;
+        int P = X0 + pl; if (P >= Mx) P -= Mx;
+        const bool shared = pl < SW - 1 || pl >= NP;
+        float* gp = grid + (size_t)cb0 * Mtot + ((size_t)P * My + y) * Mz + z0;
+        switch (P & 7) {
+#define PSWF_FLUSH(K)                                                                          \
+  case K:                                                                                      \
+    _Pragma("unroll") for (int c = 0; c < CB; ++c) {                                           \
+      if (shared) red_add_v2(gp + (size_t)c * Mtot, acc[K][0][c], acc[K][1][c]);               \
+      else *reinterpret_cast<float2*>(gp + (size_t)c * Mtot) = make_float2(acc[K][0][c], acc[K][1][c]); \
+      acc[K][0][c] = 0.f;                                                                      \
+      acc[K][1][c] = 0.f;                                                                      \
+    }                                                                                          \
     break;
-        PSWF_FLUSH(0) PSWF_FLUSH(1) PSWF_FLUSH(2) PSWF_FLUSH(3)
-        PSWF_FLUSH(4) PSWF_FLUSH(5) PSWF_FLUSH(6) PSWF_FLUSH(7)
+          PSWF_FLUSH(0) PSWF_FLUSH(1) PSWF_FLUSH(2) PSWF_FLUSH(3)
+          PSWF_FLUSH(4) PSWF_FLUSH(5) PSWF_FLUSH(6) PSWF_FLUSH(7)
 #undef PSWF_FLUSH
+        }
       }
     }
   }
 }
 
-template <int WY, int WZ>
+template <int WY, int WZ, int NCTA>
 struct SpreadLaunch {
   using S = SpreadShape<WY, WZ>;
   static size_t smem_bytes(int cap, int recf) { return S::kHeader + S::kTables + 2 * (size_t)cap * recf * 4; }
 
   template <int CB>
-  static void run(pswf_lr_plan* p, int XS, int cap, int recf, int cb0, cudaStream_t st) {
+  static void run(pswf_lr_plan* p, int nseg, int cap, int recf, int cb0, cudaStream_t st) {
     const int Mx = p->M[0], My = p->M[1], Mz = p->M[2];
-    const int npy = (My + S::TY - 1) / S::TY, npz = (Mz + S::TZ - 1) / S::TZ, nseg = (Mx + XS - 1) / XS;
+    const int npy = (My + S::TY - 1) / S::TY, npz = (Mz + S::TZ - 1) / S::TZ;
     const size_t sm = smem_bytes(cap, recf);
-    auto kern = k_spread_os<WY, WZ, CB>;
+    auto kern = k_spread_os<WY, WZ, CB, NCTA>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    kern<<<(unsigned)(npy * npz * nseg), S::NT, sm, st>>>(Mx, My, Mz, XS, npy, npz, cap, recf, cb0, p->d_count,
+    kern<<<(unsigned)(npy * npz * nseg), S::NT, sm, st>>>(Mx, My, Mz, nseg, npy, npz, cap, recf, cb0, p->d_count,
                                                          (const float*)p->d_rec, (float*)p->d_grid);
+  }
+
+  static void all_channels(pswf_lr_plan* p, cudaStream_t st) {
+    const int recf = stencil_rec_floats(p->C);
+    // staging capacity: NCTA CTAs per SM
+    const size_t budget = (size_t)(227 * 1024) / NCTA - 1024;
+    int cap = (int)((budget - S::kHeader - S::kTables) / (2 * (size_t)recf * 4));
+    cap &= ~7;
+    // x segments: ONE wave of CTAs.  The atoms are partitioned over the segments, so short segments
+    // cost no extra arithmetic, only RED traffic for the 7 shared planes; a second, partly filled
+    // wave would cost a full segment time (512 CTAs on 444 slots; profiles/r1b).
+    const int npatch = ((p->M[1] + S::TY - 1) / S::TY) * ((p->M[2] + S::TZ - 1) / S::TZ);
+    int nseg = NCTA * p->sm_count / npatch;
+    nseg = std::max(1, std::min(nseg, p->M[0] / SW));
+    const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
+    cudaMemsetAsync(p->d_grid, 0, sizeof(float) * Mtot * p->C, st);   // the RED-merged planes start from zero
+    int cb0 = 0;
+    while (cb0 < p->C) {
+      const int left = p->C - cb0;
+      if (left >= 4) { run<4>(p, nseg, cap, recf, cb0, st); cb0 += 4; }
+      else if (left == 3) { run<3>(p, nseg, cap, recf, cb0, st); cb0 += 3; }
+      else if (left == 2) { run<2>(p, nseg, cap, recf, cb0, st); cb0 += 2; }
+      else { run<1>(p, nseg, cap, recf, cb0, st); cb0 += 1; }
+    }
   }
 };
 
@@ -458,30 +518,7 @@ void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const floa
 
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {
   (void)n;
-  using L = SpreadLaunch<2, 2>;
-  const int recf = stencil_rec_floats(p->C);
-  // staging capacity: three CTAs per SM
-  const size_t budget = 74 * 1024;
-  int cap = (int)((budget - L::S::kHeader - L::S::kTables) / (2 * (size_t)recf * 4));
-  cap &= ~7;
-  // x segments: ONE wave of CTAs (3 resident per SM).  Every segment re-reads 7 halo planes, so the
-  // segments are as long as a single wave allows; a second, partly filled wave costs a full segment
-  // time (512 CTAs on 444 slots ran 2 x 23 planes instead of 1 x 29; profiles/r1b).
-  const int Mx = p->M[0];
-  const int npatch = ((p->M[1] + L::S::TY - 1) / L::S::TY) * ((p->M[2] + L::S::TZ - 1) / L::S::TZ);
-  const int slots = 3 * p->sm_count;
-  int nseg = slots / npatch;
-  if (nseg < 1) nseg = 1;
-  int XS = (Mx + nseg - 1) / nseg;
-  if (XS < 8) XS = 8;
-  int cb0 = 0;
-  while (cb0 < p->C) {
-    const int left = p->C - cb0;
-    if (left >= 4) { L::run<4>(p, XS, cap, recf, cb0, st); cb0 += 4; }
-    else if (left == 3) { L::run<3>(p, XS, cap, recf, cb0, st); cb0 += 3; }
-    else if (left == 2) { L::run<2>(p, XS, cap, recf, cb0, st); cb0 += 2; }
-    else { L::run<1>(p, XS, cap, recf, cb0, st); cb0 += 1; }
-  }
+  SpreadLaunch<2, 2, 3>::all_channels(p, st);
 }
 
 }  // namespace pswf

@@ -230,6 +230,29 @@ def test_window_widths_and_ragged_grids_fp32(w, grid):
     check_vs(b, ref, 5e-6, 2e-5, label="w=%d ref vs B" % w)
 
 
+def test_dense_cells_exceed_staging_buffers_fp32():
+    """Degenerate density: 1500 atoms inside two grid cells (plus a sparse background), so that one
+    cell row holds far more atoms than the spread kernel's shared-memory staging buffer (sub-row
+    rounds) and than the gather kernel's 32-atom record stage (re-staging inside a cell).  Fast path
+    vs reference path vs oracle B."""
+    rng = np.random.default_rng(77)
+    box, grid, w = [16.0] * 3, [32, 32, 32], 8
+    h = 0.5
+    clump1 = np.array([3.1, 7.3, 15.8]) + rng.uniform(0, 1, (1000, 3)) * h
+    clump2 = np.array([15.7, 0.1, 0.2]) + rng.uniform(0, 1, (500, 3)) * h      # wraps in x
+    pos = np.concatenate([clump1, clump2, rng.uniform(0, 16, (300, 3))])
+    pos = np.mod(pos, 16.0).astype(np.float32).astype(np.float64)
+    N = len(pos)
+    q = rng.normal(0, 0.5, (4, N)).astype(np.float32).astype(np.float64)
+    wl = dict(pos=pos, q=q, exponents=[1, 1, 3, 6], box=box, grid=grid, w=w, c=12.024, precision="f32")
+    a = run_gpu(wl, kernel_path=0)
+    b = run_gpu(wl, kernel_path=1)
+    i = a["info"]
+    ref = G.gridded(pos, q, wl["exponents"], box, grid, w, wl["c"], i["r_c"], i["c_window"])
+    check_vs(a, ref, 5e-6, 2e-5, label="dense fast vs B")
+    check_vs(b, ref, 5e-6, 2e-5, label="dense ref vs B")
+
+
 @pytest.mark.parametrize("C", [1, 2, 3, 5, 8, 11])
 def test_channel_counts_fp32(C):
     rng = np.random.default_rng(C)
