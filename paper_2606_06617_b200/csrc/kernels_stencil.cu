@@ -182,6 +182,7 @@ struct SpreadShape {
   static constexpr int NT = 32 * WY * WZ;
   static constexpr int kHeader = 128 + 2 * 32 * 4 + 3 * 32 * 16;  // mbar+desc | rowoff | rowinfo
   static constexpr int kTables = 3 * NROW * NB * 4;
+  static constexpr int kRuns = SW * NT * 8;   // per thread: 8 packed run descriptors of the current round
   static_assert(NROW <= 32, "one lane per row in the round builder");
   static_assert(2 * sizeof(RoundDesc) + 16 <= 128, "header");
 };
@@ -190,35 +191,49 @@ __device__ __forceinline__ void red_add_v2(float* p, float a, float b) {
   asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
 }
 
-// One thread's walk over its atoms of a round: rows [r, r_hi) of the plane table; per row the cells
-// s_z = z0-7 .. z0+1 are one contiguous run [a.x, b.y) of the row's atoms (clipped to the round's
-// [a0, a1)); atoms of the first cell miss column z0+1 (j < ja) and atoms of the last cell miss column
-// z0 (j >= jb).  The run of the NEXT row is fetched while the current one is processed, so that a row
-// change costs a few register moves instead of a dependent shared-memory round trip (in v3 the row
-// changes -- divergent, two LDS latencies deep -- took as long as the FMAs; profiles/r1c).
+// One thread's atoms of a round are (at most) 8 runs of staged records, one per cell row s_y = y-7 .. y:
+// the cells s_z = z0-7 .. z0+1 of the row, clipped to the round's atom range [a0, a1).  Atoms of the
+// first cell miss column z0+1 (j < ja) and atoms of the last cell miss column z0 (j >= jb).
+// The runs are computed once per round in a uniform, fully unrolled pass (all lanes busy, shared-
+// memory latencies overlapped) and left in shared memory as packed descriptors {j | jend << 16,
+// ja | jb << 16} in staged-record units.  (In v3 every lane derived its next run inside the atom
+// loop: a divergent, two-LDS-deep row change on nearly every warp iteration, as costly as the FMAs;
+// profiles/r1c.)
+__device__ __forceinline__ void build_runs(uint2* runs, const int NT, const int r_beg, const int r_hi, const int* Lp,
+                                           const int NB, const int* ro, const int a0, const int a1) {
+#pragma unroll
+  for (int i = 0; i < SW; ++i) {
+    const int rr = r_beg + i;
+    if (rr < r_hi) {
+      const int2 a = *reinterpret_cast<const int2*>(Lp + rr * NB);
+      const int2 b = *reinterpret_cast<const int2*>(Lp + rr * NB + SW);
+      const int off = ro[rr] - a0;      // staged position of the row's atom 0
+      const int j = off + max(a.x, a0);
+      const int jend = max(j, off + min(b.y, a1));
+      const int ja = min(max(off + a.y, 0), 0xffff);
+      const int jb = min(max(off + b.x, 0), 0xffff);
+      runs[i * NT] = make_uint2((unsigned)j | ((unsigned)jend << 16), (unsigned)ja | ((unsigned)jb << 16));
+    }
+  }
+}
+
 template <int CB>
-__device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], int r, const int r_hi, const int* Lp, const int NB,
-                                           const int* ro, const float* rbase, const int recf, const int cb0,
-                                           const int oy, const int oz, const int a0, const int a1) {
+__device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], const uint2* runs, const int NT, const int nrows,
+                                           const float* rbase, const int recf, const int cb0, const int oy,
+                                           const int oz) {
   int j = 0, jend = 0, ja = 0, jb = 0;
-  int nj = 0, njend = 0, nja = 0, njb = 0;
-  bool pending = false;
-  auto fetch = [&](int rr) {
-    const int2 a = *reinterpret_cast<const int2*>(Lp + rr * NB);
-    const int2 b = *reinterpret_cast<const int2*>(Lp + rr * NB + SW);
-    const int off = ro[rr];      // staged position of the row's atom a0
-    nj = off + max(a.x, a0) - a0;
-    njend = off + min(b.y, a1) - a0;
-    nja = off + a.y - a0;
-    njb = off + b.x - a0;
-  };
-  if (r < r_hi) { fetch(r); ++r; pending = true; }
+  int k = 0;                     // descriptors fetched so far
+  uint2 nd = make_uint2(0u, 0u);
+  if (nrows > 0) { nd = runs[0]; k = 1; }
+  bool pending = nrows > 0;
   for (;;) {
-    // row change (divergent, register moves only); the lanes reconverge before the atom body
+    // row change (divergent, but register-only: the next descriptor was fetched a run ago); the lanes
+    // reconverge before the atom body
     while (j >= jend && pending) {
-      j = nj; jend = njend; ja = nja; jb = njb;
-      pending = r < r_hi;
-      if (pending) { fetch(r); ++r; }
+      j = (int)(nd.x & 0xffffu); jend = (int)(nd.x >> 16);
+      ja = (int)(nd.y & 0xffffu); jb = (int)(nd.y >> 16);
+      pending = k < nrows;
+      if (pending) { nd = runs[k * NT]; ++k; }
     }
     if (j >= jend) break;
     const float* rp = rbase + j * recf;
@@ -244,9 +259,9 @@ __device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], int r, const
     for (int c = 0; c < CB; ++c) {
       const float v0 = p0 * qv[c], v1 = p1 * qv[c];
 #pragma unroll
-      for (int k = 0; k < SW; ++k) {
-        acc[k][0][c] = fmaf(wx[k], v0, acc[k][0][c]);
-        acc[k][1][c] = fmaf(wx[k], v1, acc[k][1][c]);
+      for (int k2 = 0; k2 < SW; ++k2) {
+        acc[k2][0][c] = fmaf(wx[k2], v0, acc[k2][0][c]);
+        acc[k2][1][c] = fmaf(wx[k2], v1, acc[k2][1][c]);
       }
     }
     ++j;
@@ -265,7 +280,8 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
   int* s_rowoff = reinterpret_cast<int*>(smem + 128);                 // [2][32]
   int4* s_row = reinterpret_cast<int4*>(smem + 128 + 256);            // [3][32]  {gA0, nA, gB0, nB}
   int* s_L = reinterpret_cast<int*>(smem + S::kHeader);               // [3][NROW][NB]
-  float* s_rec = reinterpret_cast<float*>(smem + S::kHeader + S::kTables);  // [2][cap * recf]
+  uint2* s_run = reinterpret_cast<uint2*>(smem + S::kHeader + S::kTables) + threadIdx.x;   // [8][NT], this thread's
+  float* s_rec = reinterpret_cast<float*>(smem + S::kHeader + S::kTables + S::kRuns);     // [2][cap * recf]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   int bid = blockIdx.x;
@@ -408,8 +424,8 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
       const int tb = d.p % 3;
       const int r_beg = max(rlo, d.r0);
       const int r_hi = lane_ok ? min(rlo + SW, d.r1) : r_beg;
-      walk_atoms<CB>(acc, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32,
-                     s_rec + (size_t)cur * cap * recf, recf, cb0, oy, oz, d.a0, d.a1);
+      build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32, d.a0, d.a1);
+      walk_atoms<CB>(acc, s_run, NT, r_hi - r_beg, s_rec + (size_t)cur * cap * recf, recf, cb0, oy, oz);
     }
     // ---- plane complete: its slot leaves the window; after the last cell plane so do the 7 planes
     //      beyond it.  Planes shared with a neighbouring segment are added (RED), the others stored.
@@ -442,7 +458,7 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
 template <int WY, int WZ, int NCTA>
 struct SpreadLaunch {
   using S = SpreadShape<WY, WZ>;
-  static size_t smem_bytes(int cap, int recf) { return S::kHeader + S::kTables + 2 * (size_t)cap * recf * 4; }
+  static size_t smem_bytes(int cap, int recf) { return S::kHeader + S::kTables + S::kRuns + 2 * (size_t)cap * recf * 4; }
 
   template <int CB>
   static void run(pswf_lr_plan* p, int nseg, int cap, int recf, int cb0, cudaStream_t st) {
@@ -459,7 +475,7 @@ struct SpreadLaunch {
     const int recf = stencil_rec_floats(p->C);
     // staging capacity: NCTA CTAs per SM
     const size_t budget = (size_t)(227 * 1024) / NCTA - 1024;
-    int cap = (int)((budget - S::kHeader - S::kTables) / (2 * (size_t)recf * 4));
+    int cap = (int)((budget - S::kHeader - S::kTables - S::kRuns) / (2 * (size_t)recf * 4));
     cap &= ~7;
     // x segments: ONE wave of CTAs.  The atoms are partitioned over the segments, so short segments
     // cost no extra arithmetic, only RED traffic for the 7 shared planes; a second, partly filled
