@@ -114,6 +114,15 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
 
 
+def profiled_traffic(kernel):
+    """DRAM bytes per launch of a kernel from the committed ncu --set full capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "r1c_traffic.json")
+    try:
+        return int(json.load(open(path))["dram_bytes_per_launch"][kernel])
+    except Exception:
+        return None
+
+
 def algorithmic_bytes(N, C, M, B=4):
     """SURVEY.md §8(d) / DESIGN.md §6: bytes each stage must move per evaluation."""
     Mtot = M[0] * M[1] * M[2]
@@ -288,7 +297,10 @@ def run_ours(args):
     alu_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12          # fp32 FMA peak at max clock, TFLOP/s
     ach = flops_alg[dom] / (stage_ms[dom] * 1e-3) / 1e12
     roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
-                "frac": ach / alu_peak, "traffic": None,
+                "frac": ach / alu_peak,
+                "traffic": profiled_traffic(dom) if (args.cfg == 4 and args.atoms is None and args.kernel_path == 0) else None,
+                "traffic_source": "profiles/r1c_ncu_full.md (dram__bytes_read+write of one launch, config 4)",
+                "alg_flops": flops_alg[dom], "alg_bytes": bytes_alg[dom],
                 "peak_source": "148 SM x 128 FMA/clk x 2 x %.0f MHz (DESIGN.md §6)" % sm_max,
                 "hbm_achieved_gbs": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9,
                 "hbm_frac": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9 / peak_gbs}
@@ -304,7 +316,11 @@ def run_ours(args):
     if not args.no_cpu_baseline:
         cb = cpu_baseline(wl, info["r_c"])
 
-    launches_per_step = {"ref": 9, "fast": 10}["fast" if args.kernel_path == 0 else "ref"]
+    # this library's own kernels per evaluation (cuFFT's 6 kernels and 3 memsets not counted):
+    # fast: bin_count, 3 scan kernels, perm, records, spread, scale, finalize, interleave, gather (C <= 4)
+    # ref:  bin_count, 3 scan kernels, scatter, spread_ref, scale, finalize, gather_ref
+    groups = (C + 3) // 4
+    launches_per_step = {"ref": 9, "fast": 8 + 3 * groups}["fast" if args.kernel_path == 0 else "ref"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
