@@ -2,7 +2,8 @@
 // spread with global atomics, the fused scale+reduce kernel over the half spectrum, and a
 // warp-per-atom gather.  They run every configuration in both precisions (any even w <= 16,
 // any channel count); the fp64 path and kernel_path = 1 always use them.  The tiled fp32
-// kernels in kernels_fast.cu replace spread and gather on the default path.
+// kernels in kernels_stencil.cu / kernels_gather.cu replace sort-scatter, spread and gather on the
+// default path.
 #include "kernels_common.cuh"
 #include "launch.hpp"
 
