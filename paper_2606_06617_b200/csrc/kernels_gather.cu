@@ -205,6 +205,10 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   const unsigned plane = (unsigned)Mx * My, wrap = plane * (unsigned)Mz;
   const V* g0 = gridt + (size_t)ix0 * My + iy;
   const V* g1 = gridt + (size_t)ix1 * My + iy;
+  // keep the two lane pointers in registers: left to itself ptxas re-derives them from the kernel
+  // parameter with a uniform constant load in front of every refill load (70% of the refill's stall
+  // samples in profiles/r1c)
+  asm volatile("" : "+l"(g0), "+l"(g1));
   // record offsets of this lane's (x,y) weights (records are rotated by the cell index mod 8)
   const int ox0 = (sx + b0) & 7, ox1 = ox0 ^ 4, oy = SW + ((sy + c_off) & 7);
 

@@ -222,6 +222,10 @@ template <int CB>
 __device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], const uint2* runs, const int NT, const int nrows,
                                            const float* rbase, const int recf, const int cb0, const int oy,
                                            const int oz) {
+  // loop invariants pinned to registers (ptxas otherwise reloads the kernel parameters from the
+  // constant bank inside the atom loop, a uniform-load latency per iteration)
+  int recf_r = recf, cb0_r = cb0;
+  asm volatile("" : "+r"(recf_r), "+r"(cb0_r));
   int j = 0, jend = 0, ja = 0, jb = 0;
   int k = 0;                     // descriptors fetched so far
   uint2 nd = make_uint2(0u, 0u);
@@ -237,19 +241,19 @@ __device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], const uint2*
       if (pending) { nd = runs[k * NT]; ++k; }
     }
     if (j >= jend) break;
-    const float* rp = rbase + j * recf;
+    const float* rp = rbase + j * recf_r;
     const float4 wa = *reinterpret_cast<const float4*>(rp);
     const float4 wb = *reinterpret_cast<const float4*>(rp + 4);
     float qv[CB];
     if constexpr (CB >= 3) {
-      const float4 t = *reinterpret_cast<const float4*>(rp + 3 * SW + cb0);
+      const float4 t = *reinterpret_cast<const float4*>(rp + 3 * SW + cb0_r);
       qv[0] = t.x; qv[1] = t.y; qv[2] = t.z;
       if constexpr (CB == 4) qv[3] = t.w;
     } else if constexpr (CB == 2) {
-      const float2 t = *reinterpret_cast<const float2*>(rp + 3 * SW + cb0);
+      const float2 t = *reinterpret_cast<const float2*>(rp + 3 * SW + cb0_r);
       qv[0] = t.x; qv[1] = t.y;
     } else {
-      qv[0] = rp[3 * SW + cb0];
+      qv[0] = rp[3 * SW + cb0_r];
     }
     const float wyv = rp[oy];
     const float2 wzv = *reinterpret_cast<const float2*>(rp + oz);
