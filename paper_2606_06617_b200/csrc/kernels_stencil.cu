@@ -45,6 +45,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   asm volatile(
       "{\n"
@@ -185,7 +188,7 @@ struct SpreadShape {
   static constexpr int kTables = 3 * NROW * NB * 4;
   static constexpr int kRuns = SW * NT * 8;   // per thread: 8 packed run descriptors of the current round
   static_assert(NROW <= 32, "one lane per row in the round builder");
-  static_assert(2 * sizeof(RoundDesc) + 16 <= 128, "header");
+  static_assert(2 * sizeof(RoundDesc) + 32 <= 128, "header");
 };
 
 __device__ __forceinline__ void red_add_v2(float* p, float a, float b) {
@@ -274,14 +277,15 @@ __device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], const uint2*
 }
 
 template <int WY, int WZ, int CB, int NCTA>
-__global__ void __launch_bounds__(32 * WY * WZ, NCTA)
+__global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer warps + one producer warp
     k_spread_os(int Mx, int My, int Mz, int nseg, int npy, int npz, int cap, int recf, int cb0,
                 const int* __restrict__ start, const float* __restrict__ rec, float* __restrict__ grid) {
   using S = SpreadShape<WY, WZ>;
   constexpr int NROW = S::NROW, NB = S::NB, NT = S::NT;
   extern __shared__ __align__(128) unsigned char smem[];
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem);                 // [2]
-  RoundDesc* s_desc = reinterpret_cast<RoundDesc*>(smem + 16);        // [2]
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);                 // [2] records of a round have landed
+  uint64_t* empty = full + 2;                                         // [2] all consumer warps are done with them
+  RoundDesc* s_desc = reinterpret_cast<RoundDesc*>(smem + 32);        // [2]
   int* s_rowoff = reinterpret_cast<int*>(smem + 128);                 // [2][32]
   int4* s_row = reinterpret_cast<int4*>(smem + 128 + 256);            // [3][32]  {gA0, nA, gB0, nB}
   int* s_L = reinterpret_cast<int*>(smem + S::kHeader);               // [3][NROW][NB]
@@ -316,7 +320,7 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
   auto build_plane = [&](int pl) {
     const int tb = pl % 3;
     const int sx = X0 + pl;
-    for (int t = tid; t < NROW * NB; t += NT) {
+    for (int t = lane; t < NROW * NB; t += 32) {
       const int r = t / NB, b = t - r * NB;
       const int syu = Y0 - (SW - 1) + r;
       int val = 0;
@@ -341,7 +345,7 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
   };
 
   // round builder (warp 0): the next round starts at (plane pn, row rn0, atom an0 of that row)
-  auto build_round = [&](int pn, int rn0, int an0, int nb) {
+  auto build_round = [&](int pn, int rn0, int an0, int nb) -> RoundDesc {
     RoundDesc nd;
     nd.p = pn; nd.r0 = rn0; nd.r1 = NROW; nd.a0 = 0; nd.a1 = INT_MAX; nd.total = 0; nd.flush = 1;
     nd.np = pn + 1; nd.nr = 0; nd.na = 0;
@@ -374,35 +378,59 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
       }
       const bool in_round = lane >= rn0 && lane < nd.r1;
       if (in_round) s_rowoff[nb * 32 + lane] = so;
-      if (nd.total > 0) {
-        if (lane == 0) mbar_arrive_expect_tx(&mbar[nb], (uint32_t)nd.total * recf * 4u);
-        __syncwarp();
-        if (in_round && cnt > 0) {
-          const int4 ri = s_row[tb * 32 + lane];   // the row = run A (ri.y atoms at ri.x) then run B
-          const int lo = nd.a0, hi = nd.a0 + cnt;
-          const int a_lo = min(lo, ri.y), a_hi = min(hi, ri.y);
-          const int b_lo = max(lo, ri.y) - ri.y, b_hi = max(hi, ri.y) - ri.y;
-          float* dst = s_rec + (size_t)nb * cap * recf + (size_t)so * recf;
-          if (a_hi > a_lo)
-            bulk_g2s(dst, rec + (size_t)(ri.x + a_lo) * recf, (uint32_t)(a_hi - a_lo) * recf * 4u, &mbar[nb]);
-          if (b_hi > b_lo)
-            bulk_g2s(dst + (size_t)(a_hi - a_lo) * recf, rec + (size_t)(ri.z + b_lo) * recf,
-                     (uint32_t)(b_hi - b_lo) * recf * 4u, &mbar[nb]);
-        }
+      if (lane == 0) s_desc[nb] = nd;
+      __syncwarp();   // descriptor and row offsets are written before the barrier can complete
+      if (lane == 0) {
+        if (nd.total > 0) mbar_arrive_expect_tx(&full[nb], (uint32_t)nd.total * recf * 4u);
+        else mbar_arrive(&full[nb]);
       }
+      __syncwarp();
+      if (in_round && cnt > 0) {
+        const int4 ri = s_row[tb * 32 + lane];   // the row = run A (ri.y atoms at ri.x) then run B
+        const int lo = nd.a0, hi = nd.a0 + cnt;
+        const int a_lo = min(lo, ri.y), a_hi = min(hi, ri.y);
+        const int b_lo = max(lo, ri.y) - ri.y, b_hi = max(hi, ri.y) - ri.y;
+        float* dst = s_rec + (size_t)nb * cap * recf + (size_t)so * recf;
+        if (a_hi > a_lo)
+          bulk_g2s(dst, rec + (size_t)(ri.x + a_lo) * recf, (uint32_t)(a_hi - a_lo) * recf * 4u, &full[nb]);
+        if (b_hi > b_lo)
+          bulk_g2s(dst + (size_t)(a_hi - a_lo) * recf, rec + (size_t)(ri.z + b_lo) * recf,
+                   (uint32_t)(b_hi - b_lo) * recf * 4u, &full[nb]);
+      }
+    } else {          // past the last plane: the terminal descriptor
+      if (lane == 0) s_desc[nb] = nd;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&full[nb]);
     }
-    if (lane == 0) s_desc[nb] = nd;
+    return nd;
   };
 
   if (tid == 0) {
-    mbar_init(&mbar[0], 1);
-    mbar_init(&mbar[1], 1);
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    mbar_init(&empty[0], WY * WZ);
+    mbar_init(&empty[1], WY * WZ);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  build_plane(0);
-  if (NP > 1) build_plane(1);
   __syncthreads();
-  if (warp == 0) build_round(0, 0, 0, 0);
+
+  if (warp == WY * WZ) {
+    // ---- producer warp: cell-boundary tables one plane ahead, rounds two ahead of the consumers.
+    //      Table slot (p+1) % 3 last served plane p-2, whose rounds were all released before the
+    //      empty barrier of the first round of plane p could be passed (two staging buffers).
+    build_plane(0);
+    __syncwarp();
+    int pn = 0, rn = 0, an = 0;
+    for (int n = 0;; ++n) {
+      const int nb = n & 1;
+      if (n >= 2) mbar_wait(&empty[nb], ((n >> 1) - 1) & 1);
+      const RoundDesc nd = build_round(pn, rn, an, nb);
+      if (nd.p >= NP) break;
+      if (nd.r0 == 0 && nd.a0 == 0 && nd.p + 1 < NP) { build_plane(nd.p + 1); __syncwarp(); }
+      pn = nd.np; rn = nd.nr; an = nd.na;
+    }
+    return;
+  }
 
   float acc[SW][2][CB];
 #pragma unroll
@@ -412,18 +440,12 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
 #pragma unroll
       for (int c = 0; c < CB; ++c) acc[k][u][c] = 0.f;
 
-  uint32_t phase0 = 0, phase1 = 0;
-  for (int it = 0;; ++it) {
-    __syncthreads();
-    const int cur = it & 1;
+  // ---- consumer warps: free-running, coupled to the producer (and to nothing else) by the barriers
+  for (int n = 0;; ++n) {
+    const int cur = n & 1;
+    mbar_wait(&full[cur], (n >> 1) & 1);
     const RoundDesc d = s_desc[cur];
     if (d.p >= NP) break;
-    if (warp == 0) build_round(d.np, d.nr, d.na, cur ^ 1);
-    if (d.r0 == 0 && d.a0 == 0 && d.p + 2 < NP) build_plane(d.p + 2);
-    if (d.total > 0) {
-      if (cur == 0) { mbar_wait(&mbar[0], phase0); phase0 ^= 1; }
-      else          { mbar_wait(&mbar[1], phase1); phase1 ^= 1; }
-    }
     // ---- this thread's atoms of the round ----
     {
       const int tb = d.p % 3;
@@ -432,6 +454,8 @@ __global__ void __launch_bounds__(32 * WY * WZ, NCTA)
       build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32, d.a0, d.a1);
       walk_atoms<CB>(acc, s_run, NT, r_hi - r_beg, s_rec + (size_t)cur * cap * recf, recf, cb0, oy, oz);
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[cur]);   // this warp is done with the staged records and the round's offsets
     // ---- plane complete: its slot leaves the window; after the last cell plane so do the 7 planes
     //      beyond it.  Planes shared with a neighbouring segment are added (RED), the others stored.
     if (d.flush && lane_ok) {
@@ -472,7 +496,7 @@ struct SpreadLaunch {
     const size_t sm = smem_bytes(cap, recf);
     auto kern = k_spread_os<WY, WZ, CB, NCTA>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    kern<<<(unsigned)(npy * npz * nseg), S::NT, sm, st>>>(Mx, My, Mz, nseg, npy, npz, cap, recf, cb0, p->d_count,
+    kern<<<(unsigned)(npy * npz * nseg), S::NT + 32, sm, st>>>(Mx, My, Mz, nseg, npy, npz, cap, recf, cb0, p->d_count,
                                                          (const float*)p->d_rec, (float*)p->d_grid);
   }
 
@@ -547,7 +571,9 @@ void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {
   (void)n;
   // 16 x 32 column patches (8 warps), two CTAs per SM: measured 396 us against 407 us for 16 x 16
   // patches x 3 CTAs and 444 us for 16 x 16 x 4 CTAs at configuration 4
-  SpreadLaunch<2, 4, 2>::all_channels(p, st);
+  // 16 x 16 column patches: 4 consumer warps + 1 producer warp, three CTAs per SM (136 registers).
+  // Measured at configuration 4: 364 us; 16 x 32 patches x 2 CTAs (113 registers) 418 us.
+  SpreadLaunch<2, 2, 3>::all_channels(p, st);
 }
 
 }  // namespace pswf
