@@ -341,6 +341,39 @@ def test_zero_mode_option():
     assert abs(a["E_channels"][0] - b["E_channels"][0]) < 1e-6 * abs(a["E_channels"][0])
 
 
+def test_autograd_wrapper_matches_oracle_gradients():
+    """long_range_energy: backward gives dE/dr = -F and dE/dq = phi of oracle A (cfg 2, fp32 gates), scaled
+    by the incoming gradient; in fp64 (cfg 1) dE/dq agrees with central differences of the GPU energy."""
+    from paper_2606_06617_b200.autograd import long_range_energy
+    dev = torch.device("cuda:0")
+    wl = workloads.make(2)
+    plan = make_plan(wl)
+    pos = torch.tensor(wl["pos"], dtype=torch.float32, device=dev, requires_grad=True)
+    q = torch.tensor(wl["q"], dtype=torch.float32, device=dev, requires_grad=True)
+    E = long_range_energy(plan, pos, q)
+    (3.0 * E).backward()
+    torch.cuda.synchronize()
+    E_ref, _, phi_ref, F_ref = oracle_A(wl, plan.info()["r_c"])
+    assert abs(E.item() - E_ref) <= TOL_E32 * abs(E_ref)
+    assert rel(pos.grad.double().cpu().numpy(), -3.0 * F_ref) <= TOL_F32
+    assert rel(q.grad.double().cpu().numpy(), 3.0 * phi_ref) <= TOL_F32
+    plan.destroy()
+
+    wl = workloads.make(1)
+    plan = make_plan(wl)
+    pos = torch.tensor(wl["pos"], dtype=torch.float64, device=dev)
+    q = torch.tensor(wl["q"], dtype=torch.float64, device=dev, requires_grad=True)
+    long_range_energy(plan, pos, q).backward()
+    for a, i in [(0, 3), (0, 40)]:
+        d = 1e-4
+        qp, qm = q.detach().clone(), q.detach().clone()
+        qp[a, i] += d
+        qm[a, i] -= d
+        fd = (long_range_energy(plan, pos, qp).item() - long_range_energy(plan, pos, qm).item()) / (2 * d)
+        assert abs(fd - q.grad[a, i].item()) <= 1e-8 * max(1.0, abs(fd))     # E is quadratic in q
+    plan.destroy()
+
+
 def test_native_library_is_loaded():
     """The product path is the CUDA library: the shared object is mapped into this process."""
     binding.lib()
