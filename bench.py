@@ -317,10 +317,10 @@ def run_ours(args):
         cb = cpu_baseline(wl, info["r_c"])
 
     # this library's own kernels per evaluation (cuFFT's 6 kernels and 3 memsets not counted):
-    # fast: bin_count, 3 scan kernels, perm, records, spread, scale, finalize, interleave, gather (C <= 4)
-    # ref:  bin_count, 3 scan kernels, scatter, spread_ref, scale, finalize, gather_ref
+    # fast: bin_count, scan, perm, records, spread, scale, finalize, interleave, gather (C <= 4)
+    # ref:  bin_count, scan, scatter, spread_ref, scale, finalize, gather_ref
     groups = (C + 3) // 4
-    launches_per_step = {"ref": 9, "fast": 8 + 3 * groups}["fast" if args.kernel_path == 0 else "ref"]
+    launches_per_step = {"ref": 7, "fast": 6 + 3 * groups}["fast" if args.kernel_path == 0 else "ref"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",

@@ -31,20 +31,34 @@ __global__ void k_bin_count(int n, const T* __restrict__ pos, GridGeom<T> g, int
   rank[i] = atomicAdd(&count[k], 1);
 }
 
-// Exclusive scan of count[0..n) in place, three kernels (block scan, scan of block sums, add).
+// Exclusive scan of count[0..n) in place in ONE pass (decoupled look-back): a tile of 4096 counts per
+// CTA; tiles are handed out by a ticket counter, so every tile a CTA waits for is already running.
+// state[0] = ticket counter, state[1 + t] = (status << 32) | value of tile t with status 1 = the
+// tile's own sum, 2 = inclusive prefix up to and including the tile; zeroed before each launch.
 constexpr int kScanThreads = 512;
 constexpr int kScanItems = 8;
 
-__global__ void k_scan_blocks(int n, int* __restrict__ data, int* __restrict__ blocksums) {
+__global__ void __launch_bounds__(kScanThreads) k_scan_lookback(int n, int* __restrict__ data,
+                                                                unsigned long long* __restrict__ state,
+                                                                int total_slot, int total) {
   __shared__ int warp_tot[kScanThreads / 32];
-  const int base = (blockIdx.x * kScanThreads + threadIdx.x) * kScanItems;
+  __shared__ int s_tile, s_prefix;
+  if (threadIdx.x == 0) s_tile = (int)atomicAdd(reinterpret_cast<unsigned int*>(state), 1u);
+  __syncthreads();
+  const int tile = s_tile;
+  const int base = (tile * kScanThreads + threadIdx.x) * kScanItems;
   int v[kScanItems];
   int sum = 0;
+  if (base + kScanItems <= n) {
+    const int4 a = *reinterpret_cast<const int4*>(data + base);
+    const int4 b = *reinterpret_cast<const int4*>(data + base + 4);
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+  } else {
 #pragma unroll
-  for (int j = 0; j < kScanItems; ++j) {
-    v[j] = (base + j < n) ? data[base + j] : 0;
-    sum += v[j];
+    for (int j = 0; j < kScanItems; ++j) v[j] = (base + j < n) ? data[base + j] : 0;
   }
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) sum += v[j];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   int incl = sum;
 #pragma unroll
@@ -63,62 +77,40 @@ __global__ void k_scan_blocks(int n, int* __restrict__ data, int* __restrict__ b
       if (lane >= o) inc += u;
     }
     if (lane < kScanThreads / 32) warp_tot[lane] = inc - t;  // exclusive warp offsets
-    if (lane == 31) blocksums[blockIdx.x] = inc;
-  }
-  __syncthreads();
-  int run = warp_tot[wid] + incl - sum;
-#pragma unroll
-  for (int j = 0; j < kScanItems; ++j) {
-    if (base + j < n) data[base + j] = run;
-    run += v[j];
-  }
-}
-
-__global__ void k_scan_sums(int nblocks, int* __restrict__ blocksums) {
-  // single block: exclusive scan of blocksums, any length
-  __shared__ int warp_tot[32];
-  __shared__ int carry_s;
-  if (threadIdx.x == 0) carry_s = 0;
-  __syncthreads();
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int base = 0; base < nblocks; base += blockDim.x) {
-    int i = base + threadIdx.x;
-    int v = (i < nblocks) ? blocksums[i] : 0;
-    int incl = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      int t = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += t;
-    }
-    if (lane == 31) warp_tot[wid] = incl;
-    __syncthreads();
-    if (wid == 0) {
-      int t = warp_tot[lane];
-      int inc = t;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        int u = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += u;
+    if (lane == 31) {                                         // inc = the tile's sum
+      volatile unsigned long long* st = state + 1;
+      int prefix = 0;
+      if (tile == 0) {
+        st[0] = (2ull << 32) | (unsigned int)inc;
+      } else {
+        st[tile] = (1ull << 32) | (unsigned int)inc;
+        for (int p = tile - 1;; --p) {
+          unsigned long long sv;
+          do { sv = st[p]; } while ((sv >> 32) == 0ull);
+          prefix += (int)(unsigned int)sv;
+          if ((sv >> 32) == 2ull) break;
+        }
+        st[tile] = (2ull << 32) | (unsigned int)(prefix + inc);
       }
-      warp_tot[lane] = inc - t;
+      s_prefix = prefix;
     }
-    __syncthreads();
-    int carry = carry_s;
-    if (i < nblocks) blocksums[i] = carry + warp_tot[wid] + incl - v;
-    __syncthreads();
-    if (threadIdx.x == blockDim.x - 1) carry_s = carry + warp_tot[wid] + incl;
-    __syncthreads();
   }
-}
-
-__global__ void k_scan_add(int n, int* __restrict__ data, const int* __restrict__ blocksums, int total_slot,
-                           int total) {
-  const int base = (blockIdx.x * kScanThreads + threadIdx.x) * kScanItems;
-  const int add = blocksums[blockIdx.x];
+  __syncthreads();
+  int run = s_prefix + warp_tot[wid] + incl - sum;
+  if (base + kScanItems <= n) {
+    int o[kScanItems];
 #pragma unroll
-  for (int j = 0; j < kScanItems; ++j)
-    if (base + j < n) data[base + j] += add;
-  if (blockIdx.x == 0 && threadIdx.x == 0) data[total_slot] = total;
+    for (int j = 0; j < kScanItems; ++j) { o[j] = run; run += v[j]; }
+    *reinterpret_cast<int4*>(data + base) = make_int4(o[0], o[1], o[2], o[3]);
+    *reinterpret_cast<int4*>(data + base + 4) = make_int4(o[4], o[5], o[6], o[7]);
+  } else {
+#pragma unroll
+    for (int j = 0; j < kScanItems; ++j) {
+      if (base + j < n) data[base + j] = run;
+      run += v[j];
+    }
+  }
+  if (tile == 0 && threadIdx.x == 0) data[total_slot] = total;
 }
 
 template <class T>
@@ -344,9 +336,8 @@ void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const Gri
   cudaMemsetAsync(p->d_count, 0, sizeof(int) * ((size_t)Mtot + 1), st);
   if (n > 0)
     k_bin_count<T><<<(n + 255) / 256, 256, 0, st>>>(n, pos, g, p->d_count, p->d_key, p->d_rank);
-  k_scan_blocks<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_blocksums);
-  k_scan_sums<<<1, 1024, 0, st>>>(p->n_scan_blocks, p->d_blocksums);
-  k_scan_add<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_blocksums, Mtot, n);
+  cudaMemsetAsync(p->d_scan_state, 0, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), st);
+  k_scan_lookback<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_scan_state, Mtot, n);
   if (n > 0 && scatter)
     k_scatter<T><<<(n + 255) / 256, 256, 0, st>>>(n, p->C, p->cap_atoms, pos, q, g, p->d_count, p->d_key,
                                                    p->d_rank, p->d_perm, p->d_si0, (T*)p->d_sdelta,

@@ -85,7 +85,7 @@ struct pswf_lr_plan {
   void* d_gridi = nullptr;        // real  [M][CB] channel-interleaved copy of the potential grid (fast gather)
   void* d_spec = nullptr;         // cplx  [C][Mx][My][Mz/2+1]
   int* d_count = nullptr;         // [Mtot + 1] cell counts -> exclusive starts
-  int* d_blocksums = nullptr;
+  unsigned long long* d_scan_state = nullptr;   // [1 + n_scan_blocks] ticket counter + tile states of the scan
   int n_scan_blocks = 0;
   double* d_Ech = nullptr;        // [C]
   double* d_Etot = nullptr;       // [1] (execute_host staging)

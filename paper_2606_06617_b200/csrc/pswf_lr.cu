@@ -394,7 +394,7 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       if (!rc && stencil_path_supported(p)) rc = dev_alloc(&p->d_gridi, gather_grid_bytes(p), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_count, sizeof(int) * (Mtot + 1), &b);
       p->n_scan_blocks = (int)((Mtot + 4095) / 4096);
-      if (!rc) rc = dev_alloc((void**)&p->d_blocksums, sizeof(int) * (size_t)p->n_scan_blocks, &b);
+      if (!rc) rc = dev_alloc((void**)&p->d_scan_state, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Etot, sizeof(double), &b);
       p->workspace_bytes += b;
@@ -615,7 +615,7 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   cudaDeviceSynchronize();
   free_atoms(p);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
-                  p->d_grid,  p->d_spec,    p->d_count,    p->d_blocksums, p->d_Ech,      p->d_Etot,
+                  p->d_grid,  p->d_spec,    p->d_count,    p->d_scan_state, p->d_Ech,      p->d_Etot,
                   p->d_gridi};
   for (void* q : ptrs)
     if (q) cudaFree(q);
