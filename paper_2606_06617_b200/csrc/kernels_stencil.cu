@@ -96,9 +96,11 @@ __global__ void __launch_bounds__(256) k_perm(int n, const int* __restrict__ sta
 }
 
 // One thread per SORTED slot j: gathers pos / q of atom perm[j] (random 32-byte reads out of L2; the
-// inputs fit it), builds the records and leaves them through shared memory so that the CTA writes
-// 128 consecutive records with fully coalesced 16-byte stores.  (Scattering finished records from
-// atom order cost 300 us: 17 partially written sectors per atom; profiles/r1b.)
+// inputs fit it) and builds the records.  The 112-byte weight records straddle 32-byte sectors, so
+// they leave through shared memory and the CTA writes 128 consecutive records with fully coalesced
+// 16-byte stores; the 96-byte derivative records are three whole sectors each and are stored
+// directly (staging them too halved the resident CTAs: 100 us instead of 58 us).  (Scattering
+// finished records from atom order cost 300 us: 17 partially written sectors per atom; profiles/r1b.)
 //
 // The panel polynomials arrive BY VALUE (kernel parameter space = constant bank): with the panel
 // index and the power static, every Horner step is one FFMA with a constant-bank operand and no
@@ -111,15 +113,13 @@ __global__ void __launch_bounds__(kRecThreads) k_records(int n, int C, int recf,
                                                          const __grid_constant__ WindowPoly P,
                                                          const int* __restrict__ perm, float* __restrict__ rec,
                                                          float* __restrict__ drec) {
-  extern __shared__ __align__(16) float s_stage[];   // [kRecThreads][recf] | [kRecThreads][24]
-  float* s_rec = s_stage;
-  float* s_drec = s_stage + kRecThreads * recf;
+  extern __shared__ __align__(16) float s_rec[];   // [kRecThreads][recf]
   const int j0 = blockIdx.x * kRecThreads;
   const int j = j0 + threadIdx.x;
   if (j < n) {
     const int i = __ldg(perm + j);
     float* r = s_rec + threadIdx.x * recf;
-    float* dr = s_drec + threadIdx.x * (3 * SW);
+    float* dr = drec + (size_t)j * (3 * SW);   // 96 bytes = three whole 32-byte sectors: stored directly
     const float px[3] = {__ldg(pos + 3 * (size_t)i), __ldg(pos + 3 * (size_t)i + 1), __ldg(pos + 3 * (size_t)i + 2)};
     for (int c0 = 0; c0 < recf - 3 * SW; c0 += 4) {
       float qq[4];
@@ -159,9 +159,7 @@ __global__ void __launch_bounds__(kRecThreads) k_records(int n, int C, int recf,
   const int nrec = min(kRecThreads, n - j0);
   const int rq = recf >> 2;
   float4* grec = reinterpret_cast<float4*>(rec + (size_t)j0 * recf);
-  float4* gdrec = reinterpret_cast<float4*>(drec + (size_t)j0 * (3 * SW));
   for (int t = threadIdx.x; t < nrec * rq; t += kRecThreads) grec[t] = reinterpret_cast<const float4*>(s_rec)[t];
-  for (int t = threadIdx.x; t < nrec * 6; t += kRecThreads) gdrec[t] = reinterpret_cast<const float4*>(s_drec)[t];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -551,7 +549,7 @@ void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const floa
   if (n <= 0) return;
   const int recf = stencil_rec_floats(p->C);
   k_perm<<<(n + 255) / 256, 256, 0, st>>>(n, p->d_count, p->d_key, p->d_rank, p->d_perm);
-  const size_t sm = sizeof(float) * kRecThreads * (size_t)(recf + 3 * SW);
+  const size_t sm = sizeof(float) * kRecThreads * (size_t)recf;
   const unsigned nb = (unsigned)((n + kRecThreads - 1) / kRecThreads);
 #define PSWF_REC(D)                                                                                              \
   case D:                                                                                                        \
