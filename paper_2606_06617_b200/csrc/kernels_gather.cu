@@ -131,7 +131,7 @@ __host__ __device__ constexpr int gather_warp_floats(int recf) { return kStage *
 
 template <int CB, int GBX, int GBY, int NCTA>   // GBX x GBY cell rows (warps) per CTA, NCTA resident CTAs per SM
 __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
-    k_gather_rows(int n, int C, int cb0, int Mx, int My, int Mz, int nbx, int nby, int recf,
+    k_gather_rows(int n, int C, int cb0, int Mx, int My, int Mz, int nseg, int nbx, int nby, int recf,
                   const int* __restrict__ start, const float* __restrict__ rec, const float* __restrict__ drec,
                   const int* __restrict__ perm, const typename VecOf<CB>::type* __restrict__ gridt,
                   float* __restrict__ phi, float* __restrict__ Facc, int accumulate_F) {
@@ -145,10 +145,12 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   // at the same time share most of their footprints in L1
   int bid = blockIdx.x;
   const int by = bid % nby; bid /= nby;
-  const int bx = bid % nbx; bid /= nbx;
-  const int seg = bid;
+  const int bx = bid % nbx;
   const int sx = bx * GBX + wid / GBY, sy = by * GBY + wid % GBY;
   if (sx >= Mx || sy >= My) return;
+  // the warp walks the z segments of its row one after the other (a CTA per segment spent a tenth
+  // of its short life being launched)
+  for (int seg = 0; seg < nseg; ++seg) {
   const int Z0 = seg * ZSEG, Z1 = min(Z0 + ZSEG, Mz);
 
   // cell boundaries of the segment: lane l <-> cell Z0 + l; the atoms of the row are one run
@@ -159,7 +161,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
     jhi_l = __ldg(start + key + 1);
   }
   const unsigned mask = __ballot_sync(0xffffffffu, jhi_l > jlo_l);
-  if (mask == 0u) return;   // no atoms in this segment of the row (vacuum)
+  if (mask == 0u) continue;   // no atoms in this segment of the row (vacuum)
   const int first = __ffs(mask) - 1, last = 31 - __clz(mask);
   const int jbeg = __shfl_sync(0xffffffffu, jlo_l, first), jend = __shfl_sync(0xffffffffu, jhi_l, last);
 
@@ -335,6 +337,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   }
   retire();
   flush(jend - js);
+  }   // segments
 }
 
 }  // namespace
@@ -359,7 +362,7 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, cudaStre
   const size_t Mtot = (size_t)Mx * My * Mz;
   const int nseg = (Mz + ZSEG - 1) / ZSEG;
   const int nbx = (Mx + GBX - 1) / GBX, nby = (My + GBY - 1) / GBY;
-  const unsigned blocks = (unsigned)(nseg * nbx * nby);
+  const unsigned blocks = (unsigned)(nbx * nby);
   const dim3 iblocks((unsigned)((Mz + 31) / 32), (unsigned)((My + 31) / 32), (unsigned)Mx);
   const int recf = stencil_rec_floats(p->C);
   const size_t smem = sizeof(float) * GBX * GBY * (size_t)gather_warp_floats(recf);
@@ -375,7 +378,7 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, cudaStre
     k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);                          \
     auto kern = k_gather_rows<CBV, GBX, GBY, NCTA>;                                                         \
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \
-    kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nbx, nby, recf, p->d_count,        \
+    kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nbx, nby, recf, p->d_count,        \
                                                (const float*)p->d_rec, (const float*)p->d_drec, p->d_perm,  \
                                                (const V*)gi, phi, F, acc);                                  \
     gi += Mtot * CBV;                                                                                       \
