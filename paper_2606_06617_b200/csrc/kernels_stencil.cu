@@ -189,6 +189,23 @@ struct SpreadShape {
   static_assert(2 * sizeof(RoundDesc) + 32 <= 128, "header");
 };
 
+// Packed FP32 pairs (sm_100a FFMA2: one instruction, two IEEE fused multiply-adds per lane -- the FLOP
+// rate of FFMA at half the issue slots; the stencil kernels are issue-bound, not FMA-pipe-bound).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+  f32x2 d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+  return d;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+
 __device__ __forceinline__ void red_add_v2(float* p, float a, float b) {
   asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
 }
@@ -220,7 +237,7 @@ __device__ __forceinline__ void build_runs(uint2* runs, const int NT, const int 
 }
 
 template <int CB>
-__device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], const uint2* runs, const int NT, const int nrows,
+__device__ __forceinline__ void walk_atoms(f32x2 (&acc)[SW / 2][2][CB], const uint2* runs, const int NT, const int nrows,
                                            const float* rbase, const int recf, const int cb0, const int oy,
                                            const int oz) {
   // loop invariants pinned to registers (ptxas otherwise reloads the kernel parameters from the
@@ -260,14 +277,16 @@ __device__ __forceinline__ void walk_atoms(float (&acc)[SW][2][CB], const uint2*
     const float2 wzv = *reinterpret_cast<const float2*>(rp + oz);
     const float p0 = j < jb ? wyv * wzv.x : 0.f;
     const float p1 = j >= ja ? wyv * wzv.y : 0.f;
-    const float wx[SW] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+    // x pairs (k, k+1) share one FFMA2: acc[k/2] = {plane k, plane k+1} += {wx[k], wx[k+1]} * {v, v}
+    const f32x2 wx[SW / 2] = {pack2(wa.x, wa.y), pack2(wa.z, wa.w), pack2(wb.x, wb.y), pack2(wb.z, wb.w)};
 #pragma unroll
     for (int c = 0; c < CB; ++c) {
       const float v0 = p0 * qv[c], v1 = p1 * qv[c];
+      const f32x2 d0 = pack2(v0, v0), d1 = pack2(v1, v1);
 #pragma unroll
-      for (int k2 = 0; k2 < SW; ++k2) {
-        acc[k2][0][c] = fmaf(wx[k2], v0, acc[k2][0][c]);
-        acc[k2][1][c] = fmaf(wx[k2], v1, acc[k2][1][c]);
+      for (int k2 = 0; k2 < SW / 2; ++k2) {
+        acc[k2][0][c] = ffma2(wx[k2], d0, acc[k2][0][c]);
+        acc[k2][1][c] = ffma2(wx[k2], d1, acc[k2][1][c]);
       }
     }
     ++j;
@@ -430,13 +449,13 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
     return;
   }
 
-  float acc[SW][2][CB];
+  f32x2 acc[SW / 2][2][CB];   // register window: acc[k/2][column][channel] = {plane k, plane k+1}, k = x mod 8
 #pragma unroll
-  for (int k = 0; k < SW; ++k)
+  for (int k = 0; k < SW / 2; ++k)
 #pragma unroll
     for (int u = 0; u < 2; ++u)
 #pragma unroll
-      for (int c = 0; c < CB; ++c) acc[k][u][c] = 0.f;
+      for (int c = 0; c < CB; ++c) acc[k][u][c] = 0ull;
 
   // ---- consumer warps: free-running, coupled to the producer (and to nothing else) by the barriers
   for (int n = 0;; ++n) {
@@ -467,10 +486,14 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
 #define PSWF_FLUSH(K)                                                                          \
   case K:                                                                                      \
     _Pragma("unroll") for (int c = 0; c < CB; ++c) {                                           \
-      if (shared) red_add_v2(gp + (size_t)c * Mtot, acc[K][0][c], acc[K][1][c]);               \
-      else *reinterpret_cast<float2*>(gp + (size_t)c * Mtot) = make_float2(acc[K][0][c], acc[K][1][c]); \
-      acc[K][0][c] = 0.f;                                                                      \
-      acc[K][1][c] = 0.f;                                                                      \
+      float a0, a1, b0, b1;                                                                    \
+      unpack2(acc[K / 2][0][c], a0, a1);                                                       \
+      unpack2(acc[K / 2][1][c], b0, b1);                                                       \
+      const float s0 = (K & 1) ? a1 : a0, s1 = (K & 1) ? b1 : b0;                              \
+      if (shared) red_add_v2(gp + (size_t)c * Mtot, s0, s1);                                   \
+      else *reinterpret_cast<float2*>(gp + (size_t)c * Mtot) = make_float2(s0, s1);            \
+      acc[K / 2][0][c] = (K & 1) ? pack2(a0, 0.f) : pack2(0.f, a1);                            \
+      acc[K / 2][1][c] = (K & 1) ? pack2(b0, 0.f) : pack2(0.f, b1);                            \
     }                                                                                          \
     break;
           PSWF_FLUSH(0) PSWF_FLUSH(1) PSWF_FLUSH(2) PSWF_FLUSH(3)
