@@ -28,6 +28,8 @@
 //  * per atom: z contraction with value and derivative weights in one pass (2 x 8 x 2 FFMA per
 //    channel per lane), combination with the (x,y) weights, 9-shuffle transpose-reduce of
 //    (phi_a, F_x, F_y, F_z), scattered store to the caller's atom order.
+#include <type_traits>
+
 #include "kernels_common.cuh"
 #include "launch.hpp"
 
@@ -114,6 +116,30 @@ __device__ __forceinline__ float reduce8(float (&v)[8], int lane) {
 
 __device__ __forceinline__ void prefetch_l1(const void* p) {
   asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+}
+
+// Packed FP32 pairs (sm_100a FFMA2: one instruction, two IEEE fused multiply-adds per lane; ptxas
+// uses its broadcast-scalar operand form for pack2(w, w)).  The gather is issue-bound, not
+// FMA-pipe-bound: pairing adjacent channels halves the FMA instruction count of the contraction.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+  f32x2 d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+  return d;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+
+__device__ __forceinline__ f32x2 ffma2v(f32x2 a, f32x2 b, f32x2 c) {   // program order kept
+  f32x2 d;
+  asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
 }
 
 constexpr int kStage = 32;       // atoms staged per warp at a time (one lane per atom for the output pass)
@@ -217,13 +243,27 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   // warm-up: the 8 planes sz0 .. sz0+7 of the first non-empty cell, slot k <- the plane z == k (mod 8)
   // (static slots: 16 independent loads in flight, straight into the window registers)
   const int sz0 = Z0 + first, sz1 = Z0 + last;
-  float win[SW][2][CB];
+  // window registers: channel pairs are held PACKED (one 64-bit register pair = {c, c+1}, exactly as
+  // the 16-byte plane loads deliver them), ready to be FFMA2 operands
+  constexpr int NE = (CB % 2 == 0) ? CB / 2 : CB;
+  using WE = typename std::conditional<CB % 2 == 0, f32x2, float>::type;
+  WE win[SW][2][NE];
+  auto ldw = [&](const V* p, WE (&d)[NE]) {
+    if constexpr (CB == 4) {
+      const ulonglong2 t = __ldg(reinterpret_cast<const ulonglong2*>(p));
+      d[0] = t.x; d[1] = t.y;
+    } else if constexpr (CB == 2) {
+      d[0] = __ldg(reinterpret_cast<const unsigned long long*>(p));
+    } else {
+      d[0] = __ldg(p);
+    }
+  };
 #pragma unroll
   for (int k = 0; k < SW; ++k) {
     int z = sz0 + ((k - sz0) & 7); if (z >= Mz) z -= Mz;
     const unsigned off = (unsigned)z * plane;
-    unpack<CB>(__ldg(g0 + off), win[k][0]);
-    unpack<CB>(__ldg(g1 + off), win[k][1]);
+    ldw(g0 + off, win[k][0]);
+    ldw(g1 + off, win[k][1]);
   }
   cp_async_wait_all();
   __syncwarp();
@@ -276,6 +316,39 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
         const float xdy[2] = {wx0 * dy, wx1 * dy};     // d/dy
         retire();   // the previous atom's reduction: independent of everything below, interleaved by ptxas
         float fx = 0.f, fy = 0.f, fz = 0.f;
+        if constexpr (CB % 2 == 0) {
+          // channel pairs (c, c+1): {S_c, S_c+1} += w * {win_c, win_c+1}, one FFMA2 each
+          f32x2 fx2 = 0ull, fy2 = 0ull, fz2 = 0ull;
+#pragma unroll
+          for (int c = 0; c < CB; c += 2) {
+            // four chains {S0, S1} x {point 0, point 1} in round-robin order (the volatile asm keeps
+            // it): 16 accumulator registers would not fit beside the 64-register window
+            f32x2 S00 = 0ull, S10 = 0ull, S01 = 0ull, S11 = 0ull;
+#pragma unroll
+            for (int k = 0; k < SW; ++k) {
+              const f32x2 ga = win[k][0][c / 2], gb = win[k][1][c / 2];
+              const f32x2 wk = pack2(wz[k], wz[k]), dk = pack2(dz[k], dz[k]);
+              S00 = ffma2v(ga, wk, S00);
+              S10 = ffma2v(ga, dk, S10);
+              S01 = ffma2v(gb, wk, S01);
+              S11 = ffma2v(gb, dk, S11);
+            }
+            const f32x2 xy0 = pack2(xy[0], xy[0]), xy1 = pack2(xy[1], xy[1]);
+            f32x2 val = ffma2(S01, xy1, ffma2(S00, xy0, 0ull));
+            f32x2 gz = ffma2(S11, xy1, ffma2(S10, xy0, 0ull));
+            f32x2 gx = ffma2(S01, pack2(dxy[1], dxy[1]), ffma2(S00, pack2(dxy[0], dxy[0]), 0ull));
+            f32x2 gy = ffma2(S01, pack2(xdy[1], xdy[1]), ffma2(S00, pack2(xdy[0], xdy[0]), 0ull));
+            const f32x2 q2 = pack2(qv[c], qv[c + 1]);
+            fx2 = ffma2(q2, gx, fx2);
+            fy2 = ffma2(q2, gy, fy2);
+            fz2 = ffma2(q2, gz, fz2);
+            unpack2(val, pend[c], pend[c + 1]);
+          }
+          float a, b;
+          unpack2(fx2, a, b); fx = -(a + b);
+          unpack2(fy2, a, b); fy = -(a + b);
+          unpack2(fz2, a, b); fz = -(a + b);
+        } else {
 #pragma unroll
         for (int c = 0; c < CB; ++c) {
           float val = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
@@ -298,6 +371,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
           fz = fmaf(-qc, gz, fz);
           pend[c] = val;
         }
+        }
 #pragma unroll
         for (int c = CB; c < 4; ++c) pend[c] = 0.f;
         pend[4] = fx; pend[5] = fy; pend[6] = fz; pend[7] = 0.f;
@@ -316,8 +390,8 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
     unsigned off = (unsigned)zz * plane;
 #define PSWF_SLOT(K)                         \
   case K:                                    \
-    unpack<CB>(__ldg(g0 + off), win[K][0]);  \
-    unpack<CB>(__ldg(g1 + off), win[K][1]);  \
+    ldw(g0 + off, win[K][0]);                \
+    ldw(g1 + off, win[K][1]);                \
     off += plane;                            \
     if (off == wrap) off = 0u;
     switch ((Z0 + ps) & 7) {
