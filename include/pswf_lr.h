@@ -109,6 +109,21 @@ int pswf_lr_execute(pswf_lr_plan* plan, int n_atoms, const void* pos, const void
 int pswf_lr_execute_host(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, double* E,
                          void* phi, void* F, void* stream);
 
+/* Real-space complement and self term: the part of the full inverse-power
+ * energy (S65), that the reciprocal path above does not contain,
+ *   E = 1/2 sum_a sum_{i != j, images} q_i^a q_j^a L_{p_a,r_c}(|r_ij|)  -  E_self,
+ *   L_{p,r_c}(r) = r^-p - S_{p,r_c}(r) for r < r_c (SI Props. 2-7, (S17)-(S33)), 0 beyond;
+ *   E_self = sum_a S_{p_a}(0) sum_i (q_i^a)^2 / (2 r_c^p_a)              (S66)-(S67).
+ * Arguments as pswf_lr_execute; phi_i^a = dE/dq_i^a and F_i = -dE/dr_i of THIS part.  With
+ * accumulate != 0 the results are ADDED to what E, phi and F already hold, so that
+ *   pswf_lr_execute(...); pswf_lr_execute_real(..., 1, stream);
+ * returns the complete energy, potentials and forces of (S65).  Asynchronous on `stream`; it re-sorts
+ * the atoms (the plan's sort buffers are shared with pswf_lr_execute: same-stream use only).
+ * Fails with PSWF_LR_ERR_GRID_TOO_COARSE when r_c >= L_d / 2 in some dimension (only the minimum
+ * image of a pair is visited). */
+int pswf_lr_execute_real(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, void* E,
+                         void* phi, void* F, int accumulate, void* stream);
+
 /* Per-channel energies of the most recent execute: device double[n_channels] (async on stream).
  * The paper reports per-component contributions. */
 int pswf_lr_channel_energies(pswf_lr_plan* plan, void* E_channels, void* stream);
@@ -136,6 +151,9 @@ int pswf_lr_debug_copy(pswf_lr_plan* plan, int what, void* dst, void* stream);
  *   kernel:  Phi^_p(k) as the scale kernel evaluates it (k in 1/A) */
 int pswf_lr_eval_window(const pswf_lr_plan* plan, int n, const double* z, double* W, double* dW);
 int pswf_lr_eval_kernel(const pswf_lr_plan* plan, int p, int n, const double* k, double* Phi);
+/*   real:    L_{p,r_c}(r) and dL/dr (r in A) from the numerator polynomials; S_p(0) of (S67) */
+int pswf_lr_eval_real(const pswf_lr_plan* plan, int p, int n, const double* r, double* L, double* dL);
+int pswf_lr_self_coefficient(const pswf_lr_plan* plan, int p, double* S0);
 
 int pswf_lr_destroy(pswf_lr_plan* plan);
 const char* pswf_lr_error_string(int code);

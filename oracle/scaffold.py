@@ -1,6 +1,7 @@
 """Validation scaffold: the pieces of (S65) that are NOT on the hot path (float64).
 
-TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).  Never timed, never compared with the GPU.
+TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).  Never timed.  `real_space_parts` is the
+parity target of the library's real-space row (pswf_lr_execute_real).
 It exists so the oracle's reciprocal part can be pinned to physics the paper fixes: the total
 
     E^(p) = E_real + (1/2V) sum_{k!=0} Phi^ |rho|^2 + E_0 - E_self        (S65)
@@ -32,6 +33,42 @@ def real_space_complement(pos, q, p, box, moll):
             mask &= ~np.eye(len(pos), dtype=bool)
         E += 0.5 * np.sum(qq[mask] * moll.L_phys(p, r[mask]))
     return float(E)
+
+
+def real_space_parts(pos, q, exponents, box, c, r_c, fd=1e-6):
+    """Real-space complement minus self term for several channels: returns (E, phi[C][N], F[N][3]) with
+        E   = sum_a [ 1/2 sum_n sum_{i,j}' q_i^a q_j^a L_{p_a,r_c}(|r_ij + n.L|) - E_self^a ]   (S64)-(S66)
+        phi = dE/dq_i^a = sum_j q_j^a L(r_ij) - S_p(0) q_i^a / r_c^p
+        F_i = -dE/dr_i, with dL/dr by central differences of L (step fd): the scaffold has no
+              closed-form derivative of its own, and none is needed at 1e-8 relative accuracy."""
+    pos = np.asarray(pos, dtype=np.float64)
+    q = np.atleast_2d(np.asarray(q, dtype=np.float64))
+    box = np.asarray(box, dtype=np.float64)
+    moll = Mollifier(c, r_c)
+    N = len(pos)
+    phi = np.zeros_like(q)
+    F = np.zeros((N, 3))
+    nmax = np.ceil(r_c / box).astype(int)
+    d0 = pos[None, :, :] - pos[:, None, :]          # d0[i, j] = r_j - r_i
+    for n in itertools.product(*[range(-k, k + 1) for k in nmax]):
+        d = d0 + np.asarray(n) * box
+        r = np.sqrt((d ** 2).sum(-1))
+        mask = (r > 0) & (r < r_c)
+        if not mask.any():
+            continue
+        ii, jj = np.nonzero(mask)
+        rr = r[ii, jj]
+        for a, p in enumerate(exponents):
+            L = moll.L_phys(p, rr)
+            dL = (moll.L_phys(p, np.minimum(rr + fd, r_c * (1 - 1e-15))) - moll.L_phys(p, rr - fd)) / \
+                 (np.minimum(rr + fd, r_c * (1 - 1e-15)) - (rr - fd))
+            np.add.at(phi[a], ii, q[a, jj] * L)
+            f = (q[a, ii] * q[a, jj] * dL / rr)[:, None] * d[ii, jj]      # F_i = + qq L'(r) (r_j - r_i)/r
+            np.add.at(F, ii, f)
+    for a, p in enumerate(exponents):
+        phi[a] -= moll.S_zero(p) * q[a] / r_c ** p
+    E = 0.5 * float(np.sum(q * phi))
+    return E, phi, F
 
 
 def self_energy(q, p, moll):

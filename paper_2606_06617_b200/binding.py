@@ -43,6 +43,7 @@ class Info(ctypes.Structure):
 
 
 EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_execute", "pswf_lr_execute_host",
+           "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient",
            "pswf_lr_channel_energies", "pswf_lr_get_info", "pswf_lr_set_profiling", "pswf_lr_stage_ms",
            "pswf_lr_debug_copy", "pswf_lr_eval_window", "pswf_lr_eval_kernel", "pswf_lr_destroy",
            "pswf_lr_error_string", "pswf_lr_version")
@@ -65,6 +66,9 @@ def lib():
         L.pswf_lr_plan_create_ex.argtypes = L.pswf_lr_plan_create.argtypes + [ctypes.POINTER(Opts)]
         L.pswf_lr_execute.argtypes = [vp, ip, vp, vp, vp, vp, vp, vp]
         L.pswf_lr_execute_host.argtypes = [vp, ip, vp, vp, dp, vp, vp, vp]
+        L.pswf_lr_execute_real.argtypes = [vp, ip, vp, vp, vp, vp, vp, ip, vp]
+        L.pswf_lr_eval_real.argtypes = [vp, ip, ip, dp, dp, dp]
+        L.pswf_lr_self_coefficient.argtypes = [vp, ip, dp]
         L.pswf_lr_channel_energies.argtypes = [vp, vp, vp]
         L.pswf_lr_get_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.pswf_lr_set_profiling.argtypes = [vp, ip]
@@ -161,6 +165,24 @@ class Plan:
         """Device tensors (torch) in the plan precision; E is a float64 device tensor of 1 element."""
         _check(lib().pswf_lr_execute(self._h, int(n_atoms), _ptr(pos), _ptr(q), _ptr(E), _ptr(phi), _ptr(F),
                                      ctypes.c_void_p(stream or 0)))
+
+    def execute_real(self, n_atoms, pos, q, E=None, phi=None, F=None, accumulate=False, stream=None):
+        """Real-space complement - self term (device tensors); accumulate=True adds to E, phi, F."""
+        _check(lib().pswf_lr_execute_real(self._h, int(n_atoms), _ptr(pos), _ptr(q), _ptr(E), _ptr(phi), _ptr(F),
+                                          1 if accumulate else 0, ctypes.c_void_p(stream or 0)))
+
+    def eval_real(self, p, r):
+        r = np.ascontiguousarray(r, dtype=np.float64)
+        L, dL = np.empty_like(r), np.empty_like(r)
+        dp = ctypes.POINTER(ctypes.c_double)
+        _check(lib().pswf_lr_eval_real(self._h, int(p), r.size, r.ctypes.data_as(dp), L.ctypes.data_as(dp),
+                                       dL.ctypes.data_as(dp)))
+        return L, dL
+
+    def self_coefficient(self, p):
+        v = ctypes.c_double(0.0)
+        _check(lib().pswf_lr_self_coefficient(self._h, int(p), ctypes.byref(v)))
+        return v.value
 
     def execute_host(self, n_atoms, pos, q, E=None, phi=None, F=None, stream=None):
         """Host buffers (numpy arrays or pinned torch CPU tensors); E: float64 host array of 1."""

@@ -27,4 +27,9 @@ void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const floa
                             cudaStream_t st);
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st);
 
+// real-space complement + self term (kernels_real.cu); uses the sort left by launch_bin_sort(scatter = true)
+template <class T>
+void launch_real_space(pswf_lr_plan* p, int n, const T* pos, const RealGeom<T>& g, const RealParams<T>& P, double* E,
+                       T* phi, T* F, int accumulate, cudaStream_t st);
+
 }  // namespace pswf

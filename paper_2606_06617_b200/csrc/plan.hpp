@@ -7,6 +7,7 @@
 
 #include "../../include/pswf_lr.h"
 #include "host_tables.hpp"
+#include "real_tables.hpp"
 
 namespace pswf {
 
@@ -56,6 +57,26 @@ struct GridGeom {
   const T* wdcoef;     // [wdeg][w]
 };
 
+// Geometry and tables of the real-space complement kernel (kernels_real.cu), passed by value.
+template <class T>
+struct RealGeom {
+  int M[3];
+  int R[3];            // cell search radius per dimension: floor(r_c / h_d) + 1
+  double invL[3];
+  T L[3];
+};
+template <class T>
+struct RealParams {
+  int C, nslots, panels, degree;
+  int slot_p[6];
+  int chan_slot[kMaxChannels];
+  T slot_pre[6];               // r_c^-p per slot
+  T self_pre[kMaxChannels];    // S_p(0) / r_c^p per channel
+  T r_c, inv_rc;
+  const T* coef;               // [slot][panel][degree+1]  N_p
+  const T* dcoef;              // [slot][panel][degree]    dN_p/dx
+};
+
 }  // namespace pswf
 
 struct pswf_lr_plan {
@@ -75,6 +96,13 @@ struct pswf_lr_plan {
   pswf::WindowTable wt;
   pswf::KernelTable kt;
   pswf::WindowPoly wpoly;         // fast path copy of wt (float, zero padded)
+  pswf::RealTable rt;             // real-space complement numerators N_p, S_p(0)
+  int real_R[3] = {0, 0, 0};      // cell search radius of the pair kernel
+  bool real_ok = false;           // r_c < L_d / 2 and 2 R_d + 1 <= M_d in every dimension
+  void* d_rcoef = nullptr;
+  void* d_rdcoef = nullptr;
+  void* d_spos = nullptr;         // real [3][cap] wrapped positions in sorted order
+  double* d_Ereal = nullptr;      // [1]
   // device tables (plan precision)
   void* d_wcoef = nullptr;
   void* d_wdcoef = nullptr;

@@ -46,7 +46,7 @@ int dev_alloc(void** ptr, size_t bytes, long long* total) {
 }
 
 void free_atoms(pswf_lr_plan* p) {
-  void** ptrs[] = {(void**)&p->d_key, (void**)&p->d_rank, (void**)&p->d_perm, (void**)&p->d_si0, &p->d_sdelta,
+  void** ptrs[] = {&p->d_spos, (void**)&p->d_key, (void**)&p->d_rank, (void**)&p->d_perm, (void**)&p->d_si0, &p->d_sdelta,
                    &p->d_sq,          &p->d_rec,          &p->d_drec,         &p->d_pos_in,       &p->d_q_in,        &p->d_phi_out,
                    &p->d_F_out};
   for (void** q : ptrs) {
@@ -70,6 +70,7 @@ int ensure_capacity(pswf_lr_plan* p, int n) {
   rc |= dev_alloc((void**)&p->d_si0, sizeof(int) * 3 * (size_t)cap, &b);
   rc |= dev_alloc(&p->d_sdelta, rs * 3 * (size_t)cap, &b);
   rc |= dev_alloc(&p->d_sq, rs * (size_t)p->C * cap, &b);
+  rc |= dev_alloc(&p->d_spos, rs * 3 * (size_t)cap, &b);
   p->cap_atoms = cap;
   size_t recb = stencil_path_supported(p) ? stencil_record_bytes(p) * (size_t)cap : 0;
   if (recb) rc |= dev_alloc(&p->d_rec, recb, &b);
@@ -217,6 +218,43 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
 
 }  // namespace
 
+namespace {
+template <class T>
+int execute_real_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* phi, T* F, int accumulate,
+                   cudaStream_t st) {
+  GridGeom<T> g = make_geom<T>(p);
+  launch_bin_sort<T>(p, n, pos, q, g, true, st);   // generic sort: perm, si0, sq
+  RealGeom<T> rg;
+  RealParams<T> P;
+  memset(&P, 0, sizeof(P));
+  for (int d = 0; d < 3; ++d) {
+    rg.M[d] = p->M[d];
+    rg.R[d] = p->real_R[d];
+    rg.invL[d] = 1.0 / p->L[d];
+    rg.L[d] = (T)p->L[d];
+  }
+  P.C = p->C;
+  P.nslots = (int)p->distinct_p.size();
+  P.panels = p->rt.panels;
+  P.degree = p->rt.degree;
+  for (int s = 0; s < P.nslots; ++s) {
+    P.slot_p[s] = p->distinct_p[s];
+    P.slot_pre[s] = (T)std::pow(p->r_c, -(double)p->distinct_p[s]);
+  }
+  for (int a = 0; a < p->C; ++a) {
+    P.chan_slot[a] = p->chan_slot[a];
+    P.self_pre[a] = (T)(p->rt.S0[p->chan_slot[a]] * std::pow(p->r_c, -(double)p->chan_p[a]));
+  }
+  P.r_c = (T)p->r_c;
+  P.inv_rc = (T)(1.0 / p->r_c);
+  P.coef = (const T*)p->d_rcoef;
+  P.dcoef = (const T*)p->d_rdcoef;
+  launch_real_space<T>(p, n, pos, rg, P, E, phi, F, accumulate, st);
+  CUDA_TRY(cudaGetLastError());
+  return 0;
+}
+}  // namespace
+
 extern "C" {
 
 const char* pswf_lr_version(void) { return "pswf_lr 0.1 (sm_100a)"; }
@@ -351,6 +389,14 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       const int panels = p->precision == PSWF_LR_F64 ? 32 : 16;
       p->kt = fit_kernels(km, p->distinct_p, panels, p->poly_eps, kMaxKernelDegree);
       for (int pp : p->distinct_p) p->Phi0.push_back(km.Phi0(pp, p->r_c));
+      // real-space complement: numerators N_p, self constants S_p(0), cell search radius
+      RealMath rm(psi);
+      p->rt = fit_real(rm, p->distinct_p, panels, p->poly_eps, kMaxKernelDegree);
+      p->real_ok = true;
+      for (int d = 0; d < 3; ++d) {
+        p->real_R[d] = (int)std::floor(p->r_c / p->h[d]) + 1;
+        if (!(p->r_c < 0.5 * p->L[d])) p->real_ok = false;
+      }
       // count modes in the ball (half spectrum), for info / roofline bytes
       long long cnt = 0;
       const double kc2 = (c / p->r_c) * (c / p->r_c);
@@ -379,11 +425,15 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
         rc |= upload<double>(&p->d_wcoef, p->wt.coef, &b);
         rc |= upload<double>(&p->d_wdcoef, p->wt.dcoef, &b);
         rc |= upload<double>(&p->d_kcoef, p->kt.coef, &b);
+        rc |= upload<double>(&p->d_rcoef, p->rt.coef, &b);
+        rc |= upload<double>(&p->d_rdcoef, p->rt.dcoef, &b);
         for (int d = 0; d < 3; ++d) rc |= upload<double>(&p->d_invW2[d], invW2[d], &b);
       } else {
         rc |= upload<float>(&p->d_wcoef, p->wt.coef, &b);
         rc |= upload<float>(&p->d_wdcoef, p->wt.dcoef, &b);
         rc |= upload<float>(&p->d_kcoef, p->kt.coef, &b);
+        rc |= upload<float>(&p->d_rcoef, p->rt.coef, &b);
+        rc |= upload<float>(&p->d_rdcoef, p->rt.dcoef, &b);
         for (int d = 0; d < 3; ++d) rc |= upload<float>(&p->d_invW2[d], invW2[d], &b);
       }
       const size_t rs = real_size(p);
@@ -397,6 +447,7 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       if (!rc) rc = dev_alloc((void**)&p->d_scan_state, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Etot, sizeof(double), &b);
+      if (!rc) rc = dev_alloc((void**)&p->d_Ereal, sizeof(double), &b);
       p->workspace_bytes += b;
     }
     if (!rc && !p->host_only) {
@@ -467,6 +518,61 @@ int pswf_lr_execute_host(pswf_lr_plan* p, int n, const void* pos, const void* q,
   if (F && n > 0) CUDA_TRY(cudaMemcpyAsync(F, p->d_F_out, rs * 3 * (size_t)n, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
   return 0;
+}
+
+int pswf_lr_execute_real(pswf_lr_plan* p, int n_atoms, const void* pos, const void* q, void* E, void* phi, void* F,
+                         int accumulate, void* stream) {
+  if (!p || n_atoms < 0) return PSWF_LR_ERR_INVALID_ARG;
+  if (n_atoms > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  if (!p->real_ok) return PSWF_LR_ERR_GRID_TOO_COARSE;   // r_c >= L_d / 2: minimum image does not suffice
+  int rc = ensure_capacity(p, n_atoms);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (p->precision == PSWF_LR_F64)
+    return execute_real_t<double>(p, n_atoms, (const double*)pos, (const double*)q, (double*)E, (double*)phi,
+                                  (double*)F, accumulate, st);
+  return execute_real_t<float>(p, n_atoms, (const float*)pos, (const float*)q, (double*)E, (float*)phi, (float*)F,
+                               accumulate, st);
+}
+
+int pswf_lr_eval_real(const pswf_lr_plan* p, int pe, int n, const double* r, double* L, double* dL) {
+  if (!p || n < 0 || (n > 0 && (!r || !L))) return PSWF_LR_ERR_INVALID_ARG;
+  int slot = -1;
+  for (size_t s = 0; s < p->distinct_p.size(); ++s)
+    if (p->distinct_p[s] == pe) slot = (int)s;
+  if (slot < 0) return PSWF_LR_ERR_UNSUPPORTED_EXPONENT;
+  const int deg = p->rt.degree, panels = p->rt.panels;
+  const double pre = std::pow(p->r_c, -(double)pe);
+  for (int i = 0; i < n; ++i) {
+    const double x = r[i] / p->r_c;
+    if (!(x > 0) || x >= 1) {
+      L[i] = 0;
+      if (dL) dL[i] = 0;
+      continue;
+    }
+    int j = std::min((int)(x * panels), panels - 1);
+    const double xi = 2 * (x * panels - j) - 1;
+    const double* cf = &p->rt.coef[((size_t)slot * panels + j) * (deg + 1)];
+    const double* df = &p->rt.dcoef[((size_t)slot * panels + j) * deg];
+    double N = cf[deg], dN = df[deg - 1];
+    for (int m = deg - 1; m >= 0; --m) N = N * xi + cf[m];
+    for (int m = deg - 2; m >= 0; --m) dN = dN * xi + df[m];
+    const double ip = std::pow(x, -(double)pe);
+    L[i] = pre * N * ip;
+    if (dL) dL[i] = pre / p->r_c * (dN * ip - pe * N * ip / x);
+  }
+  return 0;
+}
+
+int pswf_lr_self_coefficient(const pswf_lr_plan* p, int pe, double* S0) {
+  if (!p || !S0) return PSWF_LR_ERR_INVALID_ARG;
+  for (size_t s = 0; s < p->distinct_p.size(); ++s)
+    if (p->distinct_p[s] == pe) {
+      *S0 = p->rt.S0[s];
+      return 0;
+    }
+  return PSWF_LR_ERR_UNSUPPORTED_EXPONENT;
 }
 
 int pswf_lr_channel_energies(pswf_lr_plan* p, void* E_channels, void* stream) {
@@ -616,7 +722,7 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   free_atoms(p);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
                   p->d_grid,  p->d_spec,    p->d_count,    p->d_scan_state, p->d_Ech,      p->d_Etot,
-                  p->d_gridi};
+                  p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   if (p->have_fft) {

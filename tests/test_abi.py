@@ -124,6 +124,28 @@ def test_kernel_tables_match_oracle_theorem1(precision, tol):
         assert got[-1] == 0.0 and got[-2] == 0.0
 
 
+# f64 bound: the oracle forms S_p from 1 - phi + ... (cancellation ~1e-10 of r^-p at small r for p = 6)
+@pytest.mark.parametrize("precision,tol", [("f32", 3e-7), ("f64", 5e-10)])
+def test_real_space_tables_match_oracle_props_2_to_7(precision, tol):
+    """L_{p,r_c}(r), dL/dr and S_p(0) from the library's numerator polynomials N_p (host tables of the
+    real-space row) vs the oracle's closed forms (SI Props. 2-7, (S67)); dL/dr vs central differences."""
+    p = binding.Plan([31.0] * 3, [32] * 3, 6, 12.024, [1, 2, 3, 4, 5, 6], precision=precision,
+                     host_only=True)
+    i = p.info()
+    moll = Mollifier(i["c"], i["r_c"])
+    r = np.concatenate([np.linspace(0.05, 0.999, 400) * i["r_c"], [i["r_c"] * 1.0001, 3 * i["r_c"]]])
+    for pe in range(1, 7):
+        L, dL = p.eval_real(pe, r)
+        ref = moll.L_phys(pe, r)
+        # error relative to r^-p (the numerator N_p is O(1), the singular factor is explicit)
+        assert np.max(np.abs(L - ref)[:-2] * r[:-2] ** pe) < tol, pe
+        assert L[-1] == 0.0 and L[-2] == 0.0
+        h = 1e-5
+        fd = (moll.L_phys(pe, r[:-3] + h) - moll.L_phys(pe, r[:-3] - h)) / (2 * h)
+        assert np.max(np.abs(dL[:-3] - fd) * r[:-3] ** (pe + 1)) < max(tol, 2e-8) * 40, pe
+        assert abs(p.self_coefficient(pe) - moll.S_zero(pe)) < 1e-9 * abs(moll.S_zero(pe)), pe
+
+
 def test_workloads_are_seeded_and_shaped():
     from paper_2606_06617_b200 import workloads
     a, b = workloads.make(2), workloads.make(2)

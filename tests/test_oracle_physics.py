@@ -195,3 +195,35 @@ def test_mode_set_limits():
     # |m| < c L / (2 pi r_c) = 4.0035: lattice points with 0 < |m|^2 <= 16 (Gauss sphere count
     # 1+6+12+8+6+24+24+0+12+30+24+24+8+24+48+0+6 = 257 including the origin)
     assert len(m) == 256
+
+
+def test_real_space_parts_energy_forces_potentials():
+    """scaffold.real_space_parts (parity target of pswf_lr_execute_real): its energy equals the pinned
+    real_space_complement - self_energy, F = -dE/dr and phi = dE/dq by central differences of E."""
+    from oracle.scaffold import real_space_parts, real_space_complement, self_energy
+    from oracle.kernels import Mollifier
+    rng = np.random.default_rng(11)
+    box = np.array([9.0, 10.0, 11.0])
+    N = 14
+    pos = rng.uniform(0, 1, (N, 3)) * box
+    q = rng.normal(0, 1, (3, N))
+    ex = [1, 4, 6]
+    c, r_c = 12.024, 4.2
+    E, phi, F = real_space_parts(pos, q, ex, box, c, r_c)
+    moll = Mollifier(c, r_c)
+    E_ref = sum(real_space_complement(pos, q[a], ex[a], box, moll) - self_energy(q[a], ex[a], moll)
+                for a in range(3))
+    assert abs(E - E_ref) < 1e-12 * abs(E_ref)
+    h = 1e-5
+    for i, d in [(0, 0), (5, 2), (9, 1)]:
+        pp, pm = pos.copy(), pos.copy()
+        pp[i, d] += h
+        pm[i, d] -= h
+        fd = -(real_space_parts(pp, q, ex, box, c, r_c)[0] - real_space_parts(pm, q, ex, box, c, r_c)[0]) / (2 * h)
+        assert abs(fd - F[i, d]) < 1e-6 * np.abs(F).max()
+    for a, i in [(0, 3), (2, 7)]:
+        qp, qm = q.copy(), q.copy()
+        qp[a, i] += h
+        qm[a, i] -= h
+        fd = (real_space_parts(pos, qp, ex, box, c, r_c)[0] - real_space_parts(pos, qm, ex, box, c, r_c)[0]) / (2 * h)
+        assert abs(fd - phi[a, i]) < 1e-8 * np.abs(phi).max()
