@@ -263,6 +263,18 @@ def run_ours(args):
     total_s_max, atoms_all = reduce_times(total_s, N, dev)
     value = atoms_all * args.steps / total_s_max
 
+    # ---- optional: the real-space row (not part of the metric) ----
+    real_ms = None
+    if args.with_real:
+        plan.execute_real(N, pos_d[0], q_d, E_d, phi_d, F_d, True, sp)
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record(stream)
+        plan.execute_real(N, pos_d[0], q_d, E_d, phi_d, F_d, True, sp)
+        r1.record(stream)
+        torch.cuda.synchronize()
+        real_ms = r0.elapsed_time(r1)
+
     # ---- end to end through the C ABI with host buffers (H2D + compute + D2H every step) ----
     E_h = torch.zeros(1, dtype=torch.float64).pin_memory()
     phi_h = torch.empty((C, N), dtype=dt_t).pin_memory()
@@ -343,6 +355,8 @@ def run_ours(args):
                      "hbm_frac": pipeline_bytes / (ms_per_step * 1e-3) / 1e9 / peak_gbs,
                      "hbm_peak_gbs": peak_gbs, "hbm_peak_source": peak_src},
         "cpu_baseline": cb,
+        "real_space": None if real_ms is None else {"ms": real_ms, "r_c": info["r_c"],
+                                                    "note": "pswf_lr_execute_real: sort + pair kernel, one evaluation"},
         "energy_last_step": E_last,
     }
     print(json.dumps(line))
@@ -362,6 +376,9 @@ def main():
     ap.add_argument("--atoms", type=int, default=None, help="override the atom count (same box and grid)")
     ap.add_argument("--kernel-path", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--with-real", action="store_true",
+                    help="also time pswf_lr_execute_real (real-space complement + self term, SURVEY 8(f) row 1); "
+                         "reported under 'real_space', the metric is unchanged")
     ap.add_argument("--ref-atoms", type=int, default=4000, help="atoms per reference step (bounded sample)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

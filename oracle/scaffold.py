@@ -35,12 +35,14 @@ def real_space_complement(pos, q, p, box, moll):
     return float(E)
 
 
-def real_space_parts(pos, q, exponents, box, c, r_c, fd=1e-6):
+def real_space_parts(pos, q, exponents, box, c, r_c, fd=1e-6, subset=None):
     """Real-space complement minus self term for several channels: returns (E, phi[C][N], F[N][3]) with
         E   = sum_a [ 1/2 sum_n sum_{i,j}' q_i^a q_j^a L_{p_a,r_c}(|r_ij + n.L|) - E_self^a ]   (S64)-(S66)
         phi = dE/dq_i^a = sum_j q_j^a L(r_ij) - S_p(0) q_i^a / r_c^p
         F_i = -dE/dr_i, with dL/dr by central differences of L (step fd): the scaffold has no
-              closed-form derivative of its own, and none is needed at 1e-8 relative accuracy."""
+              closed-form derivative of its own, and none is needed at 1e-8 relative accuracy.
+    With `subset` (atom indices) only those atoms' phi and F are computed (rows of the pair sum against
+    ALL atoms) and E is None: the sampled check of large systems."""
     pos = np.asarray(pos, dtype=np.float64)
     q = np.atleast_2d(np.asarray(q, dtype=np.float64))
     box = np.asarray(box, dtype=np.float64)
@@ -49,7 +51,8 @@ def real_space_parts(pos, q, exponents, box, c, r_c, fd=1e-6):
     phi = np.zeros_like(q)
     F = np.zeros((N, 3))
     nmax = np.ceil(r_c / box).astype(int)
-    d0 = pos[None, :, :] - pos[:, None, :]          # d0[i, j] = r_j - r_i
+    rows = np.arange(N) if subset is None else np.asarray(subset)
+    d0 = pos[None, :, :] - pos[rows, None, :]       # d0[i, j] = r_j - r_rows[i]
     for n in itertools.product(*[range(-k, k + 1) for k in nmax]):
         d = d0 + np.asarray(n) * box
         r = np.sqrt((d ** 2).sum(-1))
@@ -58,15 +61,18 @@ def real_space_parts(pos, q, exponents, box, c, r_c, fd=1e-6):
             continue
         ii, jj = np.nonzero(mask)
         rr = r[ii, jj]
+        ri = rows[ii]
         for a, p in enumerate(exponents):
             L = moll.L_phys(p, rr)
             dL = (moll.L_phys(p, np.minimum(rr + fd, r_c * (1 - 1e-15))) - moll.L_phys(p, rr - fd)) / \
                  (np.minimum(rr + fd, r_c * (1 - 1e-15)) - (rr - fd))
-            np.add.at(phi[a], ii, q[a, jj] * L)
-            f = (q[a, ii] * q[a, jj] * dL / rr)[:, None] * d[ii, jj]      # F_i = + qq L'(r) (r_j - r_i)/r
-            np.add.at(F, ii, f)
+            np.add.at(phi[a], ri, q[a, jj] * L)
+            f = (q[a, ri] * q[a, jj] * dL / rr)[:, None] * d[ii, jj]      # F_i = + qq L'(r) (r_j - r_i)/r
+            np.add.at(F, ri, f)
     for a, p in enumerate(exponents):
         phi[a] -= moll.S_zero(p) * q[a] / r_c ** p
+    if subset is not None:
+        return None, phi[:, rows], F[rows]
     E = 0.5 * float(np.sum(q * phi))
     return E, phi, F
 

@@ -13,7 +13,7 @@ from . import binding
 
 class _LongRangeEnergy(torch.autograd.Function):
     @staticmethod
-    def forward(ctx, pos, q, plan):
+    def forward(ctx, pos, q, plan, full):
         dt = torch.float64 if plan.precision == binding.PSWF_LR_F64 else torch.float32
         if not (pos.is_cuda and q.is_cuda):
             raise RuntimeError("pswf_lr: tensors must live on a CUDA device (there is no CPU fallback)")
@@ -26,7 +26,10 @@ class _LongRangeEnergy(torch.autograd.Function):
         E = torch.empty(1, dtype=torch.float64, device=pos.device)
         phi = torch.empty((C, n), dtype=dt, device=pos.device)
         F = torch.empty((n, 3), dtype=dt, device=pos.device)
-        plan.execute(n, pos_c, q_c, E, phi, F, torch.cuda.current_stream(pos.device).cuda_stream)
+        st = torch.cuda.current_stream(pos.device).cuda_stream
+        plan.execute(n, pos_c, q_c, E, phi, F, st)
+        if full:   # + real-space complement - self term: the complete inverse-power energy (S65)
+            plan.execute_real(n, pos_c, q_c, E, phi, F, accumulate=True, stream=st)
         ctx.save_for_backward(phi, F)
         ctx.in_dtypes = (pos.dtype, q.dtype)
         return E[0]
@@ -41,10 +44,12 @@ class _LongRangeEnergy(torch.autograd.Function):
             gpos = gpos.to(ctx.in_dtypes[0])
         if gq is not None:
             gq = gq.to(ctx.in_dtypes[1])
-        return gpos, gq, None
+        return gpos, gq, None, None
 
 
-def long_range_energy(plan, pos, q):
+def long_range_energy(plan, pos, q, full=False):
     """E_lr(pos, q) as a differentiable 0-dim float64 tensor.  ``plan`` is a ``binding.Plan``;
-    ``pos`` [N,3] and ``q`` [n_channels,N] are CUDA tensors.  d/dpos = -F, d/dq = phi."""
-    return _LongRangeEnergy.apply(pos, q, plan)
+    ``pos`` [N,3] and ``q`` [n_channels,N] are CUDA tensors.  d/dpos = -F, d/dq = phi.
+    ``full=False``: the reciprocal-space part (the hot path); ``full=True``: reciprocal + real-space
+    complement - self term, i.e. the complete periodic inverse-power energy (S65)."""
+    return _LongRangeEnergy.apply(pos, q, plan, bool(full))

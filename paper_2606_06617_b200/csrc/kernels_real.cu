@@ -37,16 +37,25 @@ __global__ void __launch_bounds__(256) k_sorted_pos(int n, int cap, const T* __r
   }
 }
 
-template <class T, int CT>   // CT = compile-time channel capacity (register arrays)
+template <class T, int CT, int LPA>   // CT = channel capacity (register arrays); LPA = lanes per atom, 32 or 1
 __global__ void __launch_bounds__(128) k_real_pairs(int n, int C, int cap, RealGeom<T> g, RealParams<T> P,
                                                      const int* __restrict__ start, const int* __restrict__ si0,
                                                      const T* __restrict__ spos, const T* __restrict__ sq,
                                                      const int* __restrict__ perm, double* __restrict__ Eacc,
                                                      T* __restrict__ phi, T* __restrict__ F, int accumulate) {
   __shared__ double s_E;
+  extern __shared__ __align__(16) unsigned char s_raw[];   // numerator tables: [slot][panel][degree+1] | [..][degree]
+  T* s_cf = reinterpret_cast<T*>(s_raw);
+  T* s_df = s_cf + P.nslots * P.panels * (P.degree + 1);
+  for (int t = threadIdx.x; t < P.nslots * P.panels * (P.degree + 1); t += blockDim.x) s_cf[t] = P.coef[t];
+  for (int t = threadIdx.x; t < P.nslots * P.panels * P.degree; t += blockDim.x) s_df[t] = P.dcoef[t];
   if (threadIdx.x == 0) s_E = 0.0;
   __syncthreads();
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  // LPA = 32 (small systems: more parallelism): one WARP per sorted atom j, the lanes stride over each
+  // contiguous run of neighbour candidates and the warp reduces their contributions at the end;
+  // LPA = 1 (large systems, short runs): one thread per atom
+  const int lane = LPA == 32 ? (threadIdx.x & 31) : 0;
+  const int j = LPA == 32 ? blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5) : blockIdx.x * blockDim.x + threadIdx.x;
   double e_thread = 0.0;
   if (j < n) {
     const int Mx = g.M[0], My = g.M[1], Mz = g.M[2];
@@ -75,7 +84,7 @@ __global__ void __launch_bounds__(128) k_real_pairs(int n, int C, int cap, RealG
         if (z1 > Mz) { runs[nr][0] = row[0]; runs[nr][1] = row[z1 - Mz]; ++nr; z1 = Mz; }
         runs[nr][0] = row[z0]; runs[nr][1] = row[z1]; ++nr;
         for (int r = 0; r < nr; ++r)
-          for (int k = runs[r][0]; k < runs[r][1]; ++k) {
+          for (int k = runs[r][0] + lane; k < runs[r][1]; k += LPA) {
             if (k == j) continue;
             T ddx = spos[k] - xj, ddy = spos[(size_t)cap + k] - yj, ddz = spos[2 * (size_t)cap + k] - zj;
             ddx -= g.L[0] * rint(ddx * (T)g.invL[0]);   // minimum image (r_c < L/2)
@@ -92,8 +101,8 @@ __global__ void __launch_bounds__(128) k_real_pairs(int n, int C, int cap, RealG
 #pragma unroll
             for (int s = 0; s < 6; ++s) {
               if (s >= P.nslots) break;
-              const T* cf = P.coef + ((size_t)s * P.panels + pj) * (P.degree + 1);
-              const T* df = P.dcoef + ((size_t)s * P.panels + pj) * P.degree;
+              const T* cf = s_cf + (s * P.panels + pj) * (P.degree + 1);
+              const T* df = s_df + (s * P.panels + pj) * P.degree;
               T N = cf[P.degree], dN = df[P.degree - 1];
               for (int m = P.degree - 1; m >= 1; --m) { N = fma(N, xi, cf[m]); dN = fma(dN, xi, df[m - 1]); }
               N = fma(N, xi, cf[0]);
@@ -119,22 +128,29 @@ __global__ void __launch_bounds__(128) k_real_pairs(int n, int C, int cap, RealG
           }
       }
     }
-    const int dst = perm[j];
+    if (LPA == 32) {
+      fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
 #pragma unroll
-    for (int a = 0; a < CT; ++a) {
-      if (a < C) {
-        const T pa = ph[a] - P.self_pre[a] * qj[a];   // self term: phi_self = -S_p(0) q / r_c^p
-        e_thread += 0.5 * (double)qj[a] * (double)pa;
-        if (phi) {
-          T* o = phi + (size_t)a * n + dst;
-          *o = accumulate ? *o + pa : pa;
+      for (int a = 0; a < CT; ++a) ph[a] = warp_sum(ph[a]);
+    }
+    if (lane == 0) {
+      const int dst = perm[j];
+#pragma unroll
+      for (int a = 0; a < CT; ++a) {
+        if (a < C) {
+          const T pa = ph[a] - P.self_pre[a] * qj[a];   // self term: phi_self = -S_p(0) q / r_c^p
+          e_thread += 0.5 * (double)qj[a] * (double)pa;
+          if (phi) {
+            T* o = phi + (size_t)a * n + dst;
+            *o = accumulate ? *o + pa : pa;
+          }
         }
       }
-    }
-    if (F) {
-      T* o = F + 3 * (size_t)dst;
-      if (accumulate) { o[0] += fx; o[1] += fy; o[2] += fz; }
-      else { o[0] = fx; o[1] = fy; o[2] = fz; }
+      if (F) {
+        T* o = F + 3 * (size_t)dst;
+        if (accumulate) { o[0] += fx; o[1] += fy; o[2] += fz; }
+        else { o[0] = fx; o[1] = fy; o[2] = fz; }
+      }
     }
   }
   e_thread = warp_sum(e_thread);
@@ -155,14 +171,20 @@ void launch_real_space(pswf_lr_plan* p, int n, const T* pos, const RealGeom<T>& 
   cudaMemsetAsync(p->d_Ereal, 0, sizeof(double), st);
   if (n > 0) {
     k_sorted_pos<T><<<(n + 255) / 256, 256, 0, st>>>(n, p->cap_atoms, pos, p->d_perm, g, (T*)p->d_spos);
-#define PSWF_REAL(CTV)                                                                                          \
-  k_real_pairs<T, CTV><<<(n + 127) / 128, 128, 0, st>>>(n, p->C, p->cap_atoms, g, P, p->d_count, p->d_si0,       \
-                                                         (const T*)p->d_spos, (const T*)p->d_sq, p->d_perm,       \
-                                                         p->d_Ereal, phi, F, accumulate)
-    if (p->C <= 4) PSWF_REAL(4);
-    else if (p->C <= 8) PSWF_REAL(8);
-    else PSWF_REAL(kMaxChannels);
+    const size_t tb = sizeof(T) * (size_t)P.nslots * P.panels * (2 * P.degree + 1);   // <= 6 * 32 * 49 * 8 = 75 KB
+#define PSWF_REAL_L(CTV, LPAV, NB)                                                                              \
+  cudaFuncSetAttribute(k_real_pairs<T, CTV, LPAV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tb);       \
+  k_real_pairs<T, CTV, LPAV><<<NB, 128, tb, st>>>(n, p->C, p->cap_atoms, g, P, p->d_count, p->d_si0,            \
+                                                  (const T*)p->d_spos, (const T*)p->d_sq, p->d_perm,            \
+                                                  p->d_Ereal, phi, F, accumulate)
+#define PSWF_REAL(CTV)                                        \
+  if (n < 65536) { PSWF_REAL_L(CTV, 32, (n + 3) / 4); }       \
+  else { PSWF_REAL_L(CTV, 1, (n + 127) / 128); }
+    if (p->C <= 4) { PSWF_REAL(4); }
+    else if (p->C <= 8) { PSWF_REAL(8); }
+    else { PSWF_REAL(kMaxChannels); }
 #undef PSWF_REAL
+#undef PSWF_REAL_L
   }
   if (E) k_real_finalize<<<1, 32, 0, st>>>(p->d_Ereal, E, accumulate);
 }

@@ -417,6 +417,26 @@ def test_real_space_complement_vs_scaffold(precision, tol):
     plan.destroy()
 
 
+def test_real_space_large_system_sampled_fp32():
+    """The thread-per-atom variant of the pair kernel (n >= 65536): 70,000 atoms at 0.1 A^-3, sampled
+    atoms against the scaffold's rows over ALL atoms (fp32 gates)."""
+    from oracle.scaffold import real_space_parts
+    rng = np.random.default_rng(31)
+    N, L = 70000, 88.8
+    pos = (rng.uniform(0, L, (N, 3))).astype(np.float32).astype(np.float64)
+    q = rng.normal(0, 0.5, (2, N)).astype(np.float32).astype(np.float64)
+    wl = dict(pos=pos, q=q, exponents=[1, 6], box=[L] * 3, grid=[48] * 3, w=8, c=12.024, precision="f32")
+    plan = make_plan(wl)
+    r_c = plan.info()["r_c"]
+    E, phi, F = _run_real(wl, plan)
+    sub = rng.choice(N, 40, replace=False)
+    _, phi_ref, F_ref = real_space_parts(pos, q, wl["exponents"], wl["box"], wl["c"], r_c, subset=sub)
+    print("real large: eps_phi=%.2e eps_F=%.2e" % (rel(phi[:, sub], phi_ref), rel(F[sub], F_ref)))
+    assert rel(phi[:, sub], phi_ref) <= 2e-5
+    assert rel(F[sub], F_ref) <= 1e-4
+    plan.destroy()
+
+
 def test_full_decomposition_on_gpu_madelung():
     """Reciprocal path + real-space complement + self term = the plain inverse-power energy (S65):
     NaCl rock salt (8 ions, a = 2, nearest-neighbour distance 1) gives the Madelung constant
@@ -433,6 +453,14 @@ def test_full_decomposition_on_gpu_madelung():
     print("Madelung from the GPU: %.10f" % madelung)
     assert abs(madelung - 1.7475645946) < 2e-9
     assert np.abs(F).max() < 1e-8         # a perfect lattice is force-free
+    # the same through the autograd wrapper
+    from paper_2606_06617_b200.autograd import long_range_energy
+    dev = torch.device("cuda:0")
+    tp = torch.tensor(pos, dtype=torch.float64, device=dev, requires_grad=True)
+    tq = torch.tensor(q, dtype=torch.float64, device=dev)
+    Et = long_range_energy(plan, tp, tq, full=True)
+    Et.backward()
+    assert abs(Et.item() - E) < 1e-12 * abs(E) and tp.grad.abs().max().item() < 1e-8
     plan.destroy()
 
 
