@@ -73,11 +73,17 @@ __global__ void __launch_bounds__(128) k_real_pairs(int n, int C, int cap, RealG
     const bool allz = 2 * g.R[2] + 1 >= Mz;
     for (int dx = 0; dx < nx; ++dx) {
       const int ix = wrap_index(x0 + dx, Mx);
+      // prune rows and z ranges that cannot reach r_c: cells k offsets apart are at least (k - 1) h apart
+      const T ax = nx == Mx ? (T)0 : (T)max(abs(dx - g.R[0]) - 1, 0) * g.h[0];
       for (int dy = 0; dy < ny; ++dy) {
         const int iy = wrap_index(y0 + dy, My);
+        const T ay = ny == My ? (T)0 : (T)max(abs(dy - g.R[1]) - 1, 0) * g.h[1];
+        const T rem2 = rc2 - ax * ax - ay * ay;
+        if (rem2 <= (T)0) continue;
+        const int Rz = min(g.R[2], (int)(sqrt(rem2) * g.inv_hz) + 1);
         const int* row = start + ((size_t)ix * My + iy) * Mz;
-        // cells cz - R .. cz + R (mod Mz): one run, or two when the range wraps
-        int z0 = allz ? 0 : cz - g.R[2], z1 = allz ? Mz : cz + g.R[2] + 1;   // [z0, z1)
+        // cells cz - Rz .. cz + Rz (mod Mz): one run, or two when the range wraps
+        int z0 = allz ? 0 : cz - Rz, z1 = allz ? Mz : cz + Rz + 1;   // [z0, z1)
         int runs[2][2];
         int nr = 0;
         if (z0 < 0) { runs[nr][0] = row[z0 + Mz]; runs[nr][1] = row[Mz]; ++nr; z0 = 0; }

@@ -64,6 +64,8 @@ struct RealGeom {
   int R[3];            // cell search radius per dimension: floor(r_c / h_d) + 1
   double invL[3];
   T L[3];
+  T h[3];              // grid spacing (cell size of the sort)
+  T inv_hz;
 };
 template <class T>
 struct RealParams {

@@ -232,7 +232,9 @@ int execute_real_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, 
     rg.R[d] = p->real_R[d];
     rg.invL[d] = 1.0 / p->L[d];
     rg.L[d] = (T)p->L[d];
+    rg.h[d] = (T)p->h[d];
   }
+  rg.inv_hz = (T)(1.0 / p->h[2]);
   P.C = p->C;
   P.nslots = (int)p->distinct_p.size();
   P.panels = p->rt.panels;
