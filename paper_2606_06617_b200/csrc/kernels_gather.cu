@@ -380,33 +380,50 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
     }
     if (rem == 0u) break;
     // advance to the next non-empty cell nxt: the planes max(cur+8, nxt) .. nxt+7 replace the ones that
-    // left the window.  All loads of an advance are issued back to back, straight into their slot
-    // registers (Duff's device over the static slots): no per-plane dispatch, no register moves.
+    // left the window.  Slot k takes the plane p_k = nxt + ((k - nxt) & 7) if that plane is new.  The
+    // eight slot refills are PREDICATED loads in one straight-line block, straight into the slot
+    // registers: ptxas guards all refill loads with one scoreboard, so in the earlier jump-into-an-
+    // unrolled-sequence form every plane of an advance waited for the previous one's data (the
+    // decoded wait masks and 25% of the stall samples in profiles/r1e say so); here they are all in
+    // flight together.
     const int nxt = __ffs(rem) - 1;
-    int ps = max(cur + SW, nxt);          // first plane to load, relative to Z0
-    int cnt = nxt + SW - ps;              // 1 .. 8 planes
-    int zz = Z0 + ps;
-    while (zz >= Mz) zz -= Mz;
-    unsigned off = (unsigned)zz * plane;
-#define PSWF_SLOT(K)                         \
-  case K:                                    \
-    ldw(g0 + off, win[K][0]);                \
-    ldw(g1 + off, win[K][1]);                \
-    off += plane;                            \
-    if (off == wrap) off = 0u;
-    switch ((Z0 + ps) & 7) {
-      do {
-        PSWF_SLOT(0) if (--cnt == 0) break;
-        PSWF_SLOT(1) if (--cnt == 0) break;
-        PSWF_SLOT(2) if (--cnt == 0) break;
-        PSWF_SLOT(3) if (--cnt == 0) break;
-        PSWF_SLOT(4) if (--cnt == 0) break;
-        PSWF_SLOT(5) if (--cnt == 0) break;
-        PSWF_SLOT(6) if (--cnt == 0) break;
-        PSWF_SLOT(7)
-      } while (--cnt != 0);
-    }
+    {
+      const int an = Z0 + nxt, first_new = Z0 + max(cur + SW, nxt);
+      const int cnt = an + SW - first_new;      // 1 .. 8 new planes
+      if (cnt <= 2) {
+        // one or two planes (62% of the advances at 0.5 atoms per cell): jump to the first slot; the
+        // second plane, if any, is predicated in the same block
+        const int z = first_new >= Mz ? first_new - Mz : first_new;
+        const unsigned off = (unsigned)z * plane;
+        unsigned off2 = off + plane; if (off2 == wrap) off2 = 0u;
+        const bool two = cnt == 2;
+        switch (first_new & 7) {
+#define PSWF_SLOT(K)                                     \
+  case K:                                                \
+    ldw(g0 + off, win[K][0]);                            \
+    ldw(g1 + off, win[K][1]);                            \
+    if (two) {                                           \
+      ldw(g0 + off2, win[(K + 1) & 7][0]);               \
+      ldw(g1 + off2, win[(K + 1) & 7][1]);               \
+    }                                                    \
+    break;
+          PSWF_SLOT(0) PSWF_SLOT(1) PSWF_SLOT(2) PSWF_SLOT(3)
+          PSWF_SLOT(4) PSWF_SLOT(5) PSWF_SLOT(6) PSWF_SLOT(7)
 #undef PSWF_SLOT
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < SW; ++k) {
+          const int pk = an + ((k - an) & 7);
+          if (pk >= first_new) {
+            const int z = pk >= Mz ? pk - Mz : pk;
+            const unsigned off = (unsigned)z * plane;
+            ldw(g0 + off, win[k][0]);
+            ldw(g1 + off, win[k][1]);
+          }
+        }
+      }
+    }
     cur = nxt;
   }
   retire();
