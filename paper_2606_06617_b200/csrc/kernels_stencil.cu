@@ -242,8 +242,8 @@ __device__ __forceinline__ void walk_atoms(f32x2 (&acc)[SW / 2][2][CB], const ui
                                            const int oz) {
   // loop invariants pinned to registers (ptxas otherwise reloads the kernel parameters from the
   // constant bank inside the atom loop, a uniform-load latency per iteration)
-  int recf_r = recf, cb0_r = cb0;
-  asm volatile("" : "+r"(recf_r), "+r"(cb0_r));
+  // (a shuffle result cannot be rematerialised from the constant bank, an empty asm can)
+  const int recf_r = __shfl_sync(0xffffffffu, recf, 0), cb0_r = __shfl_sync(0xffffffffu, cb0, 0);
   int j = 0, jend = 0, ja = 0, jb = 0;
   int k = 0;                     // descriptors fetched so far
   uint2 nd = make_uint2(0u, 0u);
