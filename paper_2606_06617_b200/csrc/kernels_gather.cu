@@ -230,7 +230,10 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   int iy = sy + c_off;      if (iy >= My) iy -= My;
   int ix0 = sx + b0;        if (ix0 >= Mx) ix0 -= Mx;
   int ix1 = sx + b0 + 4;    if (ix1 >= Mx) ix1 -= Mx;
-  const unsigned plane = (unsigned)Mx * My, wrap = plane * (unsigned)Mz;
+  // loop invariants as shuffle results: ptxas cannot rematerialise those from the constant bank (it
+  // re-read Mx, My and cb0 with LDC in every advance / atom otherwise)
+  const unsigned plane = __shfl_sync(0xffffffffu, (unsigned)Mx * My, 0), wrap = plane * (unsigned)Mz;
+  const int cb0r = __shfl_sync(0xffffffffu, cb0, 0);
   const V* g0 = gridt + (size_t)ix0 * My + iy;
   const V* g1 = gridt + (size_t)ix1 * My + iy;
   // keep the two lane pointers in registers: left to itself ptxas re-derives them from the kernel
@@ -305,7 +308,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
         const float4 zb = *reinterpret_cast<const float4*>(r + 2 * SW + 4);
         const float4 da = *reinterpret_cast<const float4*>(dr + 2 * SW);
         const float4 db = *reinterpret_cast<const float4*>(dr + 2 * SW + 4);
-        const float4 q4 = *reinterpret_cast<const float4*>(r + 3 * SW + cb0);
+        const float4 q4 = *reinterpret_cast<const float4*>(r + 3 * SW + cb0r);
         const float wx0 = r[ox0], wx1 = r[ox1], wy = r[oy];
         const float dx0 = dr[ox0], dx1 = dr[ox1], dy = dr[oy];
         const float wz[SW] = {za.x, za.y, za.z, za.w, zb.x, zb.y, zb.z, zb.w};
