@@ -116,7 +116,7 @@ def measured_peaks():
 
 def profiled_traffic(kernel):
     """DRAM bytes per launch of a kernel from the committed ncu --set full capture (profiles/), or None."""
-    path = os.path.join(ROOT, "profiles", "r1e_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r1f_traffic.json")
     try:
         return int(json.load(open(path))["dram_bytes_per_launch"][kernel])
     except Exception:
@@ -311,7 +311,7 @@ def run_ours(args):
     roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": ach / alu_peak,
                 "traffic": profiled_traffic(dom) if (args.cfg == 4 and args.atoms is None and args.kernel_path == 0) else None,
-                "traffic_source": "profiles/r1e_ncu_full.md (dram__bytes_read+write of one launch, config 4)",
+                "traffic_source": "profiles/r1f_ncu_full.md (dram__bytes_read+write of one launch, config 4)",
                 "alg_flops": flops_alg[dom], "alg_bytes": bytes_alg[dom],
                 "peak_source": "148 SM x 128 FMA/clk x 2 x %.0f MHz (DESIGN.md §6)" % sm_max,
                 "hbm_achieved_gbs": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9,
