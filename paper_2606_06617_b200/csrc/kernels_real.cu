@@ -9,7 +9,7 @@
 //
 // It reuses the reciprocal path's cell sort: atoms are ordered by stencil cell (z fastest), so the
 // neighbours of an atom within r_c are, for every (dx, dy) cell-row offset, one contiguous run of
-// the sorted arrays (two when the z range wraps).  One thread per sorted atom, all channels; each
+// the sorted arrays (two when the z range wraps).  One warp per sorted atom, all channels; each
 // distinct exponent's polynomial is evaluated once per pair and shared by its channels.
 // Requirement (host-checked): r_c < L_d / 2 (minimum image).  Cell search radius
 // R_d = floor(r_c / h_d) + 1; a dimension with 2 R_d + 1 >= M_d is searched whole.
@@ -37,25 +37,30 @@ __global__ void __launch_bounds__(256) k_sorted_pos(int n, int cap, const T* __r
   }
 }
 
-template <class T, int CT, int LPA>   // CT = channel capacity (register arrays); LPA = lanes per atom, 32 or 1
-__global__ void __launch_bounds__(128) k_real_pairs(int n, int C, int cap, RealGeom<T> g, RealParams<T> P,
-                                                     const int* __restrict__ start, const int* __restrict__ si0,
-                                                     const T* __restrict__ spos, const T* __restrict__ sq,
-                                                     const int* __restrict__ perm, double* __restrict__ Eacc,
-                                                     T* __restrict__ phi, T* __restrict__ F, int accumulate) {
+// One warp per sorted atom, lanes <-> candidate cell rows, accepted pairs COMPACTED.
+// The (dx, dy) cell rows around the atom are dealt to the lanes 32 at a time; every lane tests the
+// atoms of its row's z run against r_c (a cheap step at full lane occupancy), accepted neighbours go
+// to a per-warp queue in shared memory (ballot + popc), and whenever 32 are queued all lanes evaluate
+// one pair each -- the polynomial work runs with full warps instead of the ~38% of the lanes that a
+// test-and-evaluate loop keeps busy.
+template <class T, int CT>
+__global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, RealGeom<T> g, RealParams<T> P,
+                                                       const int* __restrict__ start, const int* __restrict__ si0,
+                                                       const T* __restrict__ spos, const T* __restrict__ sq,
+                                                       const int* __restrict__ perm, double* __restrict__ Eacc,
+                                                       T* __restrict__ phi, T* __restrict__ F, int accumulate) {
   __shared__ double s_E;
-  extern __shared__ __align__(16) unsigned char s_raw[];   // numerator tables: [slot][panel][degree+1] | [..][degree]
+  __shared__ int s_qk[4][64];        // queue of accepted neighbour indices, one ring per warp
+  __shared__ T s_qd[4][64][4];       // their minimum-image displacement and r^2
+  extern __shared__ __align__(16) unsigned char s_raw[];
   T* s_cf = reinterpret_cast<T*>(s_raw);
   T* s_df = s_cf + P.nslots * P.panels * (P.degree + 1);
   for (int t = threadIdx.x; t < P.nslots * P.panels * (P.degree + 1); t += blockDim.x) s_cf[t] = P.coef[t];
   for (int t = threadIdx.x; t < P.nslots * P.panels * P.degree; t += blockDim.x) s_df[t] = P.dcoef[t];
   if (threadIdx.x == 0) s_E = 0.0;
   __syncthreads();
-  // LPA = 32 (small systems: more parallelism): one WARP per sorted atom j, the lanes stride over each
-  // contiguous run of neighbour candidates and the warp reduces their contributions at the end;
-  // LPA = 1 (large systems, short runs): one thread per atom
-  const int lane = LPA == 32 ? (threadIdx.x & 31) : 0;
-  const int j = LPA == 32 ? blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5) : blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int j = blockIdx.x * 4 + wid;
   double e_thread = 0.0;
   if (j < n) {
     const int Mx = g.M[0], My = g.M[1], Mz = g.M[2];
@@ -67,84 +72,116 @@ __global__ void __launch_bounds__(128) k_real_pairs(int n, int C, int cap, RealG
     for (int a = 0; a < CT; ++a) { qj[a] = a < C ? sq[(size_t)a * cap + j] : (T)0; ph[a] = (T)0; }
     T fx = 0, fy = 0, fz = 0;
     const T rc2 = P.r_c * P.r_c;
-    // cells within R_d of the atom's own, every cell once: when 2 R_d + 1 >= M_d the whole dimension
     const int nx = min(2 * g.R[0] + 1, Mx), ny = min(2 * g.R[1] + 1, My);
     const int x0 = nx == Mx ? 0 : cx - g.R[0], y0 = ny == My ? 0 : cy - g.R[1];
     const bool allz = 2 * g.R[2] + 1 >= Mz;
-    for (int dx = 0; dx < nx; ++dx) {
-      const int ix = wrap_index(x0 + dx, Mx);
-      // prune rows and z ranges that cannot reach r_c: cells k offsets apart are at least (k - 1) h apart
-      const T ax = nx == Mx ? (T)0 : (T)max(abs(dx - g.R[0]) - 1, 0) * g.h[0];
-      for (int dy = 0; dy < ny; ++dy) {
-        const int iy = wrap_index(y0 + dy, My);
+    int qhead = 0, qcount = 0;   // warp-uniform
+    int* qk = s_qk[wid];
+    T (*qd)[4] = s_qd[wid];
+
+    // one accepted pair per lane: polynomial evaluation and accumulation
+    auto evaluate = [&](int k, T ddx, T ddy, T ddz, T r2) {
+      const T rr = sqrt(r2);
+      const T x = rr * P.inv_rc;
+      const int pj = min((int)(x * (T)P.panels), P.panels - 1);
+      const T xi = (T)2 * (x * (T)P.panels - (T)pj) - (T)1;
+      const T invx = (T)1 / x;
+      T Lval[6], dL[6];
+#pragma unroll
+      for (int s = 0; s < 6; ++s) {
+        if (s >= P.nslots) break;
+        const T* cf = s_cf + (s * P.panels + pj) * (P.degree + 1);
+        const T* df = s_df + (s * P.panels + pj) * P.degree;
+        T N = cf[P.degree], dN = df[P.degree - 1];
+        for (int m = P.degree - 1; m >= 1; --m) { N = fma(N, xi, cf[m]); dN = fma(dN, xi, df[m - 1]); }
+        N = fma(N, xi, cf[0]);
+        T ip = invx;
+        for (int e = 1; e < P.slot_p[s]; ++e) ip *= invx;
+        Lval[s] = P.slot_pre[s] * N * ip;
+        dL[s] = P.slot_pre[s] * P.inv_rc * (dN * ip - (T)P.slot_p[s] * N * ip * invx);
+      }
+      T fs = 0;
+#pragma unroll
+      for (int a = 0; a < CT; ++a) {
+        if (a < C) {
+          const T qk_ = sq[(size_t)a * cap + k];
+          const int s = P.chan_slot[a];
+          ph[a] = fma(qk_, Lval[s], ph[a]);
+          fs = fma(qj[a] * qk_, dL[s], fs);
+        }
+      }
+      const T sc = fs / rr;
+      fx = fma(sc, ddx, fx);
+      fy = fma(sc, ddy, fy);
+      fz = fma(sc, ddz, fz);
+    };
+    auto drain = [&](int m) {   // the first m (<= 32) queued pairs, one per lane
+      __syncwarp();
+      if (lane < m) {
+        const int e = (qhead + lane) & 63;
+        evaluate(qk[e], qd[e][0], qd[e][1], qd[e][2], qd[e][3]);
+      }
+      __syncwarp();
+      qhead = (qhead + m) & 63;
+      qcount -= m;
+    };
+
+    const int nrows = nx * ny;
+    for (int rb = 0; rb < nrows; rb += 32) {
+      // this lane's row and its (up to two) z runs
+      int k0 = 0, k1 = 0, k2 = 0, k3 = 0;
+      const int ri = rb + lane;
+      if (ri < nrows) {
+        const int dx = ri / ny, dy = ri - dx * ny;
+        const T ax = nx == Mx ? (T)0 : (T)max(abs(dx - g.R[0]) - 1, 0) * g.h[0];
         const T ay = ny == My ? (T)0 : (T)max(abs(dy - g.R[1]) - 1, 0) * g.h[1];
         const T rem2 = rc2 - ax * ax - ay * ay;
-        if (rem2 <= (T)0) continue;
-        const int Rz = min(g.R[2], (int)(sqrt(rem2) * g.inv_hz) + 1);
-        const int* row = start + ((size_t)ix * My + iy) * Mz;
-        // cells cz - Rz .. cz + Rz (mod Mz): one run, or two when the range wraps
-        int z0 = allz ? 0 : cz - Rz, z1 = allz ? Mz : cz + Rz + 1;   // [z0, z1)
-        int runs[2][2];
-        int nr = 0;
-        if (z0 < 0) { runs[nr][0] = row[z0 + Mz]; runs[nr][1] = row[Mz]; ++nr; z0 = 0; }
-        if (z1 > Mz) { runs[nr][0] = row[0]; runs[nr][1] = row[z1 - Mz]; ++nr; z1 = Mz; }
-        runs[nr][0] = row[z0]; runs[nr][1] = row[z1]; ++nr;
-        for (int r = 0; r < nr; ++r)
-          for (int k = runs[r][0] + lane; k < runs[r][1]; k += LPA) {
-            if (k == j) continue;
-            T ddx = spos[k] - xj, ddy = spos[(size_t)cap + k] - yj, ddz = spos[2 * (size_t)cap + k] - zj;
-            ddx -= g.L[0] * rint(ddx * (T)g.invL[0]);   // minimum image (r_c < L/2)
+        if (rem2 > (T)0) {
+          const int Rz = min(g.R[2], (int)(sqrt(rem2) * g.inv_hz) + 1);
+          const int* row = start + ((size_t)wrap_index(x0 + dx, Mx) * My + wrap_index(y0 + dy, My)) * Mz;
+          int z0 = allz ? 0 : cz - Rz, z1 = allz ? Mz : cz + Rz + 1;
+          if (z0 < 0) { k2 = row[z0 + Mz]; k3 = row[Mz]; z0 = 0; }
+          if (z1 > Mz) { k2 = row[0]; k3 = row[z1 - Mz]; z1 = Mz; }
+          k0 = row[z0]; k1 = row[z1];
+        }
+      }
+      // lockstep over the run positions: test, compact, evaluate when a warp's worth is queued
+      for (int seg = 0; seg < 2; ++seg) {
+        int k = seg == 0 ? k0 : k2;
+        const int kend = seg == 0 ? k1 : k3;
+        while (__any_sync(0xffffffffu, k < kend)) {
+          bool acc = false;
+          T ddx = 0, ddy = 0, ddz = 0, r2 = 0;
+          if (k < kend && k != j) {
+            ddx = spos[k] - xj; ddy = spos[(size_t)cap + k] - yj; ddz = spos[2 * (size_t)cap + k] - zj;
+            ddx -= g.L[0] * rint(ddx * (T)g.invL[0]);
             ddy -= g.L[1] * rint(ddy * (T)g.invL[1]);
             ddz -= g.L[2] * rint(ddz * (T)g.invL[2]);
-            const T r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-            if (!(r2 < rc2) || r2 <= (T)0) continue;
-            const T rr = sqrt(r2);
-            const T x = rr * P.inv_rc;
-            int pj = min((int)(x * (T)P.panels), P.panels - 1);
-            const T xi = (T)2 * (x * (T)P.panels - (T)pj) - (T)1;
-            const T invx = (T)1 / x;
-            T Lval[6], dL[6];   // per distinct exponent: L(r) and dL/dr
-#pragma unroll
-            for (int s = 0; s < 6; ++s) {
-              if (s >= P.nslots) break;
-              const T* cf = s_cf + (s * P.panels + pj) * (P.degree + 1);
-              const T* df = s_df + (s * P.panels + pj) * P.degree;
-              T N = cf[P.degree], dN = df[P.degree - 1];
-              for (int m = P.degree - 1; m >= 1; --m) { N = fma(N, xi, cf[m]); dN = fma(dN, xi, df[m - 1]); }
-              N = fma(N, xi, cf[0]);
-              T ip = invx;                       // x^-p
-              for (int e = 1; e < P.slot_p[s]; ++e) ip *= invx;
-              Lval[s] = P.slot_pre[s] * N * ip;                                          // r_c^-p N x^-p
-              dL[s] = P.slot_pre[s] * P.inv_rc * (dN * ip - (T)P.slot_p[s] * N * ip * invx);
-            }
-            T fs = 0;   // sum_a q_j^a q_k^a dL/dr
-#pragma unroll
-            for (int a = 0; a < CT; ++a) {
-              if (a < C) {
-                const T qk = sq[(size_t)a * cap + k];
-                const int s = P.chan_slot[a];
-                ph[a] = fma(qk, Lval[s], ph[a]);
-                fs = fma(qj[a] * qk, dL[s], fs);
-              }
-            }
-            const T sc = fs / rr;   // F_j = + sum qq L'(r) (r_k - r_j) / r
-            fx = fma(sc, ddx, fx);
-            fy = fma(sc, ddy, fy);
-            fz = fma(sc, ddz, fz);
+            r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+            acc = r2 < rc2 && r2 > (T)0;
           }
+          const unsigned m = __ballot_sync(0xffffffffu, acc);
+          if (acc) {
+            const int e = (qhead + qcount + __popc(m & ((1u << lane) - 1u))) & 63;
+            qk[e] = k;
+            qd[e][0] = ddx; qd[e][1] = ddy; qd[e][2] = ddz; qd[e][3] = r2;
+          }
+          qcount += __popc(m);
+          if (qcount >= 32) drain(32);
+          ++k;
+        }
       }
     }
-    if (LPA == 32) {
-      fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
+    if (qcount > 0) drain(qcount);
+    fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
 #pragma unroll
-      for (int a = 0; a < CT; ++a) ph[a] = warp_sum(ph[a]);
-    }
+    for (int a = 0; a < CT; ++a) ph[a] = warp_sum(ph[a]);
     if (lane == 0) {
       const int dst = perm[j];
 #pragma unroll
       for (int a = 0; a < CT; ++a) {
         if (a < C) {
-          const T pa = ph[a] - P.self_pre[a] * qj[a];   // self term: phi_self = -S_p(0) q / r_c^p
+          const T pa = ph[a] - P.self_pre[a] * qj[a];
           e_thread += 0.5 * (double)qj[a] * (double)pa;
           if (phi) {
             T* o = phi + (size_t)a * n + dst;
@@ -178,19 +215,15 @@ void launch_real_space(pswf_lr_plan* p, int n, const T* pos, const RealGeom<T>& 
   if (n > 0) {
     k_sorted_pos<T><<<(n + 255) / 256, 256, 0, st>>>(n, p->cap_atoms, pos, p->d_perm, g, (T*)p->d_spos);
     const size_t tb = sizeof(T) * (size_t)P.nslots * P.panels * (2 * P.degree + 1);   // <= 6 * 32 * 49 * 8 = 75 KB
-#define PSWF_REAL_L(CTV, LPAV, NB)                                                                              \
-  cudaFuncSetAttribute(k_real_pairs<T, CTV, LPAV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tb);       \
-  k_real_pairs<T, CTV, LPAV><<<NB, 128, tb, st>>>(n, p->C, p->cap_atoms, g, P, p->d_count, p->d_si0,            \
-                                                  (const T*)p->d_spos, (const T*)p->d_sq, p->d_perm,            \
-                                                  p->d_Ereal, phi, F, accumulate)
-#define PSWF_REAL(CTV)                                        \
-  if (n < 65536) { PSWF_REAL_L(CTV, 32, (n + 3) / 4); }       \
-  else { PSWF_REAL_L(CTV, 1, (n + 127) / 128); }
+#define PSWF_REAL(CTV)                                                                                          \
+  cudaFuncSetAttribute(k_real_pairs_q<T, CTV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tb);            \
+  k_real_pairs_q<T, CTV><<<(n + 3) / 4, 128, tb, st>>>(n, p->C, p->cap_atoms, g, P, p->d_count, p->d_si0,        \
+                                                        (const T*)p->d_spos, (const T*)p->d_sq, p->d_perm,        \
+                                                        p->d_Ereal, phi, F, accumulate)
     if (p->C <= 4) { PSWF_REAL(4); }
     else if (p->C <= 8) { PSWF_REAL(8); }
     else { PSWF_REAL(kMaxChannels); }
 #undef PSWF_REAL
-#undef PSWF_REAL_L
   }
   if (E) k_real_finalize<<<1, 32, 0, st>>>(p->d_Ereal, E, accumulate);
 }
