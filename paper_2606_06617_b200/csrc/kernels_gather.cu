@@ -6,7 +6,7 @@
 //
 // Design: INPUT-STATIONARY IN REGISTERS, one warp per ROW of stencil cells, swept
 // along z -- the direction in which the cell-sorted atoms are contiguous.
-//  * a warp owns the cells (s_x, s_y, s_z), s_z in one 32-cell segment.  Their atoms are ONE
+//  * a warp owns the cell row (s_x, s_y, .) and walks it in 32-cell segments.  A segment's atoms are ONE
 //    contiguous run of the sorted arrays, so records and permutation entries stream through L1
 //    (prefetched a few atoms ahead) instead of costing an L2 round trip per atom (v2, profiles/r1b:
 //    a quarter of the kernel time was spent waiting for per-atom record loads);
@@ -174,6 +174,41 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   const int bx = bid % nbx;
   const int sx = bx * GBX + wid / GBY, sy = by * GBY + wid % GBY;
   if (sx >= Mx || sy >= My) return;
+  // lane -> 2 points of the 8 x 8 (x,y) footprint: y offset c = lane & 7, x offsets b and b + 4
+  const int c_off = lane & 7, b0 = lane >> 3;
+  int iy = sy + c_off;      if (iy >= My) iy -= My;
+  int ix0 = sx + b0;        if (ix0 >= Mx) ix0 -= Mx;
+  int ix1 = sx + b0 + 4;    if (ix1 >= Mx) ix1 -= Mx;
+  // loop invariants as shuffle results: ptxas cannot rematerialise those from the constant bank (it
+  // re-read Mx, My and cb0 with LDC in every advance / atom otherwise)
+  const unsigned plane = __shfl_sync(0xffffffffu, (unsigned)Mx * My, 0), wrap = plane * (unsigned)Mz;
+  const int cb0r = __shfl_sync(0xffffffffu, cb0, 0);
+  const V* g0 = gridt + (size_t)ix0 * My + iy;
+  const V* g1 = gridt + (size_t)ix1 * My + iy;
+  // keep the two lane pointers in registers: left to itself ptxas re-derives them from the kernel
+  // parameter with a uniform constant load in front of every refill load (70% of the refill's stall
+  // samples in profiles/r1c)
+  asm volatile("" : "+l"(g0), "+l"(g1));
+  // record offsets of this lane's (x,y) weights (records are rotated by the cell index mod 8)
+  const int ox0 = (sx + b0) & 7, ox1 = ox0 ^ 4, oy = SW + ((sy + c_off) & 7);
+
+  // window registers: channel pairs are held PACKED (one 64-bit register pair = {c, c+1}, exactly as
+  // the 16-byte plane loads deliver them), ready to be FFMA2 operands
+  constexpr int NE = (CB % 2 == 0) ? CB / 2 : CB;
+  using WE = typename std::conditional<CB % 2 == 0, f32x2, float>::type;
+  WE win[SW][2][NE];
+  auto ldw = [&](const V* p, WE (&d)[NE]) {
+    if constexpr (CB == 4) {
+      const ulonglong2 t = __ldg(reinterpret_cast<const ulonglong2*>(p));
+      d[0] = t.x; d[1] = t.y;
+    } else if constexpr (CB == 2) {
+      d[0] = __ldg(reinterpret_cast<const unsigned long long*>(p));
+    } else {
+      d[0] = __ldg(p);
+    }
+  };
+  // The window survives from one segment to the next: curA is the cell whose 8 planes it holds.
+  int curA = -4 * SW;
   // the warp walks the z segments of its row one after the other (a CTA per segment spent a tenth
   // of its short life being launched)
   for (int seg = 0; seg < nseg; ++seg) {
@@ -225,52 +260,6 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   };
   stage();
 
-  // lane -> 2 points of the 8 x 8 (x,y) footprint: y offset c = lane & 7, x offsets b and b + 4
-  const int c_off = lane & 7, b0 = lane >> 3;
-  int iy = sy + c_off;      if (iy >= My) iy -= My;
-  int ix0 = sx + b0;        if (ix0 >= Mx) ix0 -= Mx;
-  int ix1 = sx + b0 + 4;    if (ix1 >= Mx) ix1 -= Mx;
-  // loop invariants as shuffle results: ptxas cannot rematerialise those from the constant bank (it
-  // re-read Mx, My and cb0 with LDC in every advance / atom otherwise)
-  const unsigned plane = __shfl_sync(0xffffffffu, (unsigned)Mx * My, 0), wrap = plane * (unsigned)Mz;
-  const int cb0r = __shfl_sync(0xffffffffu, cb0, 0);
-  const V* g0 = gridt + (size_t)ix0 * My + iy;
-  const V* g1 = gridt + (size_t)ix1 * My + iy;
-  // keep the two lane pointers in registers: left to itself ptxas re-derives them from the kernel
-  // parameter with a uniform constant load in front of every refill load (70% of the refill's stall
-  // samples in profiles/r1c)
-  asm volatile("" : "+l"(g0), "+l"(g1));
-  // record offsets of this lane's (x,y) weights (records are rotated by the cell index mod 8)
-  const int ox0 = (sx + b0) & 7, ox1 = ox0 ^ 4, oy = SW + ((sy + c_off) & 7);
-
-  // warm-up: the 8 planes sz0 .. sz0+7 of the first non-empty cell, slot k <- the plane z == k (mod 8)
-  // (static slots: 16 independent loads in flight, straight into the window registers)
-  const int sz0 = Z0 + first, sz1 = Z0 + last;
-  // window registers: channel pairs are held PACKED (one 64-bit register pair = {c, c+1}, exactly as
-  // the 16-byte plane loads deliver them), ready to be FFMA2 operands
-  constexpr int NE = (CB % 2 == 0) ? CB / 2 : CB;
-  using WE = typename std::conditional<CB % 2 == 0, f32x2, float>::type;
-  WE win[SW][2][NE];
-  auto ldw = [&](const V* p, WE (&d)[NE]) {
-    if constexpr (CB == 4) {
-      const ulonglong2 t = __ldg(reinterpret_cast<const ulonglong2*>(p));
-      d[0] = t.x; d[1] = t.y;
-    } else if constexpr (CB == 2) {
-      d[0] = __ldg(reinterpret_cast<const unsigned long long*>(p));
-    } else {
-      d[0] = __ldg(p);
-    }
-  };
-#pragma unroll
-  for (int k = 0; k < SW; ++k) {
-    int z = sz0 + ((k - sz0) & 7); if (z >= Mz) z -= Mz;
-    const unsigned off = (unsigned)z * plane;
-    ldw(g0 + off, win[k][0]);
-    ldw(g1 + off, win[k][1]);
-  }
-  cp_async_wait_all();
-  __syncwarp();
-
   // The lane sums of an atom are reduced across the warp one atom LATE, inside the next atom's
   // contraction, so that the five dependent shuffle levels (~150 cycles) overlap its FFMAs.
   float pend[8];
@@ -284,11 +273,60 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
     if ((lane & 3) == 0) s_out[8 * pend_row + out_idx] = tot;
   };
 
-  // walk the non-empty cells of the segment; between two of them the window is refilled in one go
-  int cur = first;            // current cell, relative to Z0
+  // walk the non-empty cells of the segment; the window advances to each of them in one go
   unsigned rem = mask;        // non-empty cells not yet visited
-  for (;;) {
+  bool first_cell = true;
+  while (rem != 0u) {
+    const int cur = __ffs(rem) - 1;   // current cell, relative to Z0
     rem &= rem - 1u;
+    // advance the window from cell curA to cell an: the planes max(curA+8, an) .. an+7 replace the ones
+    // that left it (all 8 at the start of a row or after a gap).  Slot k takes the plane
+    // p_k = an + ((k - an) & 7) if that plane is new.  ptxas guards all refill loads with ONE
+    // scoreboard, so any form that branches between the planes of an advance fetches them one L2
+    // round trip after the other (decoded wait masks, 25% of the stall samples in profiles/r1e):
+    // one or two planes go through a switch over the first slot with the second plane predicated,
+    // longer advances are eight predicated loads in one straight-line block.
+    {
+      const int an = Z0 + cur, first_new = max(curA + SW, an);
+      const int cnt = an + SW - first_new;      // 1 .. 8 new planes
+      if (cnt <= 2) {
+        const int z = first_new >= Mz ? first_new - Mz : first_new;
+        const unsigned off = (unsigned)z * plane;
+        unsigned off2 = off + plane; if (off2 == wrap) off2 = 0u;
+        const bool two = cnt == 2;
+        switch (first_new & 7) {
+#define PSWF_SLOT(K)                                     \
+  case K:                                                \
+    ldw(g0 + off, win[K][0]);                            \
+    ldw(g1 + off, win[K][1]);                            \
+    if (two) {                                           \
+      ldw(g0 + off2, win[(K + 1) & 7][0]);               \
+      ldw(g1 + off2, win[(K + 1) & 7][1]);               \
+    }                                                    \
+    break;
+          PSWF_SLOT(0) PSWF_SLOT(1) PSWF_SLOT(2) PSWF_SLOT(3)
+          PSWF_SLOT(4) PSWF_SLOT(5) PSWF_SLOT(6) PSWF_SLOT(7)
+#undef PSWF_SLOT
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < SW; ++k) {
+          const int pk = an + ((k - an) & 7);
+          if (pk >= first_new) {
+            const int z = pk >= Mz ? pk - Mz : pk;
+            const unsigned off = (unsigned)z * plane;
+            ldw(g0 + off, win[k][0]);
+            ldw(g1 + off, win[k][1]);
+          }
+        }
+      }
+      curA = an;
+    }
+    if (first_cell) {   // this segment's records were staged before the window loads were issued
+      cp_async_wait_all();
+      __syncwarp();
+      first_cell = false;
+    }
     {
       const int jlo = __shfl_sync(0xffffffffu, jlo_l, cur);
       const int jhi = __shfl_sync(0xffffffffu, jhi_l, cur);
@@ -381,53 +419,6 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
         pend_row = j - js;
       }
     }
-    if (rem == 0u) break;
-    // advance to the next non-empty cell nxt: the planes max(cur+8, nxt) .. nxt+7 replace the ones that
-    // left the window.  Slot k takes the plane p_k = nxt + ((k - nxt) & 7) if that plane is new.  The
-    // eight slot refills are PREDICATED loads in one straight-line block, straight into the slot
-    // registers: ptxas guards all refill loads with one scoreboard, so in the earlier jump-into-an-
-    // unrolled-sequence form every plane of an advance waited for the previous one's data (the
-    // decoded wait masks and 25% of the stall samples in profiles/r1e say so); here they are all in
-    // flight together.
-    const int nxt = __ffs(rem) - 1;
-    {
-      const int an = Z0 + nxt, first_new = Z0 + max(cur + SW, nxt);
-      const int cnt = an + SW - first_new;      // 1 .. 8 new planes
-      if (cnt <= 2) {
-        // one or two planes (62% of the advances at 0.5 atoms per cell): jump to the first slot; the
-        // second plane, if any, is predicated in the same block
-        const int z = first_new >= Mz ? first_new - Mz : first_new;
-        const unsigned off = (unsigned)z * plane;
-        unsigned off2 = off + plane; if (off2 == wrap) off2 = 0u;
-        const bool two = cnt == 2;
-        switch (first_new & 7) {
-#define PSWF_SLOT(K)                                     \
-  case K:                                                \
-    ldw(g0 + off, win[K][0]);                            \
-    ldw(g1 + off, win[K][1]);                            \
-    if (two) {                                           \
-      ldw(g0 + off2, win[(K + 1) & 7][0]);               \
-      ldw(g1 + off2, win[(K + 1) & 7][1]);               \
-    }                                                    \
-    break;
-          PSWF_SLOT(0) PSWF_SLOT(1) PSWF_SLOT(2) PSWF_SLOT(3)
-          PSWF_SLOT(4) PSWF_SLOT(5) PSWF_SLOT(6) PSWF_SLOT(7)
-#undef PSWF_SLOT
-        }
-      } else {
-#pragma unroll
-        for (int k = 0; k < SW; ++k) {
-          const int pk = an + ((k - an) & 7);
-          if (pk >= first_new) {
-            const int z = pk >= Mz ? pk - Mz : pk;
-            const unsigned off = (unsigned)z * plane;
-            ldw(g0 + off, win[k][0]);
-            ldw(g1 + off, win[k][1]);
-          }
-        }
-      }
-    }
-    cur = nxt;
   }
   retire();
   flush(jend - js);
