@@ -77,23 +77,37 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_lookback(int n, int* __re
       if (lane >= o) inc += u;
     }
     if (lane < kScanThreads / 32) warp_tot[lane] = inc - t;  // exclusive warp offsets
-    if (lane == 31) {                                         // inc = the tile's sum
-      volatile unsigned long long* st = state + 1;
-      int prefix = 0;
-      if (tile == 0) {
-        st[0] = (2ull << 32) | (unsigned int)inc;
-      } else {
-        st[tile] = (1ull << 32) | (unsigned int)inc;
-        for (int p = tile - 1;; --p) {
-          unsigned long long sv;
-          do { sv = st[p]; } while ((sv >> 32) == 0ull);
-          prefix += (int)(unsigned int)sv;
-          if ((sv >> 32) == 2ull) break;
-        }
-        st[tile] = (2ull << 32) | (unsigned int)(prefix + inc);
+    const int tile_sum = __shfl_sync(0xffffffffu, inc, 31);
+    volatile unsigned long long* st = state + 1;
+    int prefix = 0;
+    if (tile == 0) {
+      if (lane == 0) st[0] = (2ull << 32) | (unsigned int)tile_sum;
+    } else {
+      if (lane == 0) st[tile] = (1ull << 32) | (unsigned int)tile_sum;
+      // warp-wide look-back: lane l inspects tile (p - l); the window moves back 32 tiles at a time
+      for (int p = tile - 1;; p -= 32) {
+        unsigned long long sv = 2ull << 32;            // tiles before 0: an inclusive prefix of 0
+        unsigned ready;
+        do {
+          if (p - lane >= 0) sv = st[p - lane];
+          ready = __ballot_sync(0xffffffffu, (sv >> 32) != 0ull);
+          // only the lanes up to the first inclusive prefix have to be valid
+          const unsigned incl_mask = __ballot_sync(0xffffffffu, (sv >> 32) == 2ull);
+          const unsigned need = incl_mask ? ((incl_mask & (0u - incl_mask)) << 1) - 1u : 0xffffffffu;
+          if ((ready & need) == need) {
+            int pv = ((need >> lane) & 1u) ? (int)(unsigned int)sv : 0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) pv += __shfl_xor_sync(0xffffffffu, pv, o);
+            prefix += pv;
+            ready = incl_mask ? 0xffffffffu : 0xfffffffeu;   // all-ones: done; else: next window
+            break;
+          }
+        } while (true);
+        if (ready == 0xffffffffu) break;
       }
-      s_prefix = prefix;
+      if (lane == 0) st[tile] = (2ull << 32) | (unsigned int)(prefix + tile_sum);
     }
+    if (lane == 0) s_prefix = prefix;
   }
   __syncthreads();
   int run = s_prefix + warp_tot[wid] + incl - sum;
