@@ -155,6 +155,18 @@ int pswf_lr_eval_kernel(const pswf_lr_plan* plan, int p, int n, const double* k,
 int pswf_lr_eval_real(const pswf_lr_plan* plan, int p, int n, const double* r, double* L, double* dL);
 int pswf_lr_self_coefficient(const pswf_lr_plan* plan, int p, double* S0);
 
+/* Parameter selection from a target tolerance (Eq. (27)-(29)).
+ * Host-only, no plan needed.  eps_tot is split evenly, eps_band = eps_grid = eps_spread = eps_tot / 3:
+ *   c    = ln(1 / eps_band)                                            Eq. (28)
+ *   h   <= eta pi r_c / c with eta = 0.5 (reading R2), M_d = ceil(L_d / h) rounded up to a
+ *          multiple of 8 (the fast kernels' granularity)               Eq. (29)
+ *   w    = the smallest even window width in 4..16 whose spreading error estimate
+ *          10^(0.46 - 0.85 w) (relative force error of the gridded scheme against the direct k-sum
+ *          at eta = 0.5 and the default window bandwidth, fitted to the measured w = 6, 8, 12, 16
+ *          values of DESIGN.md / SURVEY.md §8(c)) is <= eps_spread.
+ * Returns PSWF_LR_ERR_INVALID_ARG for eps_tot outside [1e-13, 0.3] or non-positive box / r_c. */
+int pswf_lr_suggest_parameters(const double box[3], double eps_tot, double r_c, int grid[3], int* w, double* c);
+
 int pswf_lr_destroy(pswf_lr_plan* plan);
 const char* pswf_lr_error_string(int code);
 const char* pswf_lr_version(void);

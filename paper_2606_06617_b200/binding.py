@@ -43,7 +43,7 @@ class Info(ctypes.Structure):
 
 
 EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_execute", "pswf_lr_execute_host",
-           "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient",
+           "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient", "pswf_lr_suggest_parameters",
            "pswf_lr_channel_energies", "pswf_lr_get_info", "pswf_lr_set_profiling", "pswf_lr_stage_ms",
            "pswf_lr_debug_copy", "pswf_lr_eval_window", "pswf_lr_eval_kernel", "pswf_lr_destroy",
            "pswf_lr_error_string", "pswf_lr_version")
@@ -69,6 +69,8 @@ def lib():
         L.pswf_lr_execute_real.argtypes = [vp, ip, vp, vp, vp, vp, vp, ip, vp]
         L.pswf_lr_eval_real.argtypes = [vp, ip, ip, dp, dp, dp]
         L.pswf_lr_self_coefficient.argtypes = [vp, ip, dp]
+        L.pswf_lr_suggest_parameters.argtypes = [dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ip),
+                                                 ctypes.POINTER(ip), dp]
         L.pswf_lr_channel_energies.argtypes = [vp, vp, vp]
         L.pswf_lr_get_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.pswf_lr_set_profiling.argtypes = [vp, ip]
@@ -99,6 +101,16 @@ def _ptr(t):
     if isinstance(t, np.ndarray):
         return ctypes.c_void_p(t.ctypes.data)
     return ctypes.c_void_p(t.data_ptr())
+
+
+def suggest_parameters(box, eps_tot, r_c):
+    """(grid, w, c) for a target tolerance: Eq. (27)-(29) as read in include/pswf_lr.h (host only)."""
+    bx = (ctypes.c_double * 3)(*[float(v) for v in box])
+    grid = (ctypes.c_int * 3)()
+    w = ctypes.c_int(0)
+    c = ctypes.c_double(0.0)
+    _check(lib().pswf_lr_suggest_parameters(bx, float(eps_tot), float(r_c), grid, ctypes.byref(w), ctypes.byref(c)))
+    return list(grid), w.value, c.value
 
 
 class Plan:

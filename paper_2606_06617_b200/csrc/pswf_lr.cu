@@ -714,6 +714,31 @@ int pswf_lr_eval_kernel(const pswf_lr_plan* p, int pe, int n, const double* k, d
   return 0;
 }
 
+int pswf_lr_suggest_parameters(const double box[3], double eps_tot, double r_c, int grid[3], int* w, double* c) {
+  if (!box || !grid || !w || !c) return PSWF_LR_ERR_INVALID_ARG;
+  if (!(eps_tot >= 1e-13 && eps_tot <= 0.3) || !(r_c > 0)) return PSWF_LR_ERR_INVALID_ARG;
+  for (int d = 0; d < 3; ++d)
+    if (!(box[d] > 0)) return PSWF_LR_ERR_INVALID_ARG;
+  const double eps = eps_tot / 3.0;                 // Eq. (27), uniform allocation
+  const double cc = std::log(1.0 / eps);            // Eq. (28)
+  const double eta = 0.5;                           // reading R2
+  const double h = eta * kPi * r_c / cc;            // Eq. (29)
+  for (int d = 0; d < 3; ++d) {
+    int M = (int)std::ceil(box[d] / h);
+    M = std::max(16, ((M + 7) / 8) * 8);
+    grid[d] = M;
+  }
+  int ww = 16;
+  for (int t = 4; t <= 16; t += 2)
+    if (std::pow(10.0, 0.46 - 0.85 * t) <= eps) {
+      ww = t;
+      break;
+    }
+  *w = ww;
+  *c = cc;
+  return 0;
+}
+
 int pswf_lr_destroy(pswf_lr_plan* p) {
   if (!p) return 0;
   if (p->host_only) {

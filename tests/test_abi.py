@@ -159,3 +159,34 @@ def test_workloads_are_seeded_and_shaped():
     c5 = workloads.make(5, n_atoms=1000)
     assert c5["pos"][:, 2].min() >= 100.0 and c5["pos"][:, 2].max() < 200.0
     assert np.all(a["pos"].astype(np.float32).astype(np.float64) == a["pos"])
+
+
+@pytest.mark.parametrize("eps", [1e-3, 1e-5, 1e-7])
+def test_suggested_parameters_meet_the_tolerance(eps):
+    """pswf_lr_suggest_parameters (Eq. (27)-(29)): with the suggested (grid, w, c) the gridded scheme
+    (oracle B) stays within the grid + spreading share 2 eps / 3 of the direct k-sum (oracle A) in the
+    relative force and energy errors, and the next smaller window would not (the choice is tight);
+    c = ln(3 / eps), grid spacing <= 0.5 pi r_c / c."""
+    from oracle import gridded as G
+    from oracle.direct import direct_sums
+    rng = np.random.default_rng(5)
+    box, r_c, N = [11.0, 12.0, 13.0], 3.2, 40
+    grid, w, c = binding.suggest_parameters(box, eps, r_c)
+    assert abs(c - np.log(3.0 / eps)) < 1e-12
+    assert all(box[d] / grid[d] <= 0.5 * np.pi * r_c / c * (1 + 1e-12) and grid[d] % 8 == 0 for d in range(3))
+    pos = rng.uniform(0, 1, (N, 3)) * box
+    q = rng.normal(0, 1, (2, N))
+    q -= q.mean(axis=1, keepdims=True)
+    ex = [1, 6]
+    EA, _, phiA, FA = direct_sums(pos, q, ex, box, c, r_c, grid=grid)
+
+    def err(width):
+        eta = c * max(box[d] / grid[d] for d in range(3)) / (np.pi * r_c)
+        E, _, phi, F = G.gridded(pos, q, ex, box, grid, width, c, r_c, width * (3.55 - 1.55 * eta))
+        return abs(E - EA) / abs(EA), np.linalg.norm(F - FA) / np.linalg.norm(FA)
+
+    eE, eF = err(w)
+    print("eps=%g grid=%s w=%d c=%.3f: eps_E=%.2e eps_F=%.2e" % (eps, grid, w, c, eE, eF))
+    assert eF <= 2 * eps / 3 and eE <= 2 * eps / 3
+    if w > 4:
+        assert err(w - 2)[1] > 0.5 * eps / 3      # a narrower window would (nearly) exhaust the spreading share
