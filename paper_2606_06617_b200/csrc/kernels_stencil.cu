@@ -182,11 +182,17 @@ struct SpreadShape {
   static constexpr int TY = 8 * WY, TZ = 8 * WZ;
   static constexpr int NROW = TY + 7, NCELL = TZ + 7, NB = TZ + 8;
   static constexpr int NT = 32 * WY * WZ;
-  static constexpr int kHeader = 128 + 2 * 32 * 4 + 3 * 32 * 16;  // mbar+desc | rowoff | rowinfo
-  static constexpr int kTables = 3 * NROW * NB * 4;
+  // staging buffers in flight, and cell-boundary tables (kStages + 1: plane p+1 is built while rounds
+  // of plane p+1-kStages may still be read).  Three stages were measured: the smaller buffers split
+  // every plane into two rounds and the spread went from 329 to 405 us.
+  static constexpr int kStages = 2;
+  static constexpr int kTabs = kStages + 1;
+  static constexpr int kOffDesc = 64, kOffRowoff = 192, kOffRow = kOffRowoff + kStages * 32 * 4;
+  static constexpr int kHeader = kOffRow + kTabs * 32 * 16;   // mbar | desc | rowoff | rowinfo
+  static constexpr int kTables = kTabs * NROW * NB * 4;
   static constexpr int kRuns = SW * NT * 8;   // per thread: 8 packed run descriptors of the current round
   static_assert(NROW <= 32, "one lane per row in the round builder");
-  static_assert(2 * sizeof(RoundDesc) + 32 <= 128, "header");
+  static_assert(kOffDesc + kStages * sizeof(RoundDesc) <= kOffRowoff && 2 * kStages * 8 <= kOffDesc, "header");
 };
 
 // Packed FP32 pairs (sm_100a FFMA2: one instruction, two IEEE fused multiply-adds per lane -- the FLOP
@@ -300,12 +306,13 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
   using S = SpreadShape<WY, WZ>;
   constexpr int NROW = S::NROW, NB = S::NB, NT = S::NT;
   extern __shared__ __align__(128) unsigned char smem[];
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem);                 // [2] records of a round have landed
-  uint64_t* empty = full + 2;                                         // [2] all consumer warps are done with them
-  RoundDesc* s_desc = reinterpret_cast<RoundDesc*>(smem + 32);        // [2]
-  int* s_rowoff = reinterpret_cast<int*>(smem + 128);                 // [2][32]
-  int4* s_row = reinterpret_cast<int4*>(smem + 128 + 256);            // [3][32]  {gA0, nA, gB0, nB}
-  int* s_L = reinterpret_cast<int*>(smem + S::kHeader);               // [3][NROW][NB]
+  constexpr int NS = S::kStages, NTAB = S::kTabs;
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem);                 // [NS] records of a round have landed
+  uint64_t* empty = full + NS;                                        // [NS] all consumer warps are done with them
+  RoundDesc* s_desc = reinterpret_cast<RoundDesc*>(smem + S::kOffDesc);   // [NS]
+  int* s_rowoff = reinterpret_cast<int*>(smem + S::kOffRowoff);       // [NS][32]
+  int4* s_row = reinterpret_cast<int4*>(smem + S::kOffRow);            // [NTAB][32]  {gA0, nA, gB0, nB}
+  int* s_L = reinterpret_cast<int*>(smem + S::kHeader);               // [NTAB][NROW][NB]
   uint2* s_run = reinterpret_cast<uint2*>(smem + S::kHeader + S::kTables) + threadIdx.x;   // [8][NT], this thread's
   float* s_rec = reinterpret_cast<float*>(smem + S::kHeader + S::kTables + S::kRuns);     // [2][cap * recf]
 
@@ -335,7 +342,7 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
   const size_t Mtot = (size_t)Mx * My * Mz;
 
   auto build_plane = [&](int pl) {
-    const int tb = pl % 3;
+    const int tb = pl % NTAB;
     const int sx = X0 + pl;
     for (int t = lane; t < NROW * NB; t += 32) {
       const int r = t / NB, b = t - r * NB;
@@ -367,7 +374,7 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
     nd.p = pn; nd.r0 = rn0; nd.r1 = NROW; nd.a0 = 0; nd.a1 = INT_MAX; nd.total = 0; nd.flush = 1;
     nd.np = pn + 1; nd.nr = 0; nd.na = 0;
     if (pn < NP) {
-      const int tb = pn % 3;
+      const int tb = pn % NTAB;
       const bool mine = lane >= rn0 && lane < NROW;
       int tot = mine ? s_L[(tb * NROW + lane) * NB + NB - 1] : 0;
       if (lane == rn0) tot -= an0;
@@ -423,24 +430,22 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
   };
 
   if (tid == 0) {
-    mbar_init(&full[0], 1);
-    mbar_init(&full[1], 1);
-    mbar_init(&empty[0], WY * WZ);
-    mbar_init(&empty[1], WY * WZ);
+    for (int i = 0; i < NS; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], WY * WZ); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
   if (warp == WY * WZ) {
     // ---- producer warp: cell-boundary tables one plane ahead, rounds two ahead of the consumers.
-    //      Table slot (p+1) % 3 last served plane p-2, whose rounds were all released before the
-    //      empty barrier of the first round of plane p could be passed (two staging buffers).
+    //      Table slot (p+1) % NTAB last served plane p-NS, whose rounds were all released before the
+    //      empty barrier of the first round of plane p could be passed (NS staging buffers: the
+    //      producer is at most NS rounds ahead, and every plane in between holds at least one round).
     build_plane(0);
     __syncwarp();
     int pn = 0, rn = 0, an = 0;
     for (int n = 0;; ++n) {
-      const int nb = n & 1;
-      if (n >= 2) mbar_wait(&empty[nb], ((n >> 1) - 1) & 1);
+      const int nb = n % NS;
+      if (n >= NS) mbar_wait(&empty[nb], ((n / NS) - 1) & 1);
       const RoundDesc nd = build_round(pn, rn, an, nb);
       if (nd.p >= NP) break;
       if (nd.r0 == 0 && nd.a0 == 0 && nd.p + 1 < NP) { build_plane(nd.p + 1); __syncwarp(); }
@@ -459,13 +464,13 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
 
   // ---- consumer warps: free-running, coupled to the producer (and to nothing else) by the barriers
   for (int n = 0;; ++n) {
-    const int cur = n & 1;
-    mbar_wait(&full[cur], (n >> 1) & 1);
+    const int cur = n % NS;
+    mbar_wait(&full[cur], (n / NS) & 1);
     const RoundDesc d = s_desc[cur];
     if (d.p >= NP) break;
     // ---- this thread's atoms of the round ----
     {
-      const int tb = d.p % 3;
+      const int tb = d.p % NTAB;
       const int r_beg = max(rlo, d.r0);
       const int r_hi = lane_ok ? min(rlo + SW, d.r1) : r_beg;
       build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32, d.a0, d.a1);
@@ -508,7 +513,7 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
 template <int WY, int WZ, int NCTA>
 struct SpreadLaunch {
   using S = SpreadShape<WY, WZ>;
-  static size_t smem_bytes(int cap, int recf) { return S::kHeader + S::kTables + S::kRuns + 2 * (size_t)cap * recf * 4; }
+  static size_t smem_bytes(int cap, int recf) { return S::kHeader + S::kTables + S::kRuns + S::kStages * (size_t)cap * recf * 4; }
 
   template <int CB>
   static void run(pswf_lr_plan* p, int nseg, int cap, int recf, int cb0, cudaStream_t st) {
@@ -525,7 +530,7 @@ struct SpreadLaunch {
     const int recf = stencil_rec_floats(p->C);
     // staging capacity: NCTA CTAs per SM
     const size_t budget = (size_t)(227 * 1024) / NCTA - 1024;
-    int cap = (int)((budget - S::kHeader - S::kTables - S::kRuns) / (2 * (size_t)recf * 4));
+    int cap = (int)((budget - S::kHeader - S::kTables - S::kRuns) / (S::kStages * (size_t)recf * 4));
     cap &= ~7;
     // x segments: ONE wave of CTAs.  The atoms are partitioned over the segments, so short segments
     // cost no extra arithmetic, only RED traffic for the 7 shared planes; a second, partly filled
