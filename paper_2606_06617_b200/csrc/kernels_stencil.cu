@@ -341,30 +341,46 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
   const int oy = SW + (y & 7), oz = 2 * SW + (z0 & 7);
   const size_t Mtot = (size_t)Mx * My * Mz;
 
+  // Cell-boundary table of plane pl (producer warp).  Step 1: lane r fetches row r's run bases (4
+  // independent loads per lane, all rows at once).  Step 2: one load per table entry, unrolled so that
+  // several L2 round trips are in flight.  (Measured neutral against re-deriving the bases per entry:
+  // the consumers' waits on the full barrier come from their own imbalance -- the slowest of the four
+  // warps gates the empty barrier -- not from the producer.)
   auto build_plane = [&](int pl) {
     const int tb = pl % NTAB;
     const int sx = X0 + pl;
+    {
+      const int syu = Y0 - (SW - 1) + lane;
+      int4 ri = make_int4(0, 0, 0, 0);
+      if (lane < NROW && syu < My) {
+        const int sy = syu < 0 ? syu + My : syu;
+        const int* rs = start + ((size_t)sx * My + sy) * Mz;
+        const int gA0 = nAc ? __ldg(rs + Mz - nAc) : 0;
+        const int eA = nAc ? __ldg(rs + Mz) : 0;
+        const int gB0 = __ldg(rs + zb0);
+        const int eB = __ldg(rs + zb0 + nBc);
+        ri = make_int4(gA0, eA - gA0, gB0, eB - gB0);
+      }
+      if (lane < NROW) s_row[tb * 32 + lane] = ri;
+    }
+    __syncwarp();
+#pragma unroll 6
     for (int t = lane; t < NROW * NB; t += 32) {
       const int r = t / NB, b = t - r * NB;
       const int syu = Y0 - (SW - 1) + r;
       int val = 0;
-      int4 ri = make_int4(0, 0, 0, 0);
       if (syu < My) {
         const int sy = syu < 0 ? syu + My : syu;
         const int* rs = start + ((size_t)sx * My + sy) * Mz;
-        const int gA0 = nAc ? __ldg(rs + Mz - nAc) : 0;
-        const int nA = nAc ? __ldg(rs + Mz) - gA0 : 0;
-        const int gB0 = __ldg(rs + zb0);
+        const int4 ri = s_row[tb * 32 + r];
         if (b < nAc) {
-          val = __ldg(rs + Mz - nAc + b) - gA0;
+          val = __ldg(rs + Mz - nAc + b) - ri.x;
         } else {
           const int bb = min(b, ncell) - nAc;
-          val = nA + __ldg(rs + zb0 + bb) - gB0;
+          val = ri.y + __ldg(rs + zb0 + bb) - ri.z;
         }
-        if (b == 0) ri = make_int4(gA0, nA, gB0, __ldg(rs + zb0 + nBc) - gB0);
       }
       s_L[(tb * NROW + r) * NB + b] = val;
-      if (b == 0) s_row[tb * 32 + r] = ri;
     }
   };
 
