@@ -211,16 +211,20 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   int curA = -4 * SW;
   // the warp walks the z segments of its row one after the other (a CTA per segment spent a tenth
   // of its short life being launched)
+  // cell boundaries of a segment: lane l <-> cell Z0 + l (the atoms of the row are one run); those of
+  // the NEXT segment are fetched while the current one is processed
+  const int* rowstart = start + ((size_t)sx * My + sy) * Mz;
+  auto fetch_bounds = [&](int sg, int& lo, int& hi) {
+    const int z = sg * ZSEG + lane;
+    lo = 0; hi = 0;
+    if (sg < nseg && z < Mz) { lo = __ldg(rowstart + z); hi = __ldg(rowstart + z + 1); }
+  };
+  int nlo, nhi;
+  fetch_bounds(0, nlo, nhi);
   for (int seg = 0; seg < nseg; ++seg) {
-  const int Z0 = seg * ZSEG, Z1 = min(Z0 + ZSEG, Mz);
-
-  // cell boundaries of the segment: lane l <-> cell Z0 + l; the atoms of the row are one run
-  int jlo_l = 0, jhi_l = 0;
-  if (Z0 + lane < Z1) {
-    const size_t key = ((size_t)sx * My + sy) * Mz + Z0 + lane;
-    jlo_l = __ldg(start + key);
-    jhi_l = __ldg(start + key + 1);
-  }
+  const int Z0 = seg * ZSEG;
+  const int jlo_l = nlo, jhi_l = nhi;
+  fetch_bounds(seg + 1, nlo, nhi);
   const unsigned mask = __ballot_sync(0xffffffffu, jhi_l > jlo_l);
   if (mask == 0u) continue;   // no atoms in this segment of the row (vacuum)
   const int first = __ffs(mask) - 1, last = 31 - __clz(mask);
