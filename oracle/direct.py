@@ -161,3 +161,39 @@ def direct_sums_c(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_m
     if rc != 0:
         raise RuntimeError("oracle_direct_sums failed: %d" % rc)
     return float(E_ch.sum()), E_ch, phi, F
+
+
+# ---------------------------------------------------------------------------------
+# Virial of the reciprocal sum ("forces and virials").
+# ---------------------------------------------------------------------------------
+def virial_direct(pos, q, exponents, box, c, r_c, grid=None, zero_mode=True):
+    """W_ab = -dE/d(eps_ab) of Eq. (5) under a homogeneous strain r -> (1 + eps) r of atoms and cell at
+    fixed q and fixed r_c:  k -> (1 - eps) k, V -> V (1 + tr eps), rho(k) unchanged, hence
+
+        W_ab = (1/2V) sum_{k in K} |rho(k)|^2 [ Phi^(k) delta_ab + Phi^'(k) k_a k_b / |k| ]
+               + delta_ab Phi0 Q_net^2 / (2V).
+
+    Phi^' is taken by central differences of Mollifier.Phi_hat (the oracle has no closed form of
+    its own for it).  Returns the symmetric 3x3 tensor, summed over channels."""
+    pos = np.asarray(pos, dtype=np.float64)
+    q = np.atleast_2d(np.asarray(q, dtype=np.float64))
+    box = np.asarray(box, dtype=np.float64)
+    V = float(np.prod(box))
+    moll = Mollifier(c, r_c)
+    m = mode_set(box, c, r_c, grid, half=False)
+    k = 2 * np.pi * m / box
+    kn = np.sqrt((k ** 2).sum(1))
+    rho = q @ np.exp(1j * pos @ k.T)               # (C, K)
+    W = np.zeros((3, 3))
+    kc = c / r_c
+    for a, p in enumerate(exponents):
+        h = 1e-6 * kn
+        up = np.minimum(kn + h, kc * (1 - 1e-14))
+        Ph = moll.Phi_hat(int(p), kn)
+        dPh = (moll.Phi_hat(int(p), up) - moll.Phi_hat(int(p), kn - h)) / (up - (kn - h))
+        r2 = np.abs(rho[a]) ** 2
+        W += np.eye(3) * (Ph * r2).sum() / (2 * V)
+        W += np.einsum("k,ka,kb->ab", dPh * r2 / kn, k, k) / (2 * V)
+        if zero_mode:
+            W += np.eye(3) * moll.Phi0(int(p)) * q[a].sum() ** 2 / (2 * V)
+    return W

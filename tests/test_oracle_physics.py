@@ -227,3 +227,50 @@ def test_real_space_parts_energy_forces_potentials():
         qm[a, i] -= h
         fd = (real_space_parts(pos, qp, ex, box, c, r_c)[0] - real_space_parts(pos, qm, ex, box, c, r_c)[0]) / (2 * h)
         assert abs(fd - phi[a, i]) < 1e-8 * np.abs(phi).max()
+
+
+def test_virial_direct_matches_strain_derivative_of_energy():
+    """oracle.direct.virial_direct: the diagonal equals -dE/d(eps_aa) by central differences of the
+    direct k-sum under a homogeneous strain of atoms and cell (mode integers fixed), charged and
+    neutral channels, p = 1, 3, 6; the tensor is symmetric and its off-diagonal part changes sign
+    under the mirror x -> -x (so a swapped or dropped index cannot hide)."""
+    from oracle.direct import virial_direct, mode_set
+    from oracle.kernels import Mollifier
+    rng = np.random.default_rng(3)
+    box = np.array([9.0, 10.0, 11.5])
+    N = 20
+    pos = rng.uniform(0, 1, (N, 3)) * box
+    q = rng.normal(0, 1, (3, N))
+    q[0] -= q[0].mean()
+    ex = [1, 3, 6]
+    c, r_c = 12.024, 3.4
+    W = virial_direct(pos, q, ex, box, c, r_c)
+    assert np.allclose(W, W.T, rtol=0, atol=1e-13 * np.abs(W).max())
+    m = mode_set(box, c, r_c, None, half=False)
+
+    def energy(bx, ps):           # Eq. (5) on the FIXED integer mode set
+        V = np.prod(bx)
+        k = 2 * np.pi * m / bx
+        kn = np.sqrt((k ** 2).sum(1))
+        rho = q @ np.exp(1j * ps @ k.T)
+        moll = Mollifier(c, r_c)
+        E = 0.0
+        for a, p in enumerate(ex):
+            ph = np.where(kn * r_c < c, moll.Phi_hat(p, np.minimum(kn, c / r_c * (1 - 1e-14))), 0.0)
+            E += (ph * np.abs(rho[a]) ** 2).sum() / (2 * V) + moll.Phi0(p) * q[a].sum() ** 2 / (2 * V)
+        return E
+
+    for d in range(3):
+        e = 1e-6
+        sp, sm = np.ones(3), np.ones(3)
+        sp[d] += e
+        sm[d] -= e
+        fd = -(energy(box * sp, pos * sp) - energy(box * sm, pos * sm)) / (2 * e)
+        assert abs(fd - W[d, d]) < 2e-7 * np.abs(W).max(), (d, fd, W[d, d])
+    pm = pos.copy()
+    pm[:, 0] = box[0] - pm[:, 0]
+    Wm = virial_direct(pm, q, ex, box, c, r_c)
+    assert np.allclose(Wm[0, 1], -W[0, 1], atol=1e-10 * np.abs(W).max())
+    assert np.allclose(Wm[0, 2], -W[0, 2], atol=1e-10 * np.abs(W).max())
+    assert np.allclose(Wm[1, 2], W[1, 2], atol=1e-10 * np.abs(W).max())
+    assert np.allclose(np.diag(Wm), np.diag(W), atol=1e-10 * np.abs(W).max())
