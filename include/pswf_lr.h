@@ -124,6 +124,17 @@ int pswf_lr_execute_host(pswf_lr_plan* plan, int n_atoms, const void* pos, const
 int pswf_lr_execute_real(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, void* E,
                          void* phi, void* F, int accumulate, void* stream);
 
+/* Virial ("forces and virials"): W_ab = -dE/d(eps_ab) under a
+ * homogeneous strain of atoms and cell at fixed q and r_c.  After pswf_lr_set_virial(plan, 1) every
+ * pswf_lr_execute accumulates the virial of the reciprocal energy in its scale kernel,
+ *   W_ab = 1/2 sum_m D(m) |rho^(m)|^2 [delta_ab + (dD/dk)/(D |k|) k_a k_b]  (+ the k = 0 term),
+ * the exact strain derivative of the gridded energy, and pswf_lr_execute_real adds (accumulate != 0) or
+ * restarts (accumulate = 0) with the pair virial -1/2 sum_{i != j} q q L'(r) r_a r_b / r.
+ * pswf_lr_virial copies it to a DEVICE buffer double[6] = xx, yy, zz, xy, xz, yz (async on stream).
+ * Pressure: P = tr W / (3V) for this part of the energy. */
+int pswf_lr_set_virial(pswf_lr_plan* plan, int enabled);
+int pswf_lr_virial(pswf_lr_plan* plan, void* W, void* stream);
+
 /* Per-channel energies of the most recent execute: device double[n_channels] (async on stream).
  * The paper reports per-component contributions. */
 int pswf_lr_channel_energies(pswf_lr_plan* plan, void* E_channels, void* stream);

@@ -43,7 +43,7 @@ class Info(ctypes.Structure):
 
 
 EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_execute", "pswf_lr_execute_host",
-           "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient", "pswf_lr_suggest_parameters",
+           "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient", "pswf_lr_suggest_parameters", "pswf_lr_set_virial", "pswf_lr_virial",
            "pswf_lr_channel_energies", "pswf_lr_get_info", "pswf_lr_set_profiling", "pswf_lr_stage_ms",
            "pswf_lr_debug_copy", "pswf_lr_eval_window", "pswf_lr_eval_kernel", "pswf_lr_destroy",
            "pswf_lr_error_string", "pswf_lr_version")
@@ -71,6 +71,8 @@ def lib():
         L.pswf_lr_self_coefficient.argtypes = [vp, ip, dp]
         L.pswf_lr_suggest_parameters.argtypes = [dp, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ip),
                                                  ctypes.POINTER(ip), dp]
+        L.pswf_lr_set_virial.argtypes = [vp, ip]
+        L.pswf_lr_virial.argtypes = [vp, vp, vp]
         L.pswf_lr_channel_energies.argtypes = [vp, vp, vp]
         L.pswf_lr_get_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.pswf_lr_set_profiling.argtypes = [vp, ip]
@@ -203,6 +205,13 @@ class Plan:
             Ep = ctypes.cast(_ptr(E), ctypes.POINTER(ctypes.c_double))
         _check(lib().pswf_lr_execute_host(self._h, int(n_atoms), _ptr(pos), _ptr(q), Ep, _ptr(phi), _ptr(F),
                                           ctypes.c_void_p(stream or 0)))
+
+    def set_virial(self, enabled):
+        _check(lib().pswf_lr_set_virial(self._h, 1 if enabled else 0))
+
+    def virial(self, out, stream=None):
+        """out: float64 device tensor of 6 (xx, yy, zz, xy, xz, yz)."""
+        _check(lib().pswf_lr_virial(self._h, _ptr(out), ctypes.c_void_p(stream or 0)))
 
     def channel_energies(self, out, stream=None):
         _check(lib().pswf_lr_channel_energies(self._h, _ptr(out), ctypes.c_void_p(stream or 0)))

@@ -208,16 +208,51 @@ __device__ __forceinline__ T kernel_value(const ScaleParams<T>& P, int slot, T x
   return s * P.slot_pre[slot];
 }
 
+// d Phi^_p / dk by the derivative of the SAME panel polynomial plus the derivative of the bare factor
+// (virial).  x = kappa / c, kappa = k r_c, dx/dk = x_per_k, dkappa/dk = c x_per_k.
 template <class T>
-__global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __restrict__ Ech, int want_E) {
+__device__ __forceinline__ T kernel_dvalue(const ScaleParams<T>& P, int slot, T x, T kappa) {
+  int j = min((int)(x * (T)P.panels), P.panels - 1);
+  T xi = (T)2 * (x * (T)P.panels - (T)j) - (T)1;
+  const T* cf = P.kcoef + ((size_t)slot * P.panels + j) * (P.degree + 1);
+  T t = cf[P.degree], dt = (T)P.degree * cf[P.degree];
+  for (int m = P.degree - 1; m >= 1; --m) {
+    t = fma(t, xi, cf[m]);
+    dt = fma(dt, xi, (T)m * cf[m]);
+  }
+  t = fma(t, xi, cf[0]);
+  dt *= (T)2 * (T)P.panels;            // dT/dx
+  const T rc = P.c * P.x_per_k;
+  T ds;
+  switch (P.slot_p[slot]) {
+    case 1: ds = dt * P.x_per_k / (kappa * kappa) - (T)2 * t * rc / (kappa * kappa * kappa); break;
+    case 2: ds = dt * P.x_per_k / kappa - t * rc / (kappa * kappa); break;
+    case 3: ds = (dt - (T)1 / x) * P.x_per_k; break;
+    case 5: ds = (dt + (T)2 * x * log(x) + x) * P.x_per_k; break;
+    default: ds = dt * P.x_per_k; break;
+  }
+  return ds * P.slot_pre[slot];
+}
+
+// VIR: also accumulate the virial W_ab = 1/2 sum_m' |rho^|^2 [D delta_ab + (dD/dk) k_a k_b / |k|] of the
+// discrete energy (its exact strain derivative: the window transform depends on k h only, which a
+// homogeneous strain leaves unchanged) into Wacc[6] = xx, yy, zz, xy, xz, yz.
+template <class T, bool VIR>
+__global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __restrict__ Ech, int want_E,
+                        double* __restrict__ Wacc) {
   const size_t Mhalf = (size_t)P.M[0] * P.M[1] * P.Mzh;
   const size_t m = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   __shared__ double red[kMaxChannels];
+  __shared__ double redw[6];
   if (threadIdx.x < kMaxChannels) red[threadIdx.x] = 0.0;
+  if (VIR && threadIdx.x < 6) redw[threadIdx.x] = 0.0;
   __syncthreads();
   bool active = m < Mhalf;
   bool inside = false;
   T D[6];
+  T dDk[6];            // (dD/dk) / |k| per slot
+  T kv[3] = {(T)0, (T)0, (T)0};
+  double wloc[6] = {0, 0, 0, 0, 0, 0};
   T herm = (T)0;
   int iz = 0;
   bool is_zero_mode = false;
@@ -241,6 +276,10 @@ __global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __
       T base = P.base * P.invW2[0][ix] * P.invW2[1][iy] * P.invW2[2][iz];
       T kappa = x * P.c;
       for (int s = 0; s < P.nslots; ++s) D[s] = base * kernel_value(P, s, x, kappa);
+      if (VIR) {
+        kv[0] = kx; kv[1] = ky; kv[2] = kz;
+        for (int s = 0; s < P.nslots; ++s) dDk[s] = base * kernel_dvalue(P, s, x, kappa) / kn;
+      }
     }
   }
   for (int c = 0; c < P.C; ++c) {
@@ -250,7 +289,16 @@ __global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __
       if (inside || is_zero_mode) {
         T d = is_zero_mode ? P.chan_D0[c] : D[P.chan_slot[c]];
         Cplx<T> v = *ptr;
-        e = (double)(herm * d * (v.x * v.x + v.y * v.y));
+        const T a2 = herm * (v.x * v.x + v.y * v.y);
+        e = (double)(a2 * d);
+        if (VIR) {
+          wloc[0] += e; wloc[1] += e; wloc[2] += e;
+          if (!is_zero_mode) {
+            const double g = (double)(a2 * dDk[P.chan_slot[c]]);
+            wloc[0] += g * kv[0] * kv[0]; wloc[1] += g * kv[1] * kv[1]; wloc[2] += g * kv[2] * kv[2];
+            wloc[3] += g * kv[0] * kv[1]; wloc[4] += g * kv[0] * kv[2]; wloc[5] += g * kv[1] * kv[2];
+          }
+        }
         v.x *= d;
         v.y *= d;
         *ptr = v;
@@ -269,6 +317,15 @@ __global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __
   if (want_E) {
     __syncthreads();
     if (threadIdx.x < P.C && red[threadIdx.x] != 0.0) atomicAdd(&Ech[threadIdx.x], 0.5 * red[threadIdx.x]);
+  }
+  if (VIR) {
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      const double t = warp_sum(wloc[i]);
+      if ((threadIdx.x & 31) == 0 && t != 0.0) atomicAdd(&redw[i], t);
+    }
+    __syncthreads();
+    if (threadIdx.x < 6 && redw[threadIdx.x] != 0.0) atomicAdd(&Wacc[threadIdx.x], 0.5 * redw[threadIdx.x]);
   }
 }
 
@@ -371,8 +428,11 @@ template <class T>
 void launch_scale(pswf_lr_plan* p, const ScaleParams<T>& P, bool want_E, cudaStream_t st) {
   const size_t Mhalf = (size_t)P.M[0] * P.M[1] * P.Mzh;
   const int threads = 256;
-  k_scale<T><<<(unsigned)((Mhalf + threads - 1) / threads), threads, 0, st>>>(P, (Cplx<T>*)p->d_spec, p->d_Ech,
-                                                                              want_E ? 1 : 0);
+  const unsigned nb = (unsigned)((Mhalf + threads - 1) / threads);
+  if (p->virial)
+    k_scale<T, true><<<nb, threads, 0, st>>>(P, (Cplx<T>*)p->d_spec, p->d_Ech, want_E ? 1 : 0, p->d_virial);
+  else
+    k_scale<T, false><<<nb, threads, 0, st>>>(P, (Cplx<T>*)p->d_spec, p->d_Ech, want_E ? 1 : 0, nullptr);
 }
 
 void launch_finalize_energy(pswf_lr_plan* p, double* E, cudaStream_t st) {

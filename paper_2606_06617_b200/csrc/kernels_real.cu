@@ -48,8 +48,10 @@ __global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, Rea
                                                        const int* __restrict__ start, const int* __restrict__ si0,
                                                        const T* __restrict__ spos, const T* __restrict__ sq,
                                                        const int* __restrict__ perm, double* __restrict__ Eacc,
-                                                       T* __restrict__ phi, T* __restrict__ F, int accumulate) {
+                                                       T* __restrict__ phi, T* __restrict__ F, int accumulate,
+                                                       double* __restrict__ Wacc) {
   __shared__ double s_E;
+  __shared__ double s_W[6];
   __shared__ int s_qk[4][64];        // queue of accepted neighbour indices, one ring per warp
   __shared__ T s_qd[4][64][4];       // their minimum-image displacement and r^2
   extern __shared__ __align__(16) unsigned char s_raw[];
@@ -58,10 +60,12 @@ __global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, Rea
   for (int t = threadIdx.x; t < P.nslots * P.panels * (P.degree + 1); t += blockDim.x) s_cf[t] = P.coef[t];
   for (int t = threadIdx.x; t < P.nslots * P.panels * P.degree; t += blockDim.x) s_df[t] = P.dcoef[t];
   if (threadIdx.x == 0) s_E = 0.0;
+  if (threadIdx.x < 6) s_W[threadIdx.x] = 0.0;
   __syncthreads();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int j = blockIdx.x * 4 + wid;
   double e_thread = 0.0;
+  T wv[6] = {0, 0, 0, 0, 0, 0};   // virial of this lane's pairs: -1/2 sum qq L'(r) d_a d_b / r (each pair is visited twice)
   if (j < n) {
     const int Mx = g.M[0], My = g.M[1], Mz = g.M[2];
     const int cx = wrap_index(si0[j], Mx), cy = wrap_index(si0[(size_t)cap + j], My),
@@ -114,6 +118,11 @@ __global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, Rea
       fx = fma(sc, ddx, fx);
       fy = fma(sc, ddy, fy);
       fz = fma(sc, ddz, fz);
+      if (Wacc) {
+        const T hs = (T)-0.5 * sc;
+        wv[0] = fma(hs * ddx, ddx, wv[0]); wv[1] = fma(hs * ddy, ddy, wv[1]); wv[2] = fma(hs * ddz, ddz, wv[2]);
+        wv[3] = fma(hs * ddx, ddy, wv[3]); wv[4] = fma(hs * ddx, ddz, wv[4]); wv[5] = fma(hs * ddy, ddz, wv[5]);
+      }
     };
     auto drain = [&](int m) {   // the first m (<= 32) queued pairs, one per lane
       __syncwarp();
@@ -198,8 +207,16 @@ __global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, Rea
   }
   e_thread = warp_sum(e_thread);
   if ((threadIdx.x & 31) == 0 && e_thread != 0.0) atomicAdd(&s_E, e_thread);
+  if (Wacc) {
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      const double t = warp_sum((double)wv[i]);
+      if ((threadIdx.x & 31) == 0 && t != 0.0) atomicAdd(&s_W[i], t);
+    }
+  }
   __syncthreads();
   if (threadIdx.x == 0 && s_E != 0.0) atomicAdd(Eacc, s_E);
+  if (Wacc && threadIdx.x < 6 && s_W[threadIdx.x] != 0.0) atomicAdd(&Wacc[threadIdx.x], s_W[threadIdx.x]);
 }
 
 __global__ void k_real_finalize(const double* __restrict__ Eacc, double* __restrict__ E, int accumulate) {
@@ -212,6 +229,9 @@ template <class T>
 void launch_real_space(pswf_lr_plan* p, int n, const T* pos, const RealGeom<T>& g, const RealParams<T>& P, double* E,
                        T* phi, T* F, int accumulate, cudaStream_t st) {
   cudaMemsetAsync(p->d_Ereal, 0, sizeof(double), st);
+  // virial: added to the plan's accumulator when accumulate is set (after pswf_lr_execute), else restarted
+  double* wacc = p->virial ? p->d_virial : nullptr;
+  if (wacc && !accumulate) cudaMemsetAsync(wacc, 0, sizeof(double) * 6, st);
   if (n > 0) {
     k_sorted_pos<T><<<(n + 255) / 256, 256, 0, st>>>(n, p->cap_atoms, pos, p->d_perm, g, (T*)p->d_spos);
     const size_t tb = sizeof(T) * (size_t)P.nslots * P.panels * (2 * P.degree + 1);   // <= 6 * 32 * 49 * 8 = 75 KB
@@ -219,7 +239,7 @@ void launch_real_space(pswf_lr_plan* p, int n, const T* pos, const RealGeom<T>& 
   cudaFuncSetAttribute(k_real_pairs_q<T, CTV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tb);            \
   k_real_pairs_q<T, CTV><<<(n + 3) / 4, 128, tb, st>>>(n, p->C, p->cap_atoms, g, P, p->d_count, p->d_si0,        \
                                                         (const T*)p->d_spos, (const T*)p->d_sq, p->d_perm,        \
-                                                        p->d_Ereal, phi, F, accumulate)
+                                                        p->d_Ereal, phi, F, accumulate, wacc)
     if (p->C <= 4) { PSWF_REAL(4); }
     else if (p->C <= 8) { PSWF_REAL(8); }
     else { PSWF_REAL(kMaxChannels); }

@@ -105,6 +105,8 @@ struct pswf_lr_plan {
   void* d_rdcoef = nullptr;
   void* d_spos = nullptr;         // real [3][cap] wrapped positions in sorted order
   double* d_Ereal = nullptr;      // [1]
+  double* d_virial = nullptr;     // [6] xx, yy, zz, xy, xz, yz (when virial accumulation is enabled)
+  bool virial = false;
   // device tables (plan precision)
   void* d_wcoef = nullptr;
   void* d_wdcoef = nullptr;

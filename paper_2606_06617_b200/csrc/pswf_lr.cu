@@ -189,6 +189,7 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   if (ev) cudaEventRecord(ev[3], st);
   // a3
   cudaMemsetAsync(p->d_Ech, 0, sizeof(double) * p->C, st);
+  if (p->virial) cudaMemsetAsync(p->d_virial, 0, sizeof(double) * 6, st);
   launch_scale<T>(p, P, true, st);
   if (E) launch_finalize_energy(p, E, st);
   if (ev) cudaEventRecord(ev[4], st);
@@ -450,6 +451,7 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Etot, sizeof(double), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ereal, sizeof(double), &b);
+      if (!rc) rc = dev_alloc((void**)&p->d_virial, sizeof(double) * 6, &b);
       p->workspace_bytes += b;
     }
     if (!rc && !p->host_only) {
@@ -575,6 +577,21 @@ int pswf_lr_self_coefficient(const pswf_lr_plan* p, int pe, double* S0) {
       return 0;
     }
   return PSWF_LR_ERR_UNSUPPORTED_EXPONENT;
+}
+
+int pswf_lr_set_virial(pswf_lr_plan* p, int enabled) {
+  if (!p) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  p->virial = enabled != 0;
+  return 0;
+}
+
+int pswf_lr_virial(pswf_lr_plan* p, void* W, void* stream) {
+  if (!p || !W) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  if (!p->virial) return PSWF_LR_ERR_INVALID_ARG;
+  CUDA_TRY(cudaMemcpyAsync(W, p->d_virial, sizeof(double) * 6, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return 0;
 }
 
 int pswf_lr_channel_energies(pswf_lr_plan* p, void* E_channels, void* stream) {
@@ -749,7 +766,7 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   free_atoms(p);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
                   p->d_grid,  p->d_spec,    p->d_count,    p->d_scan_state, p->d_Ech,      p->d_Etot,
-                  p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal};
+                  p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal, p->d_virial};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   if (p->have_fft) {

@@ -464,6 +464,72 @@ def test_full_decomposition_on_gpu_madelung():
     plan.destroy()
 
 
+def _virial(plan):
+    W = torch.zeros(6, dtype=torch.float64, device="cuda:0")
+    plan.virial(W, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    w = W.cpu().numpy()
+    return np.array([[w[0], w[3], w[4]], [w[3], w[1], w[5]], [w[4], w[5], w[2]]])
+
+
+def test_virial_reciprocal_vs_oracle():
+    """the virial accumulated in the scale kernel against the oracle's k-sum
+    virial (fp64, w = 16: aliasing-free; fp32 at w = 8 within the fp32 force gate), p = 1, 3, 6 with a
+    charged channel (zero-mode term), anisotropic box."""
+    from oracle.direct import virial_direct
+    rng = np.random.default_rng(17)
+    box, grid = [9.0, 10.0, 11.5], [24, 24, 32]
+    N = 60
+    pos = rng.uniform(0, 1, (N, 3)) * box
+    q = rng.normal(0, 1, (3, N))
+    q[0] -= q[0].mean()
+    for precision, w, tol in [("f64", 16, 1e-9), ("f32", 8, 1e-4)]:
+        pp = pos.astype(np.float32).astype(np.float64) if precision == "f32" else pos
+        qq = q.astype(np.float32).astype(np.float64) if precision == "f32" else q
+        wl = dict(pos=pp, q=qq, exponents=[1, 3, 6], box=box, grid=grid, w=w, c=12.024, precision=precision)
+        plan = make_plan(wl)
+        plan.set_virial(True)
+        run_gpu(wl, plan=plan)
+        W = _virial(plan)
+        W_ref = virial_direct(pp, qq, wl["exponents"], box, wl["c"], plan.info()["r_c"], grid=grid)
+        err = np.abs(W - W_ref).max() / np.abs(W_ref).max()
+        print("virial %s: max rel err %.2e" % (precision, err))
+        assert err <= tol
+        plan.destroy()
+
+
+def test_virial_real_space_vs_strain_derivative_of_scaffold():
+    """The pair virial of pswf_lr_execute_real: diagonal = -dE/d(eps_aa) of the scaffold's real-space
+    energy by central differences under a homogeneous strain (fp64); symmetric; and execute +
+    execute_real(accumulate) add up."""
+    from oracle.scaffold import real_space_parts
+    rng = np.random.default_rng(23)
+    box, grid = np.array([12.0, 13.0, 14.0]), [24, 24, 32]
+    N, r_c = 80, 4.4
+    pos = rng.uniform(0, 1, (N, 3)) * box
+    q = rng.normal(0, 1, (2, N))
+    ex = [1, 6]
+    wl = dict(pos=pos, q=q, exponents=ex, box=list(box), grid=grid, w=8, c=12.024, precision="f64")
+    plan = make_plan(wl, r_c=r_c)
+    plan.set_virial(True)
+    _run_real(wl, plan)
+    W = _virial(plan)
+    for d in range(3):
+        e = 1e-6
+        sp, sm = np.ones(3), np.ones(3)
+        sp[d] += e
+        sm[d] -= e
+        fd = -(real_space_parts(pos * sp, q, ex, box * sp, 12.024, r_c)[0]
+               - real_space_parts(pos * sm, q, ex, box * sm, 12.024, r_c)[0]) / (2 * e)
+        assert abs(fd - W[d, d]) <= 1e-6 * np.abs(W).max(), (d, fd, W[d, d])
+    run_gpu(wl, plan=plan)
+    W_rec = _virial(plan)
+    _run_real(wl, plan, accumulate_after_recip=True)
+    W_tot = _virial(plan)
+    assert np.abs(W_tot - (W_rec + W)).max() <= 1e-11 * np.abs(W_tot).max()
+    plan.destroy()
+
+
 def test_native_library_is_loaded():
     """The product path is the CUDA library: the shared object is mapped into this process."""
     binding.lib()
