@@ -11,13 +11,15 @@ Modules (each function cites the PAPER.md passage it follows):
   kernels.py   S^_p(k), Phi^_p(k), k=0 constants,  Theorem 1 (S47)-(S52), (S60),
                S_p(r), S_p(0)                      (S17)-(S33), (S67), (S73)-(S79)
   direct.py    oracle A: direct non-uniform        Eq. (5)-(6)
-               Fourier sums for E, phi, F
+               Fourier sums for E, phi, F;
+               virial_direct (strain derivative)
   direct_sum.c same sums in plain C/OpenMP for the
                large configurations
   gridded.py   oracle B: spread/FFT/scale/iFFT/    Eq. (20)-(26)
                gather in float64 numpy
   scaffold.py  real-space complement, self term,   (S64)-(S68), Eq. (12)
-               classical erfc Ewald (validation only)
+               classical erfc Ewald; real_space_parts is
+               the parity target of pswf_lr_execute_real
 
 Pins (tests/test_oracle_*.py) and their status are listed in DESIGN.md §3.
 Parity unpinned: none of the functions used for GPU parity; the paper's own
