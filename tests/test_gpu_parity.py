@@ -530,6 +530,36 @@ def test_virial_real_space_vs_strain_derivative_of_scaffold():
     plan.destroy()
 
 
+def test_random_configurations_fast_path_consistent_with_reference_kernels():
+    """Consistency, not a parity claim: twelve seeded random configurations (grids, densities, channel
+    counts, widths; uniform, tightly clustered and slab-shaped systems, the clustered ones drive the
+    sub-row rounds of the spread and the re-staging of the gather) through the fast kernels and
+    through the one-warp-per-atom reference kernels, which are the ones pinned to oracle B above."""
+    rng = np.random.default_rng(2024)
+    for it in range(12):
+        grid = [int(rng.choice([16, 24, 32, 40, 48, 64])) for _ in range(3)]
+        box = [float(g * rng.uniform(0.8, 2.0)) for g in grid]
+        C = int(rng.integers(1, 9))
+        w = int(rng.choice([4, 6, 8]))
+        N = int(rng.choice([1, 7, 300, 5000, 40000]))
+        mode = it % 3
+        pos = rng.uniform(0, 1, (N, 3)) * box
+        if mode == 1:
+            pos = (np.array(box) * rng.uniform(0, 1, 3) + rng.normal(0, 0.6, (N, 3))) % box
+        if mode == 2:
+            pos[:, 2] = box[2] * (0.3 + 0.2 * rng.uniform(0, 1, N))
+        pos = pos.astype(np.float32).astype(np.float64)
+        q = rng.normal(0, 0.5, (C, N)).astype(np.float32).astype(np.float64)
+        ex = [int(rng.integers(1, 7)) for _ in range(C)]
+        wl = dict(pos=pos, q=q, exponents=ex, box=box, grid=grid, w=w, c=12.024, precision="f32")
+        a = run_gpu(wl, kernel_path=0)
+        b = run_gpu(wl, kernel_path=1)
+        assert abs(a["E"] - b["E"]) <= 2e-5 * abs(b["E"]), (it, grid, N, C, w)
+        assert rel(a["phi"], b["phi"]) <= 5e-5, (it, grid, N, C, w)
+        if N > 1:
+            assert rel(a["F"], b["F"]) <= 5e-5, (it, grid, N, C, w)
+
+
 def test_native_library_is_loaded():
     """The product path is the CUDA library: the shared object is mapped into this process."""
     binding.lib()
