@@ -314,6 +314,8 @@ def run_ours(args):
                 "traffic_source": "profiles/r1f_ncu_full.md (dram__bytes_read+write of one launch, config 4)",
                 "alg_flops": flops_alg[dom], "alg_bytes": bytes_alg[dom],
                 "peak_source": "148 SM x 128 FMA/clk x 2 x %.0f MHz (DESIGN.md §6)" % sm_max,
+                "time_source": "CUDA events around the %s stage on the execute stream (for gather: the 12 us "
+                               "transposing interleave + k_gather_rows), mean over the timed steps" % dom,
                 "hbm_achieved_gbs": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9,
                 "hbm_frac": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9 / peak_gbs}
     stages = {k: {"ms": stage_ms[k], "alg_bytes": bytes_alg[k],
