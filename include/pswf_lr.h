@@ -14,7 +14,9 @@
  * and as the automatic-differentiation backward of (i)-(iv) does -- an inverse
  * FFT and a gather with the window and its derivative, giving per-atom potentials
  * phi_i^a = dE/dq_i^a and forces F_i = -dE/dr_i (q fixed).
- * No self term, no real-space term: those are off the hot path ("out of scope").
+ * pswf_lr_execute computes exactly that (no self term, no real-space term: the hot path).  The rows
+ * SURVEY.md §8(f) ranks next are separate entry points: pswf_lr_execute_real (real-space complement
+ * and self term, completing (S65)), pswf_lr_set_virial / pswf_lr_virial, pswf_lr_suggest_parameters.
  *
  * All kernels are CUDA for sm_100a; the 3-D FFTs are cuFFT.  There is no CPU fallback: every
  * call fails with PSWF_LR_ERR_CUDA when no device is usable.
