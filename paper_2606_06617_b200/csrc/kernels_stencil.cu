@@ -190,7 +190,7 @@ struct SpreadShape {
   static constexpr int kOffDesc = 64, kOffRowoff = 192, kOffRow = kOffRowoff + kStages * 32 * 4;
   static constexpr int kHeader = kOffRow + kTabs * 32 * 16;   // mbar | desc | rowoff | rowinfo
   static constexpr int kTables = kTabs * NROW * NB * 4;
-  static constexpr int kRuns = SW * NT * 8;   // per thread: 8 packed run descriptors of the current round
+  static constexpr int kRuns = (SW + 1) * NT * 8;   // per thread: 8 packed run descriptors of the current round (+1: prefetch past the last)
   static_assert(NROW <= 32, "one lane per row in the round builder");
   static_assert(kOffDesc + kStages * sizeof(RoundDesc) <= kOffRowoff && 2 * kStages * 8 <= kOffDesc, "header");
 };
@@ -211,9 +211,27 @@ __device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c) {
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
   return d;
 }
+__device__ __forceinline__ void ffma2_acc(f32x2& c, f32x2 a, f32x2 b) {   // c += a * b, in place
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+}
+
+// zero one half of a packed pair in place (the same register keeps holding the accumulator: a fresh
+// pack2() in each arm of the flush switch left ptxas with 16 register moves per atom visit)
+__device__ __forceinline__ void zero_lo(f32x2& v) {
+  asm("{\n.reg .b32 lo, hi;\nmov.b64 {lo, hi}, %0;\nmov.b64 %0, {0f00000000, hi};\n}" : "+l"(v));
+}
+__device__ __forceinline__ void zero_hi(f32x2& v) {
+  asm("{\n.reg .b32 lo, hi;\nmov.b64 {lo, hi}, %0;\nmov.b64 %0, {lo, 0f00000000};\n}" : "+l"(v));
+}
 
 __device__ __forceinline__ void red_add_v2(float* p, float a, float b) {
   asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
+}
+
+__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) {
+  f32x2 d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
 }
 
 // One thread's atoms of a round are (at most) 8 runs of staged records, one per cell row s_y = y-7 .. y:
@@ -221,11 +239,14 @@ __device__ __forceinline__ void red_add_v2(float* p, float a, float b) {
 // first cell miss column z0+1 (j < ja) and atoms of the last cell miss column z0 (j >= jb).
 // The runs are computed once per round in a uniform, fully unrolled pass (all lanes busy, shared-
 // memory latencies overlapped) and left in shared memory as packed descriptors {j | jend << 16,
-// ja | jb << 16} in staged-record units.  (In v3 every lane derived its next run inside the atom
-// loop: a divergent, two-LDS-deep row change on nearly every warp iteration, as costly as the FMAs;
-// profiles/r1c.)
-__device__ __forceinline__ void build_runs(uint2* runs, const int NT, const int r_beg, const int r_hi, const int* Lp,
-                                           const int NB, const int* ro, const int a0, const int a1) {
+// ja | jb << 16} in staged-record units; EMPTY RUNS ARE DROPPED, so the atom loop can switch runs
+// with a handful of predicated instructions instead of a divergent search for the next non-empty
+// one (v4 spent a third of its warp instructions there; profiles/r1f).  Returns the thread's atom
+// count of the round.
+__device__ __forceinline__ int build_runs(uint2* runs, const int NT, const int r_beg, const int r_hi, const int* Lp,
+                                          const int NB, const int* ro, const int a0, const int a1) {
+  int total = 0;
+  uint2* out = runs;
 #pragma unroll
   for (int i = 0; i < SW; ++i) {
     const int rr = r_beg + i;
@@ -234,68 +255,105 @@ __device__ __forceinline__ void build_runs(uint2* runs, const int NT, const int 
       const int2 b = *reinterpret_cast<const int2*>(Lp + rr * NB + SW);
       const int off = ro[rr] - a0;      // staged position of the row's atom 0
       const int j = off + max(a.x, a0);
-      const int jend = max(j, off + min(b.y, a1));
+      const int jend = off + min(b.y, a1);
       const int ja = min(max(off + a.y, 0), 0xffff);
       const int jb = min(max(off + b.x, 0), 0xffff);
-      runs[i * NT] = make_uint2((unsigned)j | ((unsigned)jend << 16), (unsigned)ja | ((unsigned)jb << 16));
+      if (jend > j) {
+        *out = make_uint2((unsigned)j | ((unsigned)jend << 16), (unsigned)ja | ((unsigned)jb << 16));
+        out += NT;
+        total += jend - j;
+      }
     }
   }
+  return total;
 }
 
+// shared-memory loads by 32-bit shared-space address (keeps the address arithmetic of the atom loop at
+// one IMAD and three adds per visit)
+__device__ __forceinline__ ulonglong2 lds_u64x2(uint32_t a) {
+  ulonglong2 v;
+  asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ f32x2 lds_u64(uint32_t a) {
+  f32x2 v;
+  asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float lds_f32(uint32_t a) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint2 lds_u32x2(uint32_t a) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+  return v;
+}
+
+// The atom loop: one trip per (atom, thread) visit, `total` trips, all bookkeeping branch-free.
+//  * v[u][c] = wy * wz[u] * q[c] as packed pairs over the two columns (FMUL2), the 32 accumulations as
+//    FFMA2 {plane k, plane k+1} += {wx[k], wx[k+1]} * v (broadcast operand form): 37 FMA-pipe
+//    instructions for 64 multiply-adds;
+//  * the next run's descriptor is fetched a run ahead; the switch is a few predicated instructions.
 template <int CB>
-__device__ __forceinline__ void walk_atoms(f32x2 (&acc)[SW / 2][2][CB], const uint2* runs, const int NT, const int nrows,
+__device__ __forceinline__ void walk_atoms(f32x2 (&acc)[SW / 2][2][CB], const uint2* runs, const int NT, const int total,
                                            const float* rbase, const int recf, const int cb0, const int oy,
                                            const int oz) {
   // loop invariants pinned to registers (ptxas otherwise reloads the kernel parameters from the
-  // constant bank inside the atom loop, a uniform-load latency per iteration)
-  // (a shuffle result cannot be rematerialised from the constant bank, an empty asm can)
-  const int recf_r = __shfl_sync(0xffffffffu, recf, 0), cb0_r = __shfl_sync(0xffffffffu, cb0, 0);
-  int j = 0, jend = 0, ja = 0, jb = 0;
-  int k = 0;                     // descriptors fetched so far
-  uint2 nd = make_uint2(0u, 0u);
-  if (nrows > 0) { nd = runs[0]; k = 1; }
-  bool pending = nrows > 0;
-  for (;;) {
-    // row change (divergent, but register-only: the next descriptor was fetched a run ago); the lanes
-    // reconverge before the atom body
-    while (j >= jend && pending) {
+  // constant bank inside the atom loop; a shuffle result cannot be rematerialised from there)
+  const uint32_t recB = 4u * (uint32_t)__shfl_sync(0xffffffffu, recf, 0);
+  const uint32_t sb = smem_u32(rbase);
+  const uint32_t qB = 4u * (3 * SW + (uint32_t)__shfl_sync(0xffffffffu, cb0, 0)), yB = 4u * oy, zB = 4u * oz;
+  uint32_t nrun = smem_u32(runs);
+  const uint32_t runB = 8u * NT;
+  uint2 nd = lds_u32x2(nrun);
+  int j = (int)(nd.x & 0xffffu), jend = (int)(nd.x >> 16), ja = (int)(nd.y & 0xffffu), jb = (int)(nd.y >> 16);
+  nrun += runB;
+  nd = lds_u32x2(nrun);          // (past the thread's last run: stale but in-bounds, never used)
+#pragma unroll 1
+  for (int t = total; t > 0; --t) {
+    const uint32_t a = sb + (uint32_t)j * recB;
+    const ulonglong2 wa = lds_u64x2(a);        // {wx0,wx1}, {wx2,wx3}
+    const ulonglong2 wb = lds_u64x2(a + 16);   // {wx4,wx5}, {wx6,wx7}
+    const float wyv = lds_f32(a + yB);
+    const f32x2 wz2 = lds_u64(a + zB);
+    f32x2 q01 = 0ull, q23 = 0ull;
+    float qv[4];
+    if constexpr (CB >= 3) {
+      const ulonglong2 tq = lds_u64x2(a + qB);
+      q01 = tq.x; q23 = tq.y;
+    } else if constexpr (CB == 2) {
+      q01 = lds_u64(a + qB);
+    } else {
+      q01 = pack2(lds_f32(a + qB), 0.f);
+    }
+    unpack2(q01, qv[0], qv[1]);
+    unpack2(q23, qv[2], qv[3]);
+    float p0, p1;
+    unpack2(fmul2(wz2, pack2(wyv, wyv)), p0, p1);
+    p0 = j < jb ? p0 : 0.f;
+    p1 = j >= ja ? p1 : 0.f;
+    ++j;
+    if (j == jend) {             // next run (if-converted: no divergence)
       j = (int)(nd.x & 0xffffu); jend = (int)(nd.x >> 16);
       ja = (int)(nd.y & 0xffffu); jb = (int)(nd.y >> 16);
-      pending = k < nrows;
-      if (pending) { nd = runs[k * NT]; ++k; }
+      nrun += runB;
+      nd = lds_u32x2(nrun);
     }
-    if (j >= jend) break;
-    const float* rp = rbase + j * recf_r;
-    const float4 wa = *reinterpret_cast<const float4*>(rp);
-    const float4 wb = *reinterpret_cast<const float4*>(rp + 4);
-    float qv[CB];
-    if constexpr (CB >= 3) {
-      const float4 t = *reinterpret_cast<const float4*>(rp + 3 * SW + cb0_r);
-      qv[0] = t.x; qv[1] = t.y; qv[2] = t.z;
-      if constexpr (CB == 4) qv[3] = t.w;
-    } else if constexpr (CB == 2) {
-      const float2 t = *reinterpret_cast<const float2*>(rp + 3 * SW + cb0_r);
-      qv[0] = t.x; qv[1] = t.y;
-    } else {
-      qv[0] = rp[3 * SW + cb0_r];
-    }
-    const float wyv = rp[oy];
-    const float2 wzv = *reinterpret_cast<const float2*>(rp + oz);
-    const float p0 = j < jb ? wyv * wzv.x : 0.f;
-    const float p1 = j >= ja ? wyv * wzv.y : 0.f;
-    // x pairs (k, k+1) share one FFMA2: acc[k/2] = {plane k, plane k+1} += {wx[k], wx[k+1]} * {v, v}
-    const f32x2 wx[SW / 2] = {pack2(wa.x, wa.y), pack2(wa.z, wa.w), pack2(wb.x, wb.y), pack2(wb.z, wb.w)};
+    const f32x2 wx[SW / 2] = {wa.x, wa.y, wb.x, wb.y};
 #pragma unroll
     for (int c = 0; c < CB; ++c) {
+      // scalar products on purpose: with FMUL2 pairs here ptxas overlays eight accumulator pairs on the
+      // dying 64-bit temporaries and copies them back every visit (16 IMAD.MOV per trip)
       const float v0 = p0 * qv[c], v1 = p1 * qv[c];
       const f32x2 d0 = pack2(v0, v0), d1 = pack2(v1, v1);
 #pragma unroll
       for (int k2 = 0; k2 < SW / 2; ++k2) {
-        acc[k2][0][c] = ffma2(wx[k2], d0, acc[k2][0][c]);
-        acc[k2][1][c] = ffma2(wx[k2], d1, acc[k2][1][c]);
+        ffma2_acc(acc[k2][0][c], wx[k2], d0);
+        ffma2_acc(acc[k2][1][c], wx[k2], d1);
       }
     }
-    ++j;
   }
 }
 
@@ -489,8 +547,9 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
       const int tb = d.p % NTAB;
       const int r_beg = max(rlo, d.r0);
       const int r_hi = lane_ok ? min(rlo + SW, d.r1) : r_beg;
-      build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32, d.a0, d.a1);
-      walk_atoms<CB>(acc, s_run, NT, r_hi - r_beg, s_rec + (size_t)cur * cap * recf, recf, cb0, oy, oz);
+      const int total =
+          build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32, d.a0, d.a1);
+      walk_atoms<CB>(acc, s_run, NT, total, s_rec + (size_t)cur * cap * recf, recf, cb0, oy, oz);
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[cur]);   // this warp is done with the staged records and the round's offsets
@@ -513,8 +572,8 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer
       const float s0 = (K & 1) ? a1 : a0, s1 = (K & 1) ? b1 : b0;                              \
       if (shared) red_add_v2(gp + (size_t)c * Mtot, s0, s1);                                   \
       else *reinterpret_cast<float2*>(gp + (size_t)c * Mtot) = make_float2(s0, s1);            \
-      acc[K / 2][0][c] = (K & 1) ? pack2(a0, 0.f) : pack2(0.f, a1);                            \
-      acc[K / 2][1][c] = (K & 1) ? pack2(b0, 0.f) : pack2(0.f, b1);                            \
+      if (K & 1) { zero_hi(acc[K / 2][0][c]); zero_hi(acc[K / 2][1][c]); }                     \
+      else { zero_lo(acc[K / 2][0][c]); zero_lo(acc[K / 2][1][c]); }                           \
     }                                                                                          \
     break;
           PSWF_FLUSH(0) PSWF_FLUSH(1) PSWF_FLUSH(2) PSWF_FLUSH(3)
