@@ -292,10 +292,13 @@ __device__ __forceinline__ uint2 lds_u32x2(uint32_t a) {
 }
 
 // The atom loop: one trip per (atom, thread) visit, `total` trips, all bookkeeping branch-free.
-//  * v[u][c] = wy * wz[u] * q[c] as packed pairs over the two columns (FMUL2), the 32 accumulations as
-//    FFMA2 {plane k, plane k+1} += {wx[k], wx[k+1]} * v (broadcast operand form): 37 FMA-pipe
-//    instructions for 64 multiply-adds;
-//  * the next run's descriptor is fetched a run ahead; the switch is a few predicated instructions.
+//  * p[u] = wy * wz[u] by one FMUL2, v[u][c] = p[u] * q[c], the 32 accumulations as FFMA2
+//    {plane k, plane k+1} += {wx[k], wx[k+1]} * v (broadcast operand form);
+//  * the next run's descriptor is fetched a run ahead; the switch is a few predicated instructions;
+//  * SOFTWARE PIPELINED: the thread-specific words of the NEXT visit (wy, wz pair, charges) are
+//    requested before the current visit's FFMA2 block, so the LDS -> FMUL2 -> FSEL -> FMUL chain that
+//    feeds the first FFMA2 no longer waits for shared memory (30% of the loop's stall samples in
+//    profiles/r2a).
 template <int CB>
 __device__ __forceinline__ void walk_atoms(f32x2 (&acc)[SW / 2][2][CB], const uint2* runs, const int NT, const int total,
                                            const float* rbase, const int recf, const int cb0, const int oy,
@@ -305,35 +308,46 @@ __device__ __forceinline__ void walk_atoms(f32x2 (&acc)[SW / 2][2][CB], const ui
   const uint32_t recB = 4u * (uint32_t)__shfl_sync(0xffffffffu, recf, 0);
   const uint32_t sb = smem_u32(rbase);
   const uint32_t qB = 4u * (3 * SW + (uint32_t)__shfl_sync(0xffffffffu, cb0, 0)), yB = 4u * oy, zB = 4u * oz;
+  if (total <= 0) return;
   uint32_t nrun = smem_u32(runs);
   const uint32_t runB = 8u * NT;
   uint2 nd = lds_u32x2(nrun);
   int j = (int)(nd.x & 0xffffu), jend = (int)(nd.x >> 16), ja = (int)(nd.y & 0xffffu), jb = (int)(nd.y >> 16);
   nrun += runB;
   nd = lds_u32x2(nrun);          // (past the thread's last run: stale but in-bounds, never used)
-#pragma unroll 1
-  for (int t = total; t > 0; --t) {
-    const uint32_t a = sb + (uint32_t)j * recB;
-    const ulonglong2 wa = lds_u64x2(a);        // {wx0,wx1}, {wx2,wx3}
-    const ulonglong2 wb = lds_u64x2(a + 16);   // {wx4,wx5}, {wx6,wx7}
-    const float wyv = lds_f32(a + yB);
-    const f32x2 wz2 = lds_u64(a + zB);
-    f32x2 q01 = 0ull, q23 = 0ull;
-    float qv[4];
+  uint32_t a = sb + (uint32_t)j * recB;
+  float wyv = lds_f32(a + yB);
+  f32x2 wz2 = lds_u64(a + zB);
+  f32x2 q01 = 0ull, q23 = 0ull;
+  auto load_q = [&](uint32_t at) {
     if constexpr (CB >= 3) {
-      const ulonglong2 tq = lds_u64x2(a + qB);
+      const ulonglong2 tq = lds_u64x2(at + qB);
       q01 = tq.x; q23 = tq.y;
     } else if constexpr (CB == 2) {
-      q01 = lds_u64(a + qB);
+      q01 = lds_u64(at + qB);
     } else {
-      q01 = pack2(lds_f32(a + qB), 0.f);
+      q01 = pack2(lds_f32(at + qB), 0.f);
     }
+  };
+  load_q(a);
+  int t = total;
+  bool more;
+#pragma unroll 1
+  do {
+    const ulonglong2 wa = lds_u64x2(a);        // {wx0,wx1}, {wx2,wx3}
+    const ulonglong2 wb = lds_u64x2(a + 16);   // {wx4,wx5}, {wx6,wx7}
+    float qv[4];
     unpack2(q01, qv[0], qv[1]);
     unpack2(q23, qv[2], qv[3]);
     float p0, p1;
     unpack2(fmul2(wz2, pack2(wyv, wyv)), p0, p1);
     p0 = j < jb ? p0 : 0.f;
     p1 = j >= ja ? p1 : 0.f;
+    float v0[CB], v1[CB];
+    // scalar products on purpose: with FMUL2 pairs here ptxas overlays eight accumulator pairs on the
+    // dying 64-bit temporaries and copies them back every visit (16 IMAD.MOV per trip)
+#pragma unroll
+    for (int c = 0; c < CB; ++c) { v0[c] = p0 * qv[c]; v1[c] = p1 * qv[c]; }
     ++j;
     if (j == jend) {             // next run (if-converted: no divergence)
       j = (int)(nd.x & 0xffffu); jend = (int)(nd.x >> 16);
@@ -341,24 +355,31 @@ __device__ __forceinline__ void walk_atoms(f32x2 (&acc)[SW / 2][2][CB], const ui
       nrun += runB;
       nd = lds_u32x2(nrun);
     }
+    more = --t > 0;
+    if (more) {                  // the next visit's words (after the last visit j is stale: no load)
+      a = sb + (uint32_t)j * recB;
+      wyv = lds_f32(a + yB);
+      wz2 = lds_u64(a + zB);
+      load_q(a);
+    }
     const f32x2 wx[SW / 2] = {wa.x, wa.y, wb.x, wb.y};
 #pragma unroll
     for (int c = 0; c < CB; ++c) {
-      // scalar products on purpose: with FMUL2 pairs here ptxas overlays eight accumulator pairs on the
-      // dying 64-bit temporaries and copies them back every visit (16 IMAD.MOV per trip)
-      const float v0 = p0 * qv[c], v1 = p1 * qv[c];
-      const f32x2 d0 = pack2(v0, v0), d1 = pack2(v1, v1);
+      const f32x2 d0 = pack2(v0[c], v0[c]), d1 = pack2(v1[c], v1[c]);
 #pragma unroll
       for (int k2 = 0; k2 < SW / 2; ++k2) {
         ffma2_acc(acc[k2][0][c], wx[k2], d0);
         ffma2_acc(acc[k2][1][c], wx[k2], d1);
       }
     }
-  }
+  } while (more);
 }
 
 template <int WY, int WZ, int CB, int NCTA>
-__global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)   // WY x WZ consumer warps + one producer warp
+// WY x WZ consumer warps + one producer warp.  (Stating the cap as __maxnreg__(136) removes ptxas's
+// register-saving copies in the atom loop, but 136 registers x 160 threads run as TWO CTAs per SM:
+// 353 us against 300 us.)
+__global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
     k_spread_os(int Mx, int My, int Mz, int nseg, int npy, int npz, int cap, int recf, int cb0,
                 const int* __restrict__ start, const float* __restrict__ rec, float* __restrict__ grid) {
   using S = SpreadShape<WY, WZ>;
