@@ -68,6 +68,9 @@ typedef struct {
   int host_only;    /* 1: build the host-side tables only (no device is touched); such a plan serves    */
                     /* pswf_lr_get_info / pswf_lr_eval_window / pswf_lr_eval_kernel and every compute    */
                     /* call on it fails with PSWF_LR_ERR_CUDA.  Not a CPU fallback.                      */
+  int debug_spectrum; /* test hook: 1 keeps a dense copy of the scaled half spectrum for                 */
+                    /* pswf_lr_debug_copy(what = 1) when the band-limited transform path is active      */
+                    /* (that path never materialises the dense spectrum otherwise).                     */
 } pswf_lr_opts;
 
 /* Read-back of what the plan resolved (all host values). */
@@ -80,6 +83,11 @@ typedef struct {
   int kernel_panels;
   long long modes_in_ball;    /* half-spectrum modes with a non-zero multiplier          */
   long long workspace_bytes;  /* device memory owned by the plan                         */
+  int fast_stencil;      /* 1: the cell-sorted fp32 spread / gather kernels run (fp32, w <= 8, M_d a     */
+                         /*    multiple of 8 and >= 16, kernel_path = 0); 0: the one-warp-per-atom ones  */
+  int band_limited_fft;  /* 1: z transforms + fused (x,y) transform / scale kernel (fp32, Mx and My      */
+                         /*    powers of two <= 256, kernel_path = 0, virial off); 0: dense 3-D cuFFT    */
+  int band_kmax[3];      /* band-limited path: kept DFT indices |m_d| <= band_kmax[d]                    */
 } pswf_lr_info;
 
 /* Create a plan.  box[3]: edge lengths; grid[3]: M_x,M_y,M_z (each >= w, product < 2^31);

@@ -30,7 +30,7 @@ class PswfLrError(RuntimeError):
 class Opts(ctypes.Structure):
     _fields_ = [("r_c", ctypes.c_double), ("c_window", ctypes.c_double), ("precision", ctypes.c_int),
                 ("max_atoms", ctypes.c_int), ("zero_mode", ctypes.c_int), ("kernel_path", ctypes.c_int),
-                ("poly_eps", ctypes.c_double), ("host_only", ctypes.c_int)]
+                ("poly_eps", ctypes.c_double), ("host_only", ctypes.c_int), ("debug_spectrum", ctypes.c_int)]
 
 
 class Info(ctypes.Structure):
@@ -39,7 +39,8 @@ class Info(ctypes.Structure):
                 ("n_channels", ctypes.c_int), ("n_distinct_p", ctypes.c_int), ("grid", ctypes.c_int * 3),
                 ("window_degree", ctypes.c_int), ("kernel_degree", ctypes.c_int),
                 ("kernel_panels", ctypes.c_int), ("modes_in_ball", ctypes.c_longlong),
-                ("workspace_bytes", ctypes.c_longlong)]
+                ("workspace_bytes", ctypes.c_longlong), ("fast_stencil", ctypes.c_int),
+                ("band_limited_fft", ctypes.c_int), ("band_kmax", ctypes.c_int * 3)]
 
 
 EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_execute", "pswf_lr_execute_host",
@@ -119,12 +120,12 @@ class Plan:
     """pswf_lr_plan_create_ex / pswf_lr_execute / pswf_lr_destroy."""
 
     def __init__(self, box, grid, w, c, exponents, r_c=0.0, c_window=0.0, precision="f32", max_atoms=0,
-                 zero_mode=0, kernel_path=0, poly_eps=0.0, host_only=False):
+                 zero_mode=0, kernel_path=0, poly_eps=0.0, host_only=False, debug_spectrum=False):
         self._h = ctypes.c_void_p()
         L = lib()
         self.precision = {"f32": PSWF_LR_F32, "f64": PSWF_LR_F64}[precision]
         o = Opts(r_c, c_window, self.precision, int(max_atoms), zero_mode, kernel_path, poly_eps,
-                 1 if host_only else 0)
+                 1 if host_only else 0, 1 if debug_spectrum else 0)
         box_a = (ctypes.c_double * 3)(*[float(b) for b in box])
         grid_a = (ctypes.c_int * 3)(*[int(g) for g in grid])
         ex = (ctypes.c_int * len(exponents))(*[int(p) for p in exponents])
@@ -155,8 +156,9 @@ class Plan:
     def info(self):
         i = Info()
         _check(lib().pswf_lr_get_info(self._h, ctypes.byref(i)))
-        d = {k: getattr(i, k) for k, _ in Info._fields_ if k != "grid"}
+        d = {k: getattr(i, k) for k, _ in Info._fields_ if k not in ("grid", "band_kmax")}
         d["grid"] = list(i.grid)
+        d["band_kmax"] = list(i.band_kmax)
         return d
 
     def eval_window(self, z):

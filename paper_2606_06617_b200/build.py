@@ -8,8 +8,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["pswf_lr.cu", "kernels_generic.cu", "kernels_stencil.cu", "kernels_gather.cu", "kernels_real.cu"]
-HEADERS = ["plan.hpp", "launch.hpp", "host_tables.hpp", "real_tables.hpp", "kernels_common.cuh",
+SOURCES = ["pswf_lr.cu", "kernels_generic.cu", "kernels_stencil.cu", "kernels_gather.cu", "kernels_fft.cu", "kernels_real.cu"]
+HEADERS = ["plan.hpp", "launch.hpp", "host_tables.hpp", "real_tables.hpp", "kernels_common.cuh", "kernels_scale.cuh",
            os.path.join("..", "..", "include", "pswf_lr.h")]
 LIB = os.path.join(HERE, "libpswf_lr.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")

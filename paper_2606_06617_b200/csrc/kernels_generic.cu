@@ -5,6 +5,7 @@
 // kernels in kernels_stencil.cu / kernels_gather.cu replace sort-scatter, spread and gather on the
 // default path.
 #include "kernels_common.cuh"
+#include "kernels_scale.cuh"
 #include "launch.hpp"
 
 namespace pswf {
@@ -185,55 +186,7 @@ __global__ void k_spread_ref(int n, int C, int cap, GridGeom<T> g, const int* __
 // Phi^_p is evaluated once per distinct exponent per mode by Horner on the smooth part
 // and reused by every channel with that exponent.
 // ------------------------------------------------------------------------------------------------
-template <class T>
-struct Cplx { T x, y; };
-
-template <class T>
-__device__ __forceinline__ T kernel_value(const ScaleParams<T>& P, int slot, T x, T kappa) {
-  // x = kappa / c in (0,1)
-  int j = min((int)(x * (T)P.panels), P.panels - 1);
-  T xi = (T)2 * (x * (T)P.panels - (T)j) - (T)1;
-  const T* cf = P.kcoef + ((size_t)slot * P.panels + j) * (P.degree + 1);
-  T t = cf[P.degree];
-  for (int m = P.degree - 1; m >= 0; --m) t = fma(t, xi, cf[m]);
-  T s;
-  switch (P.slot_p[slot]) {
-    case 1: s = t / (kappa * kappa); break;            // x 4 pi r_c^2      (S47)
-    case 2: s = t / kappa; break;                      // x 2 pi^2 r_c      (S48)
-    case 3: s = t - log(x); break;                     // x 4 pi            (S49)
-    case 4: s = t; break;                              // x pi^2 c / r_c    (S50)
-    case 5: s = t + x * x * log(x); break;             // x 2 pi c^2/(3 r_c^2)  (S51)
-    default: s = t; break;                             // x pi^2 c^3/(12 r_c^3) (S52)
-  }
-  return s * P.slot_pre[slot];
-}
-
-// d Phi^_p / dk by the derivative of the SAME panel polynomial plus the derivative of the bare factor
-// (virial).  x = kappa / c, kappa = k r_c, dx/dk = x_per_k, dkappa/dk = c x_per_k.
-template <class T>
-__device__ __forceinline__ T kernel_dvalue(const ScaleParams<T>& P, int slot, T x, T kappa) {
-  int j = min((int)(x * (T)P.panels), P.panels - 1);
-  T xi = (T)2 * (x * (T)P.panels - (T)j) - (T)1;
-  const T* cf = P.kcoef + ((size_t)slot * P.panels + j) * (P.degree + 1);
-  T t = cf[P.degree], dt = (T)P.degree * cf[P.degree];
-  for (int m = P.degree - 1; m >= 1; --m) {
-    t = fma(t, xi, cf[m]);
-    dt = fma(dt, xi, (T)m * cf[m]);
-  }
-  t = fma(t, xi, cf[0]);
-  dt *= (T)2 * (T)P.panels;            // dT/dx
-  const T rc = P.c * P.x_per_k;
-  T ds;
-  switch (P.slot_p[slot]) {
-    case 1: ds = dt * P.x_per_k / (kappa * kappa) - (T)2 * t * rc / (kappa * kappa * kappa); break;
-    case 2: ds = dt * P.x_per_k / kappa - t * rc / (kappa * kappa); break;
-    case 3: ds = (dt - (T)1 / x) * P.x_per_k; break;
-    case 5: ds = (dt + (T)2 * x * log(x) + x) * P.x_per_k; break;
-    default: ds = dt * P.x_per_k; break;
-  }
-  return ds * P.slot_pre[slot];
-}
-
+// (Cplx, kernel_value, kernel_dvalue: kernels_scale.cuh)
 // VIR: also accumulate the virial W_ab = 1/2 sum_m' |rho^|^2 [D delta_ab + (dD/dk) k_a k_b / |k|] of the
 // discrete energy (its exact strain derivative: the window transform depends on k h only, which a
 // homogeneous strain leaves unchanged) into Wacc[6] = xx, yy, zz, xy, xz, yz.

@@ -27,6 +27,14 @@ void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const floa
                             cudaStream_t st);
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st);
 
+// band-limited transform path (kernels_fft.cu)
+bool fused_fft_supported(const pswf_lr_plan* p);
+void fused_fft_limits(const pswf_lr_plan* p, int kmax[3]);
+void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t st);
+bool fused_z_supported(const pswf_lr_plan* p);   // own z transforms (power-of-two Mz); else cuFFT along z
+void launch_z_forward(pswf_lr_plan* p, cudaStream_t st);
+void launch_z_inverse(pswf_lr_plan* p, cudaStream_t st);
+
 // real-space complement + self term (kernels_real.cu); uses the sort left by launch_bin_sort(scatter = true)
 template <class T>
 void launch_real_space(pswf_lr_plan* p, int n, const T* pos, const RealGeom<T>& g, const RealParams<T>& P, double* E,

@@ -139,6 +139,14 @@ struct pswf_lr_plan {
   // cuFFT
   cufftHandle fft_fwd = 0, fft_inv = 0;
   bool have_fft = false;
+  // band-limited transform path (kernels_fft.cu): z transforms with plane-major spectra + k_xy_scale
+  bool fused_fft = false;
+  bool fused_z = false;           // z transforms by k_z_forward / k_z_inverse instead of cuFFT
+  int fused_kmax[3] = {0, 0, 0};  // kept signed DFT indices per dimension: |f| <= kmax (never Nyquist)
+  cufftHandle fft_zf = 0, fft_zi = 0;
+  void* d_spec2 = nullptr;        // cplx [Mz/2+1][C][Mx][My]; planes beyond the band stay zero
+  bool debug_dump_spectrum = false;
+  void* d_spec_dump = nullptr;    // cplx [C][Mx][My][Mz/2+1] dense copy of the scaled modes (test hook)
   // profiling
   bool profiling = false;
   std::vector<cudaEvent_t> events;  // kProfileRing * (N_STAGES + 1)

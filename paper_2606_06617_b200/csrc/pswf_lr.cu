@@ -180,26 +180,49 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   }
   if (!stencil) launch_spread_ref<T>(p, n, g, st);
   if (ev) cudaEventRecord(ev[2], st);
-  // a2
-  CUFFT_TRY(cufftSetStream(p->fft_fwd, st));
-  if (sizeof(T) == 4)
-    CUFFT_TRY(cufftExecR2C(p->fft_fwd, (cufftReal*)p->d_grid, (cufftComplex*)p->d_spec));
-  else
-    CUFFT_TRY(cufftExecD2Z(p->fft_fwd, (cufftDoubleReal*)p->d_grid, (cufftDoubleComplex*)p->d_spec));
+  // a2-a4.  Band-limited path: R2C along z (plane-major spectrum), then per kept (k_z, channel) plane
+  // forward (x,y) transform, multiply + energy, inverse (x,y) transform in one kernel, then C2R along z.
+  const bool fused = kIsF32 && p->fused_fft && !p->virial;
+  if (fused) {
+    if (p->fused_z) {
+      launch_z_forward(p, st);
+    } else {
+      CUFFT_TRY(cufftSetStream(p->fft_zf, st));
+      CUFFT_TRY(cufftExecR2C(p->fft_zf, (cufftReal*)p->d_grid, (cufftComplex*)p->d_spec));
+    }
+  } else {
+    CUFFT_TRY(cufftSetStream(p->fft_fwd, st));
+    if (sizeof(T) == 4)
+      CUFFT_TRY(cufftExecR2C(p->fft_fwd, (cufftReal*)p->d_grid, (cufftComplex*)p->d_spec));
+    else
+      CUFFT_TRY(cufftExecD2Z(p->fft_fwd, (cufftDoubleReal*)p->d_grid, (cufftDoubleComplex*)p->d_spec));
+  }
   if (ev) cudaEventRecord(ev[3], st);
   // a3
   cudaMemsetAsync(p->d_Ech, 0, sizeof(double) * p->C, st);
   if (p->virial) cudaMemsetAsync(p->d_virial, 0, sizeof(double) * 6, st);
-  launch_scale<T>(p, P, true, st);
+  if constexpr (kIsF32) {
+    if (fused) launch_xy_scale(p, P, st);
+  }
+  if (!fused) launch_scale<T>(p, P, true, st);
   if (E) launch_finalize_energy(p, E, st);
   if (ev) cudaEventRecord(ev[4], st);
   if (phi || F) {
     // a4
-    CUFFT_TRY(cufftSetStream(p->fft_inv, st));
-    if (sizeof(T) == 4)
-      CUFFT_TRY(cufftExecC2R(p->fft_inv, (cufftComplex*)p->d_spec, (cufftReal*)p->d_grid));
-    else
-      CUFFT_TRY(cufftExecZ2D(p->fft_inv, (cufftDoubleComplex*)p->d_spec, (cufftDoubleReal*)p->d_grid));
+    if (fused) {
+      if (p->fused_z) {
+        launch_z_inverse(p, st);
+      } else {
+        CUFFT_TRY(cufftSetStream(p->fft_zi, st));
+        CUFFT_TRY(cufftExecC2R(p->fft_zi, (cufftComplex*)p->d_spec2, (cufftReal*)p->d_grid));
+      }
+    } else {
+      CUFFT_TRY(cufftSetStream(p->fft_inv, st));
+      if (sizeof(T) == 4)
+        CUFFT_TRY(cufftExecC2R(p->fft_inv, (cufftComplex*)p->d_spec, (cufftReal*)p->d_grid));
+      else
+        CUFFT_TRY(cufftExecZ2D(p->fft_inv, (cufftDoubleComplex*)p->d_spec, (cufftDoubleReal*)p->d_grid));
+    }
     if (ev) cudaEventRecord(ev[5], st);
     // a5
     if constexpr (kIsF32) {
@@ -469,6 +492,30 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
                                    p->C, &ws) != CUFFT_SUCCESS)
         rc = PSWF_LR_ERR_CUFFT;
       p->workspace_bytes += (long long)ws;
+      // band-limited path: 1-D transforms along z whose complex side is plane-major [kz][c][x][y]
+      p->fused_fft = !rc && p->kernel_path == 0 && fused_fft_supported(p);
+      if (p->fused_fft) {
+        fused_fft_limits(p, p->fused_kmax);
+        p->fused_z = fused_z_supported(p);
+        const int batch = p->C * p->M[0] * p->M[1];
+        int nz[1] = {p->M[2]}, re[1] = {p->M[2]}, ce[1] = {p->M[2] / 2 + 1};
+        long long b2 = 0;
+        const size_t Mhalf = (size_t)p->M[0] * p->M[1] * (p->M[2] / 2 + 1);
+        if (cufftCreate(&p->fft_zf) != CUFFT_SUCCESS || cufftCreate(&p->fft_zi) != CUFFT_SUCCESS) rc = PSWF_LR_ERR_CUFFT;
+        if (!rc && cufftMakePlanMany(p->fft_zf, 1, nz, re, 1, p->M[2], ce, batch, 1, CUFFT_R2C, batch, &ws) !=
+                       CUFFT_SUCCESS)
+          rc = PSWF_LR_ERR_CUFFT;
+        p->workspace_bytes += (long long)ws;
+        if (!rc && cufftMakePlanMany(p->fft_zi, 1, nz, ce, batch, 1, re, 1, p->M[2], CUFFT_C2R, batch, &ws) !=
+                       CUFFT_SUCCESS)
+          rc = PSWF_LR_ERR_CUFFT;
+        p->workspace_bytes += (long long)ws;
+        if (!rc) rc = dev_alloc(&p->d_spec2, 2 * sizeof(float) * Mhalf * p->C, &b2);
+        if (!rc && cudaMemset(p->d_spec2, 0, 2 * sizeof(float) * Mhalf * p->C) != cudaSuccess) rc = PSWF_LR_ERR_CUDA;
+        p->debug_dump_spectrum = o.debug_spectrum != 0;
+        if (!rc && p->debug_dump_spectrum) rc = dev_alloc(&p->d_spec_dump, 2 * sizeof(float) * Mhalf * p->C, &b2);
+        p->workspace_bytes += b2;
+      }
     }
     if (!rc && !p->host_only) rc = ensure_capacity(p, o.max_atoms > 0 ? o.max_atoms : 1024);
   } catch (const std::bad_alloc&) {
@@ -619,6 +666,9 @@ int pswf_lr_get_info(const pswf_lr_plan* p, pswf_lr_info* info) {
   info->kernel_panels = p->kt.panels;
   info->modes_in_ball = p->modes_in_ball;
   info->workspace_bytes = p->workspace_bytes;
+  info->fast_stencil = (!p->host_only && p->kernel_path == 0 && stencil_path_supported(p)) ? 1 : 0;
+  info->band_limited_fft = (p->fused_fft && !p->virial) ? 1 : 0;
+  for (int d = 0; d < 3; ++d) info->band_kmax[d] = p->fused_kmax[d];
   return 0;
 }
 
@@ -668,6 +718,10 @@ int pswf_lr_debug_copy(pswf_lr_plan* p, int what, void* dst, void* stream) {
     nb = rs * Mtot * p->C;
   } else if (what == 1) {
     src = p->d_spec;
+    if (p->fused_fft && !p->virial) {   // the band-limited path keeps the dense spectrum only on request
+      if (!p->d_spec_dump) return PSWF_LR_ERR_INVALID_ARG;
+      src = p->d_spec_dump;
+    }
     nb = 2 * rs * Mhalf * p->C;
   } else {
     return PSWF_LR_ERR_INVALID_ARG;
@@ -766,12 +820,14 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   free_atoms(p);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
                   p->d_grid,  p->d_spec,    p->d_count,    p->d_scan_state, p->d_Ech,      p->d_Etot,
-                  p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal, p->d_virial};
+                  p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal, p->d_virial, p->d_spec2, p->d_spec_dump};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   if (p->have_fft) {
     if (p->fft_fwd) cufftDestroy(p->fft_fwd);
     if (p->fft_inv) cufftDestroy(p->fft_inv);
+    if (p->fft_zf) cufftDestroy(p->fft_zf);
+    if (p->fft_zi) cufftDestroy(p->fft_zi);
   }
   for (auto& e : p->events) cudaEventDestroy(e);
   delete p;
