@@ -28,7 +28,8 @@
  *   - Every function returns 0 on success or a negative pswf_lr_status; no exception crosses
  *     the ABI.  pswf_lr_error_string() names a code.
  *   - A plan is bound to the CUDA device current at creation and owns every workspace, table
- *     and cuFFT plan.  One plan must not be executed from two streams at once.
+ *     and cuFFT plan; calls made while another device is current switch to the plan's device and
+ *     restore the caller's afterwards.  One plan must not be executed from two streams at once.
  */
 #ifndef PSWF_LR_H
 #define PSWF_LR_H
@@ -47,7 +48,8 @@ typedef enum {
                                          /* transform would be used outside its band              */
   PSWF_LR_ERR_ALLOC = -4,
   PSWF_LR_ERR_CUDA = -5,
-  PSWF_LR_ERR_CUFFT = -6
+  PSWF_LR_ERR_CUFFT = -6,
+  PSWF_LR_ERR_BUSY = -7                  /* host submissions in flight: pswf_lr_wait_host first    */
 } pswf_lr_status;
 
 enum { PSWF_LR_F32 = 0, PSWF_LR_F64 = 1 };
@@ -118,6 +120,21 @@ int pswf_lr_execute(pswf_lr_plan* plan, int n_atoms, const void* pos, const void
  * returning.  This is the end-to-end entry point bench.py times as "e2e". */
 int pswf_lr_execute_host(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, double* E,
                          void* phi, void* F, void* stream);
+
+/* Pipelined form of pswf_lr_execute_host for streams of independent evaluations (batches of frames,
+ * ensemble members, or an MD loop whose next positions do not wait for these forces): submit enqueues
+ * the host->device copies, the evaluation and the device->host copies on three streams owned by the
+ * plan and returns at once; at most TWO submissions may be in flight (two staging slots), a third
+ * returns PSWF_LR_ERR_BUSY.  pswf_lr_wait_host blocks until the OLDEST outstanding submission has
+ * delivered E, phi and F to its host buffers.  With pinned host buffers the copy-in of submission
+ * k+1, the evaluation of k and the copy-out of k-1 overlap (PCIe is full duplex), so the sustained
+ * cost per evaluation is max(copy-in, evaluation, copy-out) instead of their sum.  Host buffers must
+ * stay valid and untouched until the matching wait returns.  Argument meaning as pswf_lr_execute_host
+ * (there is no stream argument: the plan's own streams are used).  Not to be mixed with
+ * pswf_lr_execute / pswf_lr_execute_host while submissions are in flight (PSWF_LR_ERR_BUSY). */
+int pswf_lr_submit_host(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, double* E,
+                        void* phi, void* F);
+int pswf_lr_wait_host(pswf_lr_plan* plan);
 
 /* Real-space complement and self term: the part of the full inverse-power
  * energy (S65), that the reciprocal path above does not contain,

@@ -44,6 +44,7 @@ class Info(ctypes.Structure):
 
 
 EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_execute", "pswf_lr_execute_host",
+           "pswf_lr_submit_host", "pswf_lr_wait_host",
            "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient", "pswf_lr_suggest_parameters", "pswf_lr_set_virial", "pswf_lr_virial",
            "pswf_lr_channel_energies", "pswf_lr_get_info", "pswf_lr_set_profiling", "pswf_lr_stage_ms",
            "pswf_lr_debug_copy", "pswf_lr_eval_window", "pswf_lr_eval_kernel", "pswf_lr_destroy",
@@ -207,6 +208,16 @@ class Plan:
             Ep = ctypes.cast(_ptr(E), ctypes.POINTER(ctypes.c_double))
         _check(lib().pswf_lr_execute_host(self._h, int(n_atoms), _ptr(pos), _ptr(q), Ep, _ptr(phi), _ptr(F),
                                           ctypes.c_void_p(stream or 0)))
+
+    def submit_host(self, n_atoms, pos, q, E=None, phi=None, F=None):
+        """Pipelined form of execute_host (at most two submissions in flight); see pswf_lr_submit_host."""
+        Ep = None
+        if E is not None:
+            Ep = ctypes.cast(_ptr(E), ctypes.POINTER(ctypes.c_double))
+        _check(lib().pswf_lr_submit_host(self._h, int(n_atoms), _ptr(pos), _ptr(q), Ep, _ptr(phi), _ptr(F)))
+
+    def wait_host(self):
+        _check(lib().pswf_lr_wait_host(self._h))
 
     def set_virial(self, enabled):
         _check(lib().pswf_lr_set_virial(self._h, 1 if enabled else 0))

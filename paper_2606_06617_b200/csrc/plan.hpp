@@ -94,6 +94,7 @@ struct pswf_lr_plan {
   double What0 = 0;               // W^(0) = prod_d omega_d lambda_0
   long long modes_in_ball = 0;
   long long workspace_bytes = 0;
+  long long atom_bytes = 0;       // part of workspace_bytes that scales with the atom capacity
   // host tables
   pswf::WindowTable wt;
   pswf::KernelTable kt;
@@ -120,7 +121,6 @@ struct pswf_lr_plan {
   unsigned long long* d_scan_state = nullptr;   // [1 + n_scan_blocks] ticket counter + tile states of the scan
   int n_scan_blocks = 0;
   double* d_Ech = nullptr;        // [C]
-  double* d_Etot = nullptr;       // [1] (execute_host staging)
   // per-atom workspaces (capacity cap_atoms)
   int cap_atoms = 0;
   int* d_key = nullptr;
@@ -131,10 +131,16 @@ struct pswf_lr_plan {
   void* d_sq = nullptr;           // real [C][cap]
   void* d_rec = nullptr;          // fast path: per-atom weight records
   void* d_drec = nullptr;         // fast path: per-atom derivative-weight records (gather)
-  void* d_pos_in = nullptr;       // execute_host staging
-  void* d_q_in = nullptr;
-  void* d_phi_out = nullptr;
-  void* d_F_out = nullptr;
+  // host-buffer entry points: two staging slots (slot 0 serves pswf_lr_execute_host; submit / wait
+  // alternate between both so that copy-in, evaluation and copy-out of consecutive submissions overlap)
+  void* d_pos_in[2] = {nullptr, nullptr};
+  void* d_q_in[2] = {nullptr, nullptr};
+  void* d_phi_out[2] = {nullptr, nullptr};
+  void* d_F_out[2] = {nullptr, nullptr};
+  double* d_E_out[2] = {nullptr, nullptr};
+  cudaStream_t s_in = nullptr, s_comp = nullptr, s_out = nullptr;
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+  long long n_submitted = 0, n_waited = 0;
   int last_n_atoms = 0;
   // cuFFT
   cufftHandle fft_fwd = 0, fft_inv = 0;

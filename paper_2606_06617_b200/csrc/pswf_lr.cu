@@ -23,6 +23,23 @@ using namespace pswf;
 
 namespace {
 
+// A plan is bound to the device current at its creation: every entry point that touches the device
+// switches to it for the call and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true, switched = false;
+  explicit DeviceGuard(const pswf_lr_plan* p) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != p->device) {
+      ok = cudaSetDevice(p->device) == cudaSuccess;
+      switched = ok;
+    }
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
 template <class T>
 int upload(void** dst, const std::vector<double>& src, long long* bytes) {
   std::vector<T> tmp(src.begin(), src.end());
@@ -47,8 +64,8 @@ int dev_alloc(void** ptr, size_t bytes, long long* total) {
 
 void free_atoms(pswf_lr_plan* p) {
   void** ptrs[] = {&p->d_spos, (void**)&p->d_key, (void**)&p->d_rank, (void**)&p->d_perm, (void**)&p->d_si0, &p->d_sdelta,
-                   &p->d_sq,          &p->d_rec,          &p->d_drec,         &p->d_pos_in,       &p->d_q_in,        &p->d_phi_out,
-                   &p->d_F_out};
+                   &p->d_sq,          &p->d_rec,          &p->d_drec,         &p->d_pos_in[0],    &p->d_q_in[0],     &p->d_phi_out[0],
+                   &p->d_F_out[0],    &p->d_pos_in[1],    &p->d_q_in[1],      &p->d_phi_out[1],   &p->d_F_out[1]};
   for (void** q : ptrs) {
     if (*q) cudaFree(*q);
     *q = nullptr;
@@ -60,6 +77,8 @@ int ensure_capacity(pswf_lr_plan* p, int n) {
   // growing: wait for everything in flight, then reallocate (documented in the header)
   if (cudaDeviceSynchronize() != cudaSuccess) return PSWF_LR_ERR_CUDA;
   free_atoms(p);
+  p->workspace_bytes -= p->atom_bytes;   // everything per-atom (staging slots included) was just released
+  p->atom_bytes = 0;
   int cap = std::max(n, std::max(p->cap_atoms * 2, 1024));
   const size_t rs = real_size(p);
   long long b = 0;
@@ -81,21 +100,25 @@ int ensure_capacity(pswf_lr_plan* p, int n) {
     return PSWF_LR_ERR_ALLOC;
   }
   p->workspace_bytes += b;
+  p->atom_bytes += b;
   return 0;
 }
 
-int ensure_host_staging(pswf_lr_plan* p) {
-  if (p->d_pos_in) return 0;
+int ensure_host_staging(pswf_lr_plan* p, int slots) {
   const size_t rs = real_size(p);
   long long b = 0;
   int rc = 0;
-  rc |= dev_alloc(&p->d_pos_in, rs * 3 * (size_t)p->cap_atoms, &b);
-  rc |= dev_alloc(&p->d_q_in, rs * (size_t)p->C * p->cap_atoms, &b);
-  rc |= dev_alloc(&p->d_phi_out, rs * (size_t)p->C * p->cap_atoms, &b);
-  rc |= dev_alloc(&p->d_F_out, rs * 3 * (size_t)p->cap_atoms, &b);
-  if (rc) return PSWF_LR_ERR_ALLOC;
+  for (int s = 0; s < slots; ++s) {
+    if (p->d_pos_in[s]) continue;
+    rc |= dev_alloc(&p->d_pos_in[s], rs * 3 * (size_t)p->cap_atoms, &b);
+    rc |= dev_alloc(&p->d_q_in[s], rs * (size_t)p->C * p->cap_atoms, &b);
+    rc |= dev_alloc(&p->d_phi_out[s], rs * (size_t)p->C * p->cap_atoms, &b);
+    rc |= dev_alloc(&p->d_F_out[s], rs * 3 * (size_t)p->cap_atoms, &b);
+    if (!p->d_E_out[s]) rc |= dev_alloc((void**)&p->d_E_out[s], sizeof(double), &b);
+  }
   p->workspace_bytes += b;
-  return 0;
+  p->atom_bytes += b;
+  return rc ? PSWF_LR_ERR_ALLOC : 0;
 }
 
 template <class T>
@@ -294,6 +317,7 @@ const char* pswf_lr_error_string(int code) {
     case PSWF_LR_ERR_ALLOC: return "device allocation failed";
     case PSWF_LR_ERR_CUDA: return "CUDA error (no usable device, or a kernel/launch failed)";
     case PSWF_LR_ERR_CUFFT: return "cuFFT error";
+    case PSWF_LR_ERR_BUSY: return "busy: host submissions in flight (call pswf_lr_wait_host first)";
   }
   return "unknown error";
 }
@@ -472,7 +496,6 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       p->n_scan_blocks = (int)((Mtot + 4095) / 4096);
       if (!rc) rc = dev_alloc((void**)&p->d_scan_state, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
-      if (!rc) rc = dev_alloc((void**)&p->d_Etot, sizeof(double), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ereal, sizeof(double), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_virial, sizeof(double) * 6, &b);
       p->workspace_bytes += b;
@@ -536,6 +559,8 @@ int pswf_lr_execute(pswf_lr_plan* p, int n_atoms, const void* pos, const void* q
   if (!p || n_atoms < 0) return PSWF_LR_ERR_INVALID_ARG;
   if (n_atoms > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
   if (p->host_only) return PSWF_LR_ERR_CUDA;  // a tables-only plan cannot execute
+  DeviceGuard guard(p);
+  if (!guard.ok) return PSWF_LR_ERR_CUDA;
   int rc = ensure_capacity(p, n_atoms);
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
@@ -550,24 +575,89 @@ int pswf_lr_execute_host(pswf_lr_plan* p, int n, const void* pos, const void* q,
   if (!p || n < 0) return PSWF_LR_ERR_INVALID_ARG;
   if (n > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
   if (p->host_only) return PSWF_LR_ERR_CUDA;
+  if (p->n_submitted != p->n_waited) return PSWF_LR_ERR_BUSY;
+  DeviceGuard guard(p);
+  if (!guard.ok) return PSWF_LR_ERR_CUDA;
   int rc = ensure_capacity(p, n);
   if (rc) return rc;
-  rc = ensure_host_staging(p);
+  rc = ensure_host_staging(p, 1);
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t rs = real_size(p);
   if (n > 0) {
-    CUDA_TRY(cudaMemcpyAsync(p->d_pos_in, pos, rs * 3 * (size_t)n, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(p->d_q_in, q, rs * (size_t)p->C * n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(p->d_pos_in[0], pos, rs * 3 * (size_t)n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(p->d_q_in[0], q, rs * (size_t)p->C * n, cudaMemcpyHostToDevice, st));
   }
-  rc = pswf_lr_execute(p, n, p->d_pos_in, p->d_q_in, E ? p->d_Etot : nullptr, phi ? p->d_phi_out : nullptr,
-                       F ? p->d_F_out : nullptr, stream);
+  rc = pswf_lr_execute(p, n, p->d_pos_in[0], p->d_q_in[0], E ? p->d_E_out[0] : nullptr,
+                       phi ? p->d_phi_out[0] : nullptr, F ? p->d_F_out[0] : nullptr, stream);
   if (rc) return rc;
-  if (E) CUDA_TRY(cudaMemcpyAsync(E, p->d_Etot, sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (E) CUDA_TRY(cudaMemcpyAsync(E, p->d_E_out[0], sizeof(double), cudaMemcpyDeviceToHost, st));
   if (phi && n > 0)
-    CUDA_TRY(cudaMemcpyAsync(phi, p->d_phi_out, rs * (size_t)p->C * n, cudaMemcpyDeviceToHost, st));
-  if (F && n > 0) CUDA_TRY(cudaMemcpyAsync(F, p->d_F_out, rs * 3 * (size_t)n, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(phi, p->d_phi_out[0], rs * (size_t)p->C * n, cudaMemcpyDeviceToHost, st));
+  if (F && n > 0) CUDA_TRY(cudaMemcpyAsync(F, p->d_F_out[0], rs * 3 * (size_t)n, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
+  return 0;
+}
+
+// Pipelined host-buffer evaluation.  Submission k uses staging slot k % 2:
+//   copy-in stream:   [wait: evaluation k-2 done with the slot]  H2D pos, q            -> ev_in
+//   compute stream:   [wait: ev_in, copy-out k-2 done with the slot]  the evaluation     -> ev_comp
+//   copy-out stream:  [wait: ev_comp]  D2H E, phi, F                                    -> ev_out
+// so with pinned host buffers H2D(k+1), evaluation(k) and D2H(k-1) run at the same time.
+int pswf_lr_submit_host(pswf_lr_plan* p, int n, const void* pos, const void* q, double* E, void* phi, void* F) {
+  if (!p || n < 0) return PSWF_LR_ERR_INVALID_ARG;
+  if (n > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  if (p->n_submitted - p->n_waited >= 2) return PSWF_LR_ERR_BUSY;
+  DeviceGuard guard(p);
+  if (!guard.ok) return PSWF_LR_ERR_CUDA;
+  if (n > p->cap_atoms && p->n_submitted != p->n_waited) return PSWF_LR_ERR_BUSY;   // growing reallocates
+  int rc = ensure_capacity(p, n);
+  if (rc) return rc;
+  rc = ensure_host_staging(p, 2);
+  if (rc) return rc;
+  if (!p->s_in) {
+    CUDA_TRY(cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&p->s_comp, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking));
+    for (int s = 0; s < 2; ++s) {
+      CUDA_TRY(cudaEventCreateWithFlags(&p->ev_in[s], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&p->ev_comp[s], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&p->ev_out[s], cudaEventDisableTiming));
+    }
+  }
+  const int s = (int)(p->n_submitted & 1);
+  const bool reuse = p->n_submitted >= 2;
+  const size_t rs = real_size(p);
+  if (reuse) CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_comp[s], 0));
+  if (n > 0) {
+    CUDA_TRY(cudaMemcpyAsync(p->d_pos_in[s], pos, rs * 3 * (size_t)n, cudaMemcpyHostToDevice, p->s_in));
+    CUDA_TRY(cudaMemcpyAsync(p->d_q_in[s], q, rs * (size_t)p->C * n, cudaMemcpyHostToDevice, p->s_in));
+  }
+  CUDA_TRY(cudaEventRecord(p->ev_in[s], p->s_in));
+  CUDA_TRY(cudaStreamWaitEvent(p->s_comp, p->ev_in[s], 0));
+  if (reuse) CUDA_TRY(cudaStreamWaitEvent(p->s_comp, p->ev_out[s], 0));
+  rc = pswf_lr_execute(p, n, p->d_pos_in[s], p->d_q_in[s], E ? p->d_E_out[s] : nullptr,
+                       phi ? p->d_phi_out[s] : nullptr, F ? p->d_F_out[s] : nullptr, p->s_comp);
+  if (rc) return rc;
+  CUDA_TRY(cudaEventRecord(p->ev_comp[s], p->s_comp));
+  CUDA_TRY(cudaStreamWaitEvent(p->s_out, p->ev_comp[s], 0));
+  if (E) CUDA_TRY(cudaMemcpyAsync(E, p->d_E_out[s], sizeof(double), cudaMemcpyDeviceToHost, p->s_out));
+  if (phi && n > 0)
+    CUDA_TRY(cudaMemcpyAsync(phi, p->d_phi_out[s], rs * (size_t)p->C * n, cudaMemcpyDeviceToHost, p->s_out));
+  if (F && n > 0) CUDA_TRY(cudaMemcpyAsync(F, p->d_F_out[s], rs * 3 * (size_t)n, cudaMemcpyDeviceToHost, p->s_out));
+  CUDA_TRY(cudaEventRecord(p->ev_out[s], p->s_out));
+  p->n_submitted++;
+  return 0;
+}
+
+int pswf_lr_wait_host(pswf_lr_plan* p) {
+  if (!p) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  if (p->n_submitted == p->n_waited) return PSWF_LR_ERR_INVALID_ARG;   // nothing in flight
+  const int s = (int)(p->n_waited & 1);
+  CUDA_TRY(cudaEventSynchronize(p->ev_out[s]));
+  p->n_waited++;
   return 0;
 }
 
@@ -577,6 +667,8 @@ int pswf_lr_execute_real(pswf_lr_plan* p, int n_atoms, const void* pos, const vo
   if (n_atoms > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
   if (p->host_only) return PSWF_LR_ERR_CUDA;
   if (!p->real_ok) return PSWF_LR_ERR_GRID_TOO_COARSE;   // r_c >= L_d / 2: minimum image does not suffice
+  DeviceGuard guard(p);
+  if (!guard.ok) return PSWF_LR_ERR_CUDA;
   int rc = ensure_capacity(p, n_atoms);
   if (rc) return rc;
   cudaStream_t st = (cudaStream_t)stream;
@@ -816,10 +908,20 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
     delete p;
     return 0;
   }
+  DeviceGuard guard(p);
   cudaDeviceSynchronize();
   free_atoms(p);
+  for (int s = 0; s < 2; ++s) {
+    if (p->d_E_out[s]) cudaFree(p->d_E_out[s]);
+    if (p->ev_in[s]) cudaEventDestroy(p->ev_in[s]);
+    if (p->ev_comp[s]) cudaEventDestroy(p->ev_comp[s]);
+    if (p->ev_out[s]) cudaEventDestroy(p->ev_out[s]);
+  }
+  if (p->s_in) cudaStreamDestroy(p->s_in);
+  if (p->s_comp) cudaStreamDestroy(p->s_comp);
+  if (p->s_out) cudaStreamDestroy(p->s_out);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
-                  p->d_grid,  p->d_spec,    p->d_count,    p->d_scan_state, p->d_Ech,      p->d_Etot,
+                  p->d_grid,  p->d_spec,    p->d_count,    p->d_scan_state, p->d_Ech,
                   p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal, p->d_virial, p->d_spec2, p->d_spec_dump};
   for (void* q : ptrs)
     if (q) cudaFree(q);

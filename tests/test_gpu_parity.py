@@ -337,6 +337,55 @@ def test_execute_host_matches_execute():
     plan.destroy()
 
 
+def test_pipelined_host_submissions_match_execute():
+    """pswf_lr_submit_host / pswf_lr_wait_host: five different systems through the two staging slots
+    give what the blocking call gives; a third submission in flight is refused, and so is a blocking
+    call while submissions are in flight; workspace accounting survives a capacity growth."""
+    wl = workloads.make(2)
+    n, C = len(wl["pos"]), 2
+    plan = make_plan(wl, max_atoms=64)      # the first submission has to grow the workspaces
+    rng = np.random.default_rng(5)
+    systems = []
+    for k in range(5):
+        pos = torch.as_tensor(wl["pos"] + rng.normal(0, 0.05, wl["pos"].shape), dtype=torch.float32).pin_memory()
+        q = torch.as_tensor(wl["q"] * (1.0 + 0.1 * k), dtype=torch.float32).pin_memory()
+        systems.append((pos, q))
+    outs = [(torch.zeros(1, dtype=torch.float64).pin_memory(), torch.zeros((C, n), dtype=torch.float32).pin_memory(),
+             torch.zeros((n, 3), dtype=torch.float32).pin_memory()) for _ in range(5)]
+    sp = torch.cuda.current_stream().cuda_stream
+    ref = []
+    for pos, q in systems:
+        E = torch.zeros(1, dtype=torch.float64).pin_memory()
+        phi = torch.zeros((C, n), dtype=torch.float32).pin_memory()
+        F = torch.zeros((n, 3), dtype=torch.float32).pin_memory()
+        plan.execute_host(n, pos, q, E, phi, F, sp)
+        ref.append((E.item(), phi.double().numpy().copy(), F.double().numpy().copy()))
+    w0 = plan.info()["workspace_bytes"]
+    for k in range(5):
+        if k >= 2:
+            plan.wait_host()
+        plan.submit_host(n, systems[k][0], systems[k][1], *outs[k])
+        if k == 1:
+            with pytest.raises(binding.PswfLrError) as e3:
+                plan.submit_host(n, systems[k][0], systems[k][1], *outs[k])
+            assert e3.value.code == -7
+            with pytest.raises(binding.PswfLrError) as e4:
+                plan.execute_host(n, systems[k][0], systems[k][1], *outs[k], sp)
+            assert e4.value.code == -7
+    plan.wait_host()
+    plan.wait_host()
+    with pytest.raises(binding.PswfLrError):
+        plan.wait_host()                    # nothing in flight
+    for k in range(5):
+        E, phi, F = outs[k]
+        assert abs(E.item() - ref[k][0]) < 2e-6 * abs(ref[k][0])
+        assert rel(F.double().numpy(), ref[k][2]) < 1e-5 and rel(phi.double().numpy(), ref[k][1]) < 1e-5
+    # second staging slot was added; nothing else may have changed
+    w1 = plan.info()["workspace_bytes"]
+    assert 0 < w1 - w0 <= 2 * (n * (3 + C) * 4 * 2 + 64) + 4096
+    plan.destroy()
+
+
 def test_capacity_growth_and_plan_reuse():
     small = workloads.make(2, n_atoms=300)
     big = workloads.make(2)
