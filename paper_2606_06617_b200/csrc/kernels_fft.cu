@@ -553,6 +553,66 @@ __global__ void __launch_bounds__(kZThreads)
   }
 }
 
+// Inverse z transform that writes the potential grid directly in the layout the fast gather reads,
+// transposed and channel-interleaved [z][x][y][CBV] (kernels_gather.cu), for the channels cb0 ..
+// cb0+nch-1: the separate transposing copy (k_interleave_t, 12 us at config 4) and the planar real
+// grid it read are gone.  A CTA takes (x, YT = 16 pencils in y) for all channels of the group.
+__host__ __device__ constexpr int z_tile_il(int NZ) { return NZ > 128 ? 8 : 16; }   // static shared memory <= 48 KB
+
+template <int CBV> struct ZVec;
+template <> struct ZVec<1> { using type = float; };
+template <> struct ZVec<2> { using type = float2; };
+template <> struct ZVec<4> { using type = float4; };
+
+template <int NZ, int CBV>
+__global__ void __launch_bounds__(kZThreads)
+    k_z_inverse_il(int C, int cb0, int nch, int Mx, int My, int YT, int kmaxz, const float2* __restrict__ spec,
+                   typename ZVec<CBV>::type* __restrict__ out) {
+  constexpr int pitch = NZ + 1, NT = kZThreads;
+  __shared__ __align__(16) float2 s[CBV * (z_tile_il(NZ) / 2) * pitch];
+  __shared__ float2 tw[NZ];
+  __shared__ short pos_of[NZ];
+  const int tid = threadIdx.x;
+  const int ytiles = My / YT;
+  const int yt = blockIdx.x % ytiles, x = blockIdx.x / ytiles;
+  const int y0 = yt * YT, npc = YT / 2, npen = CBV * npc;   // pencil index = ch * npc + q
+  int lgp = 0;
+  while ((1 << lgp) < npen) ++lgp;
+  for (int i = tid; i < NZ; i += NT) {
+    float sn, cs;
+    sincospif(-2.f * (float)i / (float)NZ, &sn, &cs);
+    tw[i] = make_float2(cs, sn);
+    pos_of[freq_of_pos_t<NZ>(i)] = (short)i;
+  }
+  for (int i = tid; i < npen * pitch; i += NT) s[i] = make_float2(0.f, 0.f);
+  __syncthreads();
+  const size_t pl = (size_t)C * Mx * My;
+  for (int i = tid; i < (kmaxz + 1) * nch * npc; i += NT) {
+    const int q = i % npc, r = i / npc, ch = r % nch, k = r / nch;
+    const float2* src = spec + (size_t)k * pl + ((size_t)(cb0 + ch) * Mx + x) * My + y0 + 2 * q;
+    const float4 ab = __ldg(reinterpret_cast<const float4*>(src));                              // A[k], B[k]
+    float2* sp = s + (ch * npc + q) * pitch;
+    sp[pos_of[k]] = make_float2(ab.x - ab.w, ab.y + ab.z);                                      // A + i B
+    if (k > 0) sp[pos_of[NZ - k]] = make_float2(ab.x + ab.w, ab.z - ab.y);                      // conj A + i conj B
+  }
+  __syncthreads();
+  fft_axis_t<NT, NZ, true, pitch, 1>(s, npen, lgp, nullptr, tw);
+  // out[z][x][y][CBV]: for every z a run of YT * CBV floats
+  using V = typename ZVec<CBV>::type;
+  for (int i = tid; i < NZ * YT; i += NT) {
+    const int y = i % YT, z = i / YT;
+    float v[CBV];
+#pragma unroll
+    for (int ch = 0; ch < CBV; ++ch)
+      v[ch] = reinterpret_cast<const float*>(s + (ch * npc + (y >> 1)) * pitch + z)[y & 1];
+    V o;
+    if constexpr (CBV == 1) o = v[0];
+    else if constexpr (CBV == 2) o = make_float2(v[0], v[1]);
+    else o = make_float4(v[0], v[1], v[2], v[3]);
+    out[((size_t)z * Mx + x) * My + y0 + y] = o;
+  }
+}
+
 int factor_radices(int N, int* rad) {
   int n = 0;
   while (N >= 8 && N != 16) { rad[n++] = 8; N /= 8; }   // 16 = 4 x 4
@@ -643,6 +703,33 @@ void launch_z_forward(pswf_lr_plan* p, cudaStream_t st) {
   case NZ: k_z_forward<NZ><<<nb, kZThreads, 0, st>>>(C, Mx, My, YT, p->fused_kmax[2], (const float*)p->d_grid, (float2*)p->d_spec); break;
   switch (p->M[2]) { PSWF_ZF(8) PSWF_ZF(16) PSWF_ZF(32) PSWF_ZF(64) PSWF_ZF(128) PSWF_ZF(256) default: break; }
 #undef PSWF_ZF
+}
+
+// the fast gather's layout, channel groups of 4 as in launch_fast_gather (last group 1, 2 or 4 wide)
+void launch_z_inverse_interleaved(pswf_lr_plan* p, cudaStream_t st) {
+  const int C = p->C, Mx = p->M[0], My = p->M[1];
+  int YT = std::min(z_tile_il(p->M[2]), My);
+  while (My % YT) YT >>= 1;
+  const unsigned nb = (unsigned)(Mx * (My / YT));
+  const size_t Mtot = (size_t)Mx * My * p->M[2];
+  float* gi = (float*)p->d_gridi;
+  for (int cb0 = 0; cb0 < C; cb0 += 4) {
+    const int left = C - cb0;
+    const int cbv = left >= 3 ? 4 : left, nch = std::min(left, 4);
+#define PSWF_ZIL(NZ, CBV)                                                                                         \
+  k_z_inverse_il<NZ, CBV><<<nb, kZThreads, 0, st>>>(C, cb0, nch, Mx, My, YT, p->fused_kmax[2], (const float2*)p->d_spec2, \
+                                                    (typename ZVec<CBV>::type*)gi)
+#define PSWF_ZIL_N(NZ)                     \
+  case NZ:                                 \
+    if (cbv == 4) PSWF_ZIL(NZ, 4);         \
+    else if (cbv == 2) PSWF_ZIL(NZ, 2);    \
+    else PSWF_ZIL(NZ, 1);                  \
+    break;
+    switch (p->M[2]) { PSWF_ZIL_N(16) PSWF_ZIL_N(32) PSWF_ZIL_N(64) PSWF_ZIL_N(128) PSWF_ZIL_N(256) default: break; }
+#undef PSWF_ZIL_N
+#undef PSWF_ZIL
+    gi += Mtot * cbv;
+  }
 }
 
 void launch_z_inverse(pswf_lr_plan* p, cudaStream_t st) {

@@ -446,7 +446,7 @@ size_t gather_grid_bytes(const pswf_lr_plan* p) {
 }
 
 template <int GBX, int GBY, int NCTA>
-void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream_t st) {
+void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, bool have_il, cudaStream_t st) {
   const int Mx = p->M[0], My = p->M[1], Mz = p->M[2];
   const size_t Mtot = (size_t)Mx * My * Mz;
   const int nseg = (Mz + ZSEG - 1) / ZSEG;
@@ -464,7 +464,7 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, cudaStre
 #define PSWF_GATHER(CBV, NCH)                                                                               \
   do {                                                                                                      \
     using V = typename VecOf<CBV>::type;                                                                    \
-    k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);                          \
+    if (!have_il) k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);            \
     auto kern = k_gather_rows<CBV, GBX, GBY, NCTA>;                                                         \
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \
     kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nbx, nby, recf, p->d_count,        \
@@ -480,11 +480,11 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, cudaStre
   }
 }
 
-void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream_t st) {
+void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, bool grid_is_interleaved, cudaStream_t st) {
   if (n <= 0) return;
   // 2 x 2 cell rows (4 warps) per CTA, 4 CTAs per SM: short-lived CTAs lose fewer warp slots to the
   // longest row than 8-warp ones (489 -> 474 us), and the 128-register budget is the same
-  launch_fast_gather_t<2, 2, 4>(p, n, phi, F, st);
+  launch_fast_gather_t<2, 2, 4>(p, n, phi, F, grid_is_interleaved, st);
 }
 
 }  // namespace pswf

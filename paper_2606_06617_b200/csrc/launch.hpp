@@ -22,7 +22,7 @@ int stencil_rec_floats(int C);
 size_t stencil_record_bytes(const pswf_lr_plan* p);
 size_t stencil_drecord_bytes(const pswf_lr_plan* p);
 size_t gather_grid_bytes(const pswf_lr_plan* p);
-void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, cudaStream_t st);
+void launch_fast_gather(pswf_lr_plan* p, int n, float* phi, float* F, bool grid_is_interleaved, cudaStream_t st);
 void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const float* q, const GridGeom<float>& g,
                             cudaStream_t st);
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st);
@@ -34,6 +34,7 @@ void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t 
 bool fused_z_supported(const pswf_lr_plan* p);   // own z transforms (power-of-two Mz); else cuFFT along z
 void launch_z_forward(pswf_lr_plan* p, cudaStream_t st);
 void launch_z_inverse(pswf_lr_plan* p, cudaStream_t st);
+void launch_z_inverse_interleaved(pswf_lr_plan* p, cudaStream_t st);   // writes p->d_gridi (fast gather layout)
 
 // real-space complement + self term (kernels_real.cu); uses the sort left by launch_bin_sort(scatter = true)
 template <class T>

@@ -232,10 +232,15 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   if (ev) cudaEventRecord(ev[4], st);
   if (phi || F) {
     // a4
+    bool il = false;
     if (fused) {
-      if (p->fused_z) {
+      // own z transform: straight into the gather's interleaved layout when the fast gather follows
+      // (the planar grid is then written only on request, for pswf_lr_debug_copy(what = 2))
+      il = p->fused_z && stencil && p->M[2] >= 16;
+      if (il) launch_z_inverse_interleaved(p, st);
+      if (p->fused_z && (!il || p->debug_dump_spectrum)) {
         launch_z_inverse(p, st);
-      } else {
+      } else if (!p->fused_z) {
         CUFFT_TRY(cufftSetStream(p->fft_zi, st));
         CUFFT_TRY(cufftExecC2R(p->fft_zi, (cufftComplex*)p->d_spec2, (cufftReal*)p->d_grid));
       }
@@ -249,7 +254,7 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
     if (ev) cudaEventRecord(ev[5], st);
     // a5
     if constexpr (kIsF32) {
-      if (stencil) launch_fast_gather(p, n, phi, F, st);
+      if (stencil) launch_fast_gather(p, n, phi, F, il, st);
     }
     if (!stencil) launch_gather_ref<T>(p, n, g, phi, F, st);
     if (ev) cudaEventRecord(ev[6], st);
