@@ -117,22 +117,15 @@ def c_threads():
     return int(_lib().oracle_threads())
 
 
-def direct_sums_c(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_mode=True,
-                  rho_atoms=None):
+def direct_sums_c(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_mode=True):
     """Same contract as direct_sums(), evaluated by oracle/direct_sum.c over the half mode
     set (x2; rho(-k) = conj rho(k) and Phi^ is even, so the +-k terms of Eq. (5) are equal).
     The mollifier values Phi^_p(|k|) per mode are computed here with kernels.py and passed in.
-
-    rho_atoms: optional int -- use only the first rho_atoms atoms in rho(k) (bench sampling).
     """
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     q = np.ascontiguousarray(np.atleast_2d(q), dtype=np.float64)
     box = np.ascontiguousarray(box, dtype=np.float64)
     C, N = q.shape
-    if rho_atoms is not None:
-        N = int(rho_atoms)
-        pos = np.ascontiguousarray(pos[:N])
-        q = np.ascontiguousarray(q[:, :N])
     moll = Mollifier(c, r_c)
     m = np.ascontiguousarray(mode_set(box, c, r_c, grid, half=True), dtype=np.int32)
     K = len(m)

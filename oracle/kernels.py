@@ -1,4 +1,4 @@
-"""PSWF-mollified inverse-power kernels, p = 1..6 (oracle, float64).
+"""PSWF-mollified inverse-power kernels, p = 1..6 and p = 8, 10 (oracle, float64).
 
 TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).
 
@@ -61,8 +61,23 @@ class Mollifier:
             val = (PI ** 2 / 12) * (kap ** 3 - kap ** 3 * self._A(x)
                                     - 3 * c * kap ** 2 / (2 * C0) * self._J(1, x)
                                     + c ** 3 / (2 * C0) * self._J(3, x))
+        elif p == 8:
+            # (S56), applied to (S52): S^_8(k) = (1/6) int_k^c s S^_6(s) ds  ("The Fourier-space
+            # transforms S^_8 and S^_10 follow from (S56) applied to S^_6 in (S52) and S^_8", PAPER.md:905;
+            # the upper limit is c by the truncation convention).  With J_n(x) = int_x^1 t^n phi,
+            # 1 - A = J_0 / C_0 and int_x^1 y^m J_n(y) dy = (J_{m+n+1}(x) - x^{m+1} J_n(x)) / (m+1):
+            #   S^_6 = pi^2 c^3/(12 C_0) [x^3 J_0 - (3/2) x^2 J_1 + (1/2) J_3]
+            #   S^_8 = pi^2 c^5/(72 C_0) [-x^5 J_0/5 + (3/8) x^4 J_1 - x^2 J_3/4 + (3/40) J_5]
+            val = (PI ** 2 * c ** 5 / (72 * C0)) * (-x ** 5 * self._J(0, x) / 5 + 0.375 * x ** 4 * self._J(1, x)
+                                                     - 0.25 * x ** 2 * self._J(3, x) + 0.075 * self._J(5, x))
+        elif p == 10:
+            # (S56) once more: S^_10(k) = (1/8) int_k^c s S^_8(s) ds
+            #   = pi^2 c^7/(576 C_0) [x^7 J_0/35 - x^6 J_1/16 + x^4 J_3/16 - (3/80) x^2 J_5 + J_7/112]
+            val = (PI ** 2 * c ** 7 / (576 * C0)) * (x ** 7 * self._J(0, x) / 35 - x ** 6 * self._J(1, x) / 16
+                                                      + x ** 4 * self._J(3, x) / 16 - 0.0375 * x ** 2 * self._J(5, x)
+                                                      + self._J(7, x) / 112)
         else:
-            raise ValueError("p must be in 1..6")
+            raise ValueError("p must be in 1..6, 8 or 10")
         return np.where(inside, val, 0.0)
 
     def Phi_hat(self, p, k):
@@ -95,7 +110,11 @@ class Mollifier:
             return float(rc ** (3 - 5) * (2 * PI / 3) * c ** 2 * self._J(1, zero))
         if p == 6:   # limit of (S52)
             return float(rc ** (3 - 6) * (PI ** 2 / 12) * c ** 3 / (2 * C0) * self._J(3, zero))
-        raise ValueError("p must be in 1..6")
+        if p == 8:   # (S79) with the k -> 0 limit of S^_8 above
+            return float(rc ** (3 - 8) * (PI ** 2 * c ** 5 / (72 * C0)) * 0.075 * self._J(5, zero))
+        if p == 10:
+            return float(rc ** (3 - 10) * (PI ** 2 * c ** 7 / (576 * C0)) * self._J(7, zero) / 112)
+        raise ValueError("p must be in 1..6, 8 or 10")
 
     # ---- real-space long-range kernels (validation scaffold) ------------------
     def S_zero(self, p):
@@ -107,6 +126,10 @@ class Mollifier:
             n = two_n // 2
             mom = 2 * quad(lambda t: t ** two_n * self.psi(t), np.zeros(()), np.ones(()))
             return float((-1) ** n * c ** two_n * mom / self.psi.lambda0)
+        if p == 8:     # (S59)
+            return d0(8) / 40320
+        if p == 10:
+            return -d0(10) / 3628800
         return {1: 1 / C0, 2: -d0(2) / 2, 3: -d0(2) / (3 * C0), 4: d0(4) / 24,
                 5: d0(4) / (45 * C0), 6: -d0(6) / 720}[p]
 
@@ -133,8 +156,16 @@ class Mollifier:
             val = (Phi - rr * phi + rr ** 2 * d1 / 3) / (C0 * rr ** 5)
         elif p == 6:
             val = (1 - phi + 0.625 * rr * d1 - 0.125 * rr ** 2 * d2) / rr ** 6
+        elif p == 8:    # Corollary 1 (S57)
+            d3 = self.psi.deriv(rr, 3)
+            val = (1 - phi + (11 / 16) * rr * d1 - (3 / 16) * rr ** 2 * d2 + rr ** 3 * d3 / 48) / rr ** 8
+        elif p == 10:   # (S58)
+            d3 = self.psi.deriv(rr, 3)
+            d4 = self.psi.deriv(rr, 4)
+            val = (1 - phi + (93 / 128) * rr * d1 - (29 / 128) * rr ** 2 * d2 + (7 / 192) * rr ** 3 * d3
+                   - rr ** 4 * d4 / 384) / rr ** 10
         else:
-            raise ValueError("p must be in 1..6")
+            raise ValueError("p must be in 1..6, 8 or 10")
         with np.errstate(divide="ignore"):
             out = np.where(inner, val, np.where(r > 0, r, 1.0) ** (-float(p)))
         return np.where(r == 0, self.S_zero(p), out)
