@@ -6,7 +6,7 @@
  *     E = 1/(2V) sum_a sum_{k != 0} Phi^_{p_a}(k) |rho_a(k)|^2 + sum_a E_0^{(p_a)},
  *     rho_a(k) = sum_j q_j^a exp(i k.r_j)                                   Eq. (6)
  *
- * for several channels a (latent charges q^a, exponent p_a in 1..6), by the gridded algorithm of
+ * for several channels a (latent charges q^a, exponent p_a in 1..6, 8 or 10), by the gridded algorithm of
  * (i) spread with the separable PSWF window, Eq. (20)-(21),(24); (ii) batched
  * forward 3-D FFT; (iii) diagonal scaling by Phi^_p(k)/W^(k)^2, Eq. (22),(25), with Phi^_p from
  * Eq. (14) / SI Theorem 1 (S47)-(S52) and the k = 0 constants of Eq. (17)-(19) / (S73),(S75),(S78),
@@ -43,7 +43,7 @@ typedef struct pswf_lr_plan pswf_lr_plan; /* opaque */
 typedef enum {
   PSWF_LR_OK = 0,
   PSWF_LR_ERR_INVALID_ARG = -1,          /* null pointer, non-positive size, w out of range ...   */
-  PSWF_LR_ERR_UNSUPPORTED_EXPONENT = -2, /* p outside 1..6 (p >= 7: PAPER.md:878, out of scope)   */
+  PSWF_LR_ERR_UNSUPPORTED_EXPONENT = -2, /* p not in {1..6, 8, 10} (SI Section 6)  */
   PSWF_LR_ERR_GRID_TOO_COARSE = -3,      /* h > pi r_c / c (Eq. (29)), w > M_d, or the window      */
                                          /* transform would be used outside its band              */
   PSWF_LR_ERR_ALLOC = -4,
@@ -94,7 +94,8 @@ typedef struct {
 
 /* Create a plan.  box[3]: edge lengths; grid[3]: M_x,M_y,M_z (each >= w, product < 2^31);
  * w: window width P in grid points (even, 2..16); c: mollifier bandwidth
- * (Eq. (28)), 2 <= c <= 60; exponents[n_channels]: p_a in 1..6, repeats allowed.
+ * (Eq. (28)), 2 <= c <= 60; exponents[n_channels]: p_a in 1..6 (Theorem 1) or 8, 10
+ * (Theorem 2 / Corollary 1, (S55)-(S59)), repeats allowed.
  * Host pointers; nothing is retained.  Runs the host-side PSWF eigen-solve, fits the Horner
  * tables, builds cuFFT plans, allocates workspaces. */
 int pswf_lr_plan_create(pswf_lr_plan** plan, const double box[3], const int grid[3], int w, double c,

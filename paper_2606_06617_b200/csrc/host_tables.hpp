@@ -180,6 +180,7 @@ inline WindowTable fit_window(const Pswf0& psi, int w, double eps, int max_degre
 //   p=4: pi^2 c T_4,                           T_4 = J_1/C0 - x (1 - A),  J_n = int_x^1 t^n phi
 //   p=5: (2 pi c^2 / 3)(T_5 + x^2 ln x),       T_5 = J_1 - x^2 T_3
 //   p=6: (pi^2 c^3 / 12) T_6,                  T_6 = x^3 (1 - A) - 3 x^2 J_1 / (2 C0) + J_3 / (2 C0)
+//   p=8: (pi^2 c^5 / 72) T_8,   p=10: (pi^2 c^7 / 576) T_10   (SI Section 6, see T())
 // and Phi^_p(k) = r_c^(3-p) S^_p(k r_c)  (S60).
 struct KernelMath {
   const Pswf0& psi;
@@ -200,6 +201,18 @@ struct KernelMath {
       case 4: return J(1, x) / psi.C0 - x * (1.0 - A(x));
       case 5: return J(1, x) - x * x * Llog(x);
       case 6: return x * x * x * (1.0 - A(x)) - 1.5 * x * x * J(1, x) / psi.C0 + 0.5 * J(3, x) / psi.C0;
+      // p = 8, 10: (S56) applied to (S52) and once more, integrals over [k, c] by the
+      // truncation convention; with int_x^1 y^m J_n = (J_{m+n+1} - x^{m+1} J_n) / (m+1) and 1 - A = J_0 / C0:
+      //   S^_8  = (pi^2 c^5 / 72)  T_8,   S^_10 = (pi^2 c^7 / 576) T_10
+      case 8: {
+        const double x2 = x * x, x4 = x2 * x2;
+        return (-x4 * x * J(0, x) / 5 + 0.375 * x4 * J(1, x) - 0.25 * x2 * J(3, x) + 0.075 * J(5, x)) / psi.C0;
+      }
+      case 10: {
+        const double x2 = x * x, x4 = x2 * x2, x6 = x4 * x2;
+        return (x6 * x * J(0, x) / 35 - x6 * J(1, x) / 16 + x4 * J(3, x) / 16 - 0.0375 * x2 * J(5, x) +
+                J(7, x) / 112) / psi.C0;
+      }
     }
     throw std::invalid_argument("p");
   }
@@ -214,6 +227,8 @@ struct KernelMath {
       case 4: return std::pow(r_c, -1.0) * kPi * kPi * c * T(4, 0.0);   // (S79): k -> 0 of (S50)
       case 5: return std::pow(r_c, -2.0) * (2 * kPi * c * c / 3) * T(5, 0.0);
       case 6: return std::pow(r_c, -3.0) * (kPi * kPi * c * c * c / 12) * T(6, 0.0);
+      case 8: return std::pow(r_c, -5.0) * (kPi * kPi * std::pow(c, 5) / 72) * T(8, 0.0);
+      case 10: return std::pow(r_c, -7.0) * (kPi * kPi * std::pow(c, 7) / 576) * T(10, 0.0);
     }
     throw std::invalid_argument("p");
   }

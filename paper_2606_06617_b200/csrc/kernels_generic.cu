@@ -202,8 +202,8 @@ __global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __
   __syncthreads();
   bool active = m < Mhalf;
   bool inside = false;
-  T D[6];
-  T dDk[6];            // (dD/dk) / |k| per slot
+  T D[kMaxSlots];
+  T dDk[kMaxSlots];    // (dD/dk) / |k| per slot
   T kv[3] = {(T)0, (T)0, (T)0};
   double wloc[6] = {0, 0, 0, 0, 0, 0};
   T herm = (T)0;

@@ -90,9 +90,9 @@ __global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, Rea
       const int pj = min((int)(x * (T)P.panels), P.panels - 1);
       const T xi = (T)2 * (x * (T)P.panels - (T)pj) - (T)1;
       const T invx = (T)1 / x;
-      T Lval[6], dL[6];
+      T Lval[kMaxSlots], dL[kMaxSlots];
 #pragma unroll
-      for (int s = 0; s < 6; ++s) {
+      for (int s = 0; s < kMaxSlots; ++s) {
         if (s >= P.nslots) break;
         const T* cf = s_cf + (s * P.panels + pj) * (P.degree + 1);
         const T* df = s_df + (s * P.panels + pj) * P.degree;

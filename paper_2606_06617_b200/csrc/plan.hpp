@@ -12,6 +12,7 @@
 namespace pswf {
 
 constexpr int kMaxChannels = 32;
+constexpr int kMaxSlots = 8;       // distinct exponents: 1..6, 8, 10
 constexpr int kMaxW = 16;
 constexpr int kMaxWindowDegree = 30;
 constexpr int kMaxKernelDegree = 24;
@@ -32,10 +33,10 @@ struct ScaleParams {
   int Mzh;             // Mz/2 + 1
   int C;               // channels
   int nslots;          // distinct exponents
-  int slot_p[6];       // exponent of each slot
+  int slot_p[kMaxSlots];   // exponent of each slot
   int chan_slot[kMaxChannels];
   T chan_D0[kMaxChannels];   // multiplier of the m = 0 mode per channel (0 when dropped)
-  T slot_pre[6];       // r_c^(3-p) * constant prefactor of each slot
+  T slot_pre[kMaxSlots];   // r_c^(3-p) * constant prefactor of each slot
   T kfac[3];           // 2 pi / L_d
   T x_per_k;           // r_c / c
   T c;                 // mollifier bandwidth
@@ -70,9 +71,9 @@ struct RealGeom {
 template <class T>
 struct RealParams {
   int C, nslots, panels, degree;
-  int slot_p[6];
+  int slot_p[kMaxSlots];
   int chan_slot[kMaxChannels];
-  T slot_pre[6];               // r_c^-p per slot
+  T slot_pre[kMaxSlots];       // r_c^-p per slot
   T self_pre[kMaxChannels];    // S_p(0) / r_c^p per channel
   T r_c, inv_rc;
   const T* coef;               // [slot][panel][degree+1]  N_p

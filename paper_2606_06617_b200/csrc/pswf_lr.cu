@@ -136,6 +136,8 @@ GridGeom<T> make_geom(const pswf_lr_plan* p) {
   return g;
 }
 
+bool exponent_supported(int p) { return (p >= 1 && p <= 6) || p == 8 || p == 10; }
+
 double slot_prefactor(int p, double c, double r_c) {
   // Phi^_p = r_c^(3-p) S^_p, constants of Theorem 1 folded in (see host_tables.hpp / k_scale)
   switch (p) {
@@ -144,7 +146,9 @@ double slot_prefactor(int p, double c, double r_c) {
     case 3: return 4 * kPi;
     case 4: return kPi * kPi * c / r_c;
     case 5: return 2 * kPi * c * c / (3 * r_c * r_c);
-    default: return kPi * kPi * c * c * c / (12 * r_c * r_c * r_c);
+    case 6: return kPi * kPi * c * c * c / (12 * r_c * r_c * r_c);
+    case 8: return kPi * kPi * std::pow(c / r_c, 5) / 72;      // SI Section 6, (S56) applied to (S52)
+    default: return kPi * kPi * std::pow(c / r_c, 7) / 576;    // p = 10
   }
 }
 
@@ -317,7 +321,7 @@ const char* pswf_lr_error_string(int code) {
   switch (code) {
     case PSWF_LR_OK: return "ok";
     case PSWF_LR_ERR_INVALID_ARG: return "invalid argument";
-    case PSWF_LR_ERR_UNSUPPORTED_EXPONENT: return "unsupported exponent (p must be 1..6)";
+    case PSWF_LR_ERR_UNSUPPORTED_EXPONENT: return "unsupported exponent (p must be 1..6, 8 or 10)";
     case PSWF_LR_ERR_GRID_TOO_COARSE: return "grid too coarse for (c, r_c, w, c_window)";
     case PSWF_LR_ERR_ALLOC: return "device allocation failed";
     case PSWF_LR_ERR_CUDA: return "CUDA error (no usable device, or a kernel/launch failed)";
@@ -347,7 +351,7 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
   }
   if (mtot >= 2147483647.0) return PSWF_LR_ERR_INVALID_ARG;
   for (int a = 0; a < n_channels; ++a)
-    if (exponents[a] < 1 || exponents[a] > 6) return PSWF_LR_ERR_UNSUPPORTED_EXPONENT;
+    if (!exponent_supported(exponents[a])) return PSWF_LR_ERR_UNSUPPORTED_EXPONENT;
   for (int d = 0; d < 3; ++d)
     if (grid[d] < w) return PSWF_LR_ERR_GRID_TOO_COARSE;
   pswf_lr_opts o;
@@ -393,7 +397,7 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
 
     // distinct exponents, slots
     for (int a = 0; a < n_channels; ++a) p->chan_p[a] = exponents[a];
-    for (int pp = 1; pp <= 6; ++pp)
+    for (int pp = 1; pp <= 10; ++pp)
       for (int a = 0; a < n_channels; ++a)
         if (exponents[a] == pp) {
           p->distinct_p.push_back(pp);

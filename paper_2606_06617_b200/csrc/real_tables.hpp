@@ -11,6 +11,7 @@
 //     N_4 = phi - x phi'/2                               (S24),
 //     N_5 = 1 - (Phi - x phi + x^2 phi'/3)/C0            (S29),
 //     N_6 = phi - 5 x phi'/8 + x^2 phi''/8               (S33),
+//     N_8, N_10 from Corollary 1 (S57)-(S58), PAPER.md:891-894 (derivatives of phi up to the fourth)
 // N_p and dN_p/dx are tabulated as piecewise polynomials (Horner: "the real-space
 // kernels G_p" are evaluated the same way as the window); the singular factor x^-p stays explicit.
 // Self term: E_self = S_p(0) sum_i q_i^2 / (2 r_c^p) with S_p(0) from (S67); the
@@ -22,22 +23,27 @@
 
 namespace pswf {
 
-// psi, psi', psi'' from the Legendre series (three-term recurrences differentiated once and twice)
-inline void pswf_eval_d2(const Pswf0& psi, double x, double& f, double& d1, double& d2) {
+// psi and its first four derivatives from the Legendre series (three-term recurrence differentiated
+// m times: (k+1) P_{k+1}^(m) = (2k+1) (m P_k^(m-1) + x P_k^(m)) - k P_{k-1}^(m))
+inline void pswf_eval_d4(const Pswf0& psi, double x, double (&d)[5]) {
   const std::vector<double>& a = psi.leg;
-  double p0 = 1, p1 = x, q0 = 0, q1 = 1, r0 = 0, r1 = 0;   // P_k, P_k', P_k''
-  f = a[0] + (a.size() > 1 ? a[1] * x : 0.0);
-  d1 = a.size() > 1 ? a[1] : 0.0;
-  d2 = 0;
+  double p0[5] = {1, 0, 0, 0, 0}, p1[5] = {x, 1, 0, 0, 0};
+  for (int m = 0; m < 5; ++m) d[m] = a[0] * p0[m] + (a.size() > 1 ? a[1] * p1[m] : 0.0);
   for (size_t k = 1; k + 1 < a.size(); ++k) {
-    const double p2 = ((2 * k + 1) * x * p1 - k * p0) / (k + 1);
-    const double q2 = ((2 * k + 1) * (p1 + x * q1) - k * q0) / (k + 1);
-    const double r2 = ((2 * k + 1) * (2 * q1 + x * r1) - k * r0) / (k + 1);
-    f += a[k + 1] * p2;
-    d1 += a[k + 1] * q2;
-    d2 += a[k + 1] * r2;
-    p0 = p1; p1 = p2; q0 = q1; q1 = q2; r0 = r1; r1 = r2;
+    double p2[5];
+    p2[0] = ((2 * k + 1) * x * p1[0] - k * p0[0]) / (k + 1);
+    for (int m = 1; m < 5; ++m) p2[m] = ((2 * k + 1) * (m * p1[m - 1] + x * p1[m]) - k * p0[m]) / (k + 1);
+    for (int m = 0; m < 5; ++m) {
+      d[m] += a[k + 1] * p2[m];
+      p0[m] = p1[m];
+      p1[m] = p2[m];
+    }
   }
+}
+inline void pswf_eval_d2(const Pswf0& psi, double x, double& f, double& d1, double& d2) {
+  double d[5];
+  pswf_eval_d4(psi, x, d);
+  f = d[0]; d1 = d[1]; d2 = d[2];
 }
 
 struct RealMath {
@@ -57,6 +63,18 @@ struct RealMath {
       case 4: return f - 0.5 * x * d1;
       case 5: return 1.0 - (Phi(x) - x * f + x * x * d1 / 3.0) / C0;
       case 6: return f - 0.625 * x * d1 + 0.125 * x * x * d2;
+      case 8: {    // Corollary 1 (S57): N_8 = 1 - x^8 S_8
+        double d[5];
+        pswf_eval_d4(psi, x, d);
+        return d[0] - (11.0 / 16) * x * d[1] + (3.0 / 16) * x * x * d[2] - x * x * x * d[3] / 48;
+      }
+      case 10: {   // (S58)
+        double d[5];
+        pswf_eval_d4(psi, x, d);
+        const double x2 = x * x;
+        return d[0] - (93.0 / 128) * x * d[1] + (29.0 / 128) * x2 * d[2] - (7.0 / 192) * x2 * x * d[3] +
+               x2 * x2 * d[4] / 384;
+      }
     }
     throw std::invalid_argument("p");
   }
@@ -75,6 +93,8 @@ struct RealMath {
       case 4: return deriv0(4) / 24.0;
       case 5: return deriv0(4) / (45.0 * C0);
       case 6: return -deriv0(6) / 720.0;
+      case 8: return deriv0(8) / 40320.0;        // (S59)
+      case 10: return -deriv0(10) / 3628800.0;
     }
     throw std::invalid_argument("p");
   }

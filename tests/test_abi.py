@@ -13,6 +13,8 @@ import torch
 from oracle import gridded as G
 from oracle.kernels import Mollifier
 from oracle.pswf import PSWF0
+
+EXPONENTS = (1, 2, 3, 4, 5, 6, 8, 10)   # Theorem 1 and SI Section 6 (Corollary 1)
 from paper_2606_06617_b200 import binding, build
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -50,7 +52,8 @@ def test_argument_validation_codes():
     assert code(w=18) == binding.ERR_INVALID_ARG
     assert code(c=1.0) == binding.ERR_INVALID_ARG
     assert code(box=[10.0, -1.0, 10.0]) == binding.ERR_INVALID_ARG
-    assert code(exponents=[7]) == binding.ERR_UNSUPPORTED_EXPONENT
+    for bad in (7, 9, 11, 12):
+        assert code(exponents=[bad]) == binding.ERR_UNSUPPORTED_EXPONENT
     assert code(exponents=[0]) == binding.ERR_UNSUPPORTED_EXPONENT
     assert code(grid=[16, 4, 16]) == binding.ERR_GRID_TOO_COARSE          # w > M_d
     assert code(r_c=2.0) == binding.ERR_GRID_TOO_COARSE                   # eta = 1.2 > 1, Eq. (29)
@@ -109,13 +112,13 @@ def test_window_tables_match_oracle_pswf(precision, w, tol):
 @pytest.mark.parametrize("precision,tol", [("f32", 2e-7), ("f64", 2e-13)])
 def test_kernel_tables_match_oracle_theorem1(precision, tol):
     """Phi^_p(k) from 'bare transform + smooth Horner part' vs oracle Theorem-1 quadratures."""
-    p = binding.Plan([31.0] * 3, [32] * 3, 6, 12.024, [1, 2, 3, 4, 5, 6], precision=precision,
+    p = binding.Plan([31.0] * 3, [32] * 3, 6, 12.024, list(EXPONENTS), precision=precision,
                      host_only=True)
     i = p.info()
     moll = Mollifier(i["c"], i["r_c"])
     kc = i["c"] / i["r_c"]
     k = np.concatenate([np.linspace(2 * np.pi / 31.0, kc * 0.9999, 300), [kc * 0.25, kc * 1.0001, 2 * kc]])
-    for pe in range(1, 7):
+    for pe in EXPONENTS:
         got = p.eval_kernel(pe, k)
         ref = moll.Phi_hat(pe, k)
         # error relative to the kernel's size at the smallest k of the box
@@ -129,20 +132,22 @@ def test_kernel_tables_match_oracle_theorem1(precision, tol):
 def test_real_space_tables_match_oracle_props_2_to_7(precision, tol):
     """L_{p,r_c}(r), dL/dr and S_p(0) from the library's numerator polynomials N_p (host tables of the
     real-space row) vs the oracle's closed forms (SI Props. 2-7, (S67)); dL/dr vs central differences."""
-    p = binding.Plan([31.0] * 3, [32] * 3, 6, 12.024, [1, 2, 3, 4, 5, 6], precision=precision,
+    p = binding.Plan([31.0] * 3, [32] * 3, 6, 12.024, list(EXPONENTS), precision=precision,
                      host_only=True)
     i = p.info()
     moll = Mollifier(i["c"], i["r_c"])
     r = np.concatenate([np.linspace(0.05, 0.999, 400) * i["r_c"], [i["r_c"] * 1.0001, 3 * i["r_c"]]])
-    for pe in range(1, 7):
+    for pe in EXPONENTS:
         L, dL = p.eval_real(pe, r)
         ref = moll.L_phys(pe, r)
-        # error relative to r^-p (the numerator N_p is O(1), the singular factor is explicit)
-        assert np.max(np.abs(L - ref)[:-2] * r[:-2] ** pe) < tol, pe
+        # error relative to r^-p (the numerator N_p is O(1), the singular factor is explicit); the oracle's
+        # r^-p - S_p loses digits at small r, more for p = 8, 10 (third / fourth derivative terms)
+        tol_p = max(tol, {8: 2e-8, 10: 1e-6}.get(pe, 0.0))
+        assert np.max(np.abs(L - ref)[:-2] * r[:-2] ** pe) < tol_p, pe
         assert L[-1] == 0.0 and L[-2] == 0.0
         h = 1e-5
         fd = (moll.L_phys(pe, r[:-3] + h) - moll.L_phys(pe, r[:-3] - h)) / (2 * h)
-        assert np.max(np.abs(dL[:-3] - fd) * r[:-3] ** (pe + 1)) < max(tol, 2e-8) * 40, pe
+        assert np.max(np.abs(dL[:-3] - fd) * r[:-3] ** (pe + 1)) < max(tol_p, 2e-8) * 40, pe
         assert abs(p.self_coefficient(pe) - moll.S_zero(pe)) < 1e-9 * abs(moll.S_zero(pe)), pe
 
 

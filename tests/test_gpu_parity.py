@@ -80,6 +80,29 @@ def test_all_exponents_fp64_vs_oracle_A():
     check_vs(out, oracle_A(wl, out["info"]["r_c"]), 1e-9, 1e-9, label="p=1..6 f64 vs A")
 
 
+def test_exponents_8_and_10_fp64_vs_oracle_A():
+    """SI Section 6 (Theorem 2, Corollary 1): channels with p = 8 and p = 10 beside p = 1 and 6, charged
+    channels (zero mode (S79)), fp64 with w = 16 against the direct k-sum."""
+    rng = np.random.default_rng(78)
+    box, grid = [11.0, 12.5, 10.0], [18, 21, 16]
+    N = 50
+    wl = dict(pos=rng.uniform(0, 1, (N, 3)) * box, q=rng.normal(0, 0.5, (4, N)), exponents=[8, 1, 10, 6],
+              box=box, grid=grid, w=16, c=12.024, precision="f64")
+    out = run_gpu(wl)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), 1e-9, 1e-9, label="p=8,1,10,6 f64 vs A")
+
+
+@pytest.mark.parametrize("kernel_path", [0, 1])
+def test_exponents_8_and_10_fp32_vs_oracle_A(kernel_path):
+    """Config-3-shaped system (rock-salt sites, 8 neutralised latent channels, 64^3, w = 8) with the exponents
+    p = 8, 8, 10, 10, 1, 3, 6, 6: the fast fp32 kernels and the band-limited transform path with eight
+    channels and five distinct exponents, at north_star's fp32 gates."""
+    wl = workloads.make(3, n_atoms=6000)
+    wl["exponents"] = [8, 8, 10, 10, 1, 3, 6, 6]
+    out = run_gpu(wl, kernel_path=kernel_path)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), TOL_E32, TOL_F32, label="p=8,10 f32 vs A path%d" % kernel_path)
+
+
 # ---- configs 2, 3, 5: fp32 vs the definition ---------------------------------------------------
 
 @pytest.mark.parametrize("kernel_path", [0, 1])
@@ -483,18 +506,19 @@ def _run_real(wl, plan, accumulate_after_recip=False):
 @pytest.mark.parametrize("precision,tol", [("f64", 1e-9), ("f32", 2e-5)])
 def test_real_space_complement_vs_scaffold(precision, tol):
     """E_real - E_self, phi and F of pswf_lr_execute_real against the oracle
-    scaffold (plain pair loops over images, closed-form S_p of SI Props. 2-7), all six exponents,
+    scaffold (plain pair loops over images, closed-form S_p of SI Props. 2-7 and Corollary 1), all eight exponents,
     atoms across the periodic boundary, an anisotropic box."""
     from oracle.scaffold import real_space_parts
     rng = np.random.default_rng(21)
     box, grid, w = [12.0, 13.0, 14.0], [24, 24, 32], 6
     N = 150
     pos = rng.uniform(0, 1, (N, 3)) * box
-    q = rng.normal(0, 1, (6, N))
+    q = rng.normal(0, 1, (8, N))
     if precision == "f32":
         pos = pos.astype(np.float32).astype(np.float64)
         q = q.astype(np.float32).astype(np.float64)
-    wl = dict(pos=pos, q=q, exponents=[1, 2, 3, 4, 5, 6], box=box, grid=grid, w=w, c=12.024, precision=precision)
+    wl = dict(pos=pos, q=q, exponents=[1, 2, 3, 4, 5, 6, 8, 10], box=box, grid=grid, w=w, c=12.024,
+              precision=precision)
     plan = make_plan(wl, r_c=4.4)
     E, phi, F = _run_real(wl, plan)
     E_ref, phi_ref, F_ref = real_space_parts(pos, q, wl["exponents"], box, wl["c"], 4.4)
