@@ -5,6 +5,9 @@ TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).
 Definition (Eq. (5)-(6)), per channel a with exponent p:
 
     rho_a(k) = sum_j q_j^a e^{i k.r_j},                    k = 2 pi (m_x/L_x, m_y/L_y, m_z/L_z)
+               (general cell, "cell tensor Omega": rows a_1, a_2, a_3 of the 3x3 matrix h are the
+                lattice vectors, r = s h with fractional s, and k_m = 2 pi m h^-T so that k_m . r = 2 pi m . s;
+                V = |det h|.  `box` may be three edge lengths or such a 3x3 matrix everywhere below.)
     E        = 1/(2V) sum_a [ sum_{k in K} Phi^_p(k) |rho_a(k)|^2 + Phi0_p (Q_net^a)^2 ]
     phi_i^a  = dE/dq_i^a = (1/V) [ sum_K Phi^_p(k) Re(e^{-i k.r_i} rho_a(k)) + Phi0_p Q_net^a ]
     F_i      = -dE/dr_i (q fixed)
@@ -22,19 +25,31 @@ import numpy as np
 from .kernels import Mollifier
 
 
+def cell_matrix(box):
+    """3x3 cell matrix (rows = lattice vectors) from three edge lengths or a 3x3 array."""
+    box = np.asarray(box, dtype=np.float64)
+    return np.diag(box) if box.ndim == 1 else box.reshape(3, 3)
+
+
+def recip_vectors(box, m):
+    """k_m = 2 pi m h^-T (rows), Cartesian."""
+    return 2 * np.pi * np.asarray(m, dtype=np.float64) @ np.linalg.inv(cell_matrix(box)).T
+
+
 def mode_set(box, c, r_c, grid=None, half=False):
     """Integer mode vectors m (K,3) of the set K above.  half=True keeps one of each
     +-m pair (the first non-zero component positive)."""
-    box = np.asarray(box, dtype=np.float64)
+    cell = cell_matrix(box)
     kc = c / r_c
-    mmax = np.floor(kc * box / (2 * np.pi)).astype(int) + 1
+    # |m_d| = |a_d . k| / 2 pi <= |a_d| |k| / 2 pi
+    mmax = np.floor(kc * np.linalg.norm(cell, axis=1) / (2 * np.pi)).astype(int) + 1
     if grid is not None:
         # |m_d| < M_d/2  (strict: Nyquist planes excluded, reading R11)
         lim = (np.asarray(grid) - 1) // 2
         mmax = np.minimum(mmax, lim)
     ax = [np.arange(-mm, mm + 1) for mm in mmax]
     m = np.stack(np.meshgrid(*ax, indexing="ij"), axis=-1).reshape(-1, 3)
-    k = 2 * np.pi * m / box
+    k = recip_vectors(cell, m)
     kn = np.sqrt((k ** 2).sum(1))
     keep = (kn * r_c < c) & np.any(m != 0, axis=1)
     m = m[keep]
@@ -54,12 +69,12 @@ def direct_sums(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_mod
     """
     pos = np.asarray(pos, dtype=np.float64)
     q = np.atleast_2d(np.asarray(q, dtype=np.float64))
-    box = np.asarray(box, dtype=np.float64)
+    cell = cell_matrix(box)
     C, N = q.shape
-    V = float(np.prod(box))
+    V = float(abs(np.linalg.det(cell)))
     moll = Mollifier(c, r_c)
-    m = mode_set(box, c, r_c, grid, half=False)
-    k = 2 * np.pi * m / box                       # (K,3)
+    m = mode_set(cell, c, r_c, grid, half=False)
+    k = recip_vectors(cell, m)                    # (K,3)
     kn = np.sqrt((k ** 2).sum(1))
     kn_u, inv = np.unique(kn, return_inverse=True)   # Phi^ depends on |k| only
     idx = np.arange(N) if subset is None else np.asarray(subset)
@@ -124,12 +139,17 @@ def direct_sums_c(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_m
     """
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     q = np.ascontiguousarray(np.atleast_2d(q), dtype=np.float64)
-    box = np.ascontiguousarray(box, dtype=np.float64)
+    cell = cell_matrix(box)
     C, N = q.shape
     moll = Mollifier(c, r_c)
-    m = np.ascontiguousarray(mode_set(box, c, r_c, grid, half=True), dtype=np.int32)
+    m = np.ascontiguousarray(mode_set(cell, c, r_c, grid, half=True), dtype=np.int32)
     K = len(m)
-    kn = np.sqrt(((2 * np.pi * m / box) ** 2).sum(1))
+    kn = np.sqrt((recip_vectors(cell, m) ** 2).sum(1))
+    # the C routine takes fractional coordinates s = r h^-1 (k_m . r = 2 pi m . s), the reciprocal
+    # basis 2 pi h^-T (row d = the k vector of m = e_d) for the force, and the cell volume
+    frac = np.ascontiguousarray(pos @ np.linalg.inv(cell))
+    recip = np.ascontiguousarray(2 * np.pi * np.linalg.inv(cell).T)
+    V = float(abs(np.linalg.det(cell)))
     kn_u, inv = np.unique(kn, return_inverse=True)   # Phi^ depends on |k| only
     Ph = np.empty((C, K))
     cache = {}
@@ -147,7 +167,7 @@ def direct_sums_c(pos, q, exponents, box, c, r_c, grid=None, subset=None, zero_m
     def P(a, t=dp):
         return a.ctypes.data_as(t)
     rc = _lib().oracle_direct_sums(
-        ctypes.c_long(N), P(pos), ctypes.c_int(C), P(q), P(box),
+        ctypes.c_long(N), P(frac), ctypes.c_int(C), P(q), P(recip), ctypes.c_double(V),
         ctypes.c_long(K), P(m, ctypes.POINTER(ctypes.c_int32)), P(Ph), P(Phi0),
         ctypes.c_long(len(idx)), P(idx, ctypes.POINTER(ctypes.c_int64)),
         P(E_ch), P(phi), P(F))
@@ -170,11 +190,11 @@ def virial_direct(pos, q, exponents, box, c, r_c, grid=None, zero_mode=True):
     its own for it).  Returns the symmetric 3x3 tensor, summed over channels."""
     pos = np.asarray(pos, dtype=np.float64)
     q = np.atleast_2d(np.asarray(q, dtype=np.float64))
-    box = np.asarray(box, dtype=np.float64)
-    V = float(np.prod(box))
+    cell = cell_matrix(box)
+    V = float(abs(np.linalg.det(cell)))
     moll = Mollifier(c, r_c)
-    m = mode_set(box, c, r_c, grid, half=False)
-    k = 2 * np.pi * m / box
+    m = mode_set(cell, c, r_c, grid, half=False)
+    k = recip_vectors(cell, m)
     kn = np.sqrt((k ** 2).sum(1))
     rho = q @ np.exp(1j * pos @ k.T)               # (C, K)
     W = np.zeros((3, 3))

@@ -2,7 +2,8 @@
  *
  * TEST INFRASTRUCTURE ONLY (see oracle/__init__.py).  Shares nothing with the CUDA path.
  *
- * For every channel a (exponent p_a) and every mode k = 2 pi (mx/Lx, my/Ly, mz/Lz) of the
+ * For every channel a (exponent p_a) and every mode k_m = 2 pi m h^-T of the cell h (rows =
+ * lattice vectors; orthorhombic: k = 2 pi (mx/Lx, my/Ly, mz/Lz)) of the
  * HALF mode set passed in (one of each +-k pair; rho(-k) = conj rho(k) and Phi^ is even, so
  * each listed mode counts twice in the full sum of Eq. (5)):
  *
@@ -13,8 +14,9 @@
  *
  * Phi^_a(k) (already r_c^(3-p) S^_p(k r_c), (S60)) and the zero-mode constants Phi0_a are
  * computed by oracle/kernels.py and passed in.  The only rearrangement of the definition is
- * e^{ik.r} = e^{i kx x} e^{i ky y} e^{i kz z}, with the three factors tabulated per atom by
- * direct cos/sin calls (no recurrences).
+ * e^{ik.r} = e^{2 pi i m.s} = e^{2 pi i mx sx} e^{2 pi i my sy} e^{2 pi i mz sz} in the fractional
+ * coordinates s = r h^-1 the caller passes, with the three factors tabulated per atom by direct
+ * cos/sin calls (no recurrences); the force needs the Cartesian k_m = sum_d m_d recip[d][.].
  */
 #include <math.h>
 #ifndef M_PI
@@ -44,12 +46,12 @@ static void phase_table(double r, double L, int mmax, double *tab) {
     }
 }
 
-int oracle_direct_sums(long N, const double *pos /*[N][3]*/, int C, const double *q /*[C][N]*/,
-                       const double *box /*[3]*/, long K, const int32_t *m /*[K][3]*/,
+int oracle_direct_sums(long N, const double *pos /*[N][3] fractional*/, int C, const double *q /*[C][N]*/,
+                       const double *recip /*[3][3] = 2 pi h^-T*/, double V, long K, const int32_t *m /*[K][3]*/,
                        const double *Phi /*[C][K]*/, const double *Phi0 /*[C]*/, long n_sub,
                        const int64_t *sub /*[n_sub]*/, double *E_ch /*[C]*/,
                        double *phi /*[C][n_sub]*/, double *F /*[n_sub][3]*/) {
-    const double V = box[0] * box[1] * box[2];
+    const double box[3] = {1.0, 1.0, 1.0};   /* fractional coordinates: period 1 in every direction */
     int mmax[3] = {0, 0, 0};
     for (long k = 0; k < K; ++k)
         for (int d = 0; d < 3; ++d)
@@ -135,8 +137,11 @@ int oracle_direct_sums(long N, const double *pos /*[N][3]*/, int C, const double
                     double t_re = pr * re + pi * im, t_im = pr * im - pi * re;
                     double w = Phi[(long)a * K + k];
                     ph += w * t_re;
-                    for (int d = 0; d < 3; ++d)
-                        g[d] += w * t_im * (2.0 * M_PI * (double)m[3 * k + d] / box[d]);
+                    for (int d = 0; d < 3; ++d) {
+                        const double kd = (double)m[3 * k + 0] * recip[0 * 3 + d] + (double)m[3 * k + 1] * recip[1 * 3 + d] +
+                                          (double)m[3 * k + 2] * recip[2 * 3 + d];
+                        g[d] += w * t_im * kd;
+                    }
                 }
                 phi[(long)a * n_sub + s] = (2.0 * ph + Phi0[a] * Qn[a]) / V;
                 for (int d = 0; d < 3; ++d) Fi[d] -= q[(long)a * N + i] * 2.0 * g[d] / V;

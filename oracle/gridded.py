@@ -19,6 +19,16 @@ PAPER.md:76, 1099).  The window is evaluated from the Legendre series of psi_0^{
 import numpy as np
 from .pswf import PSWF0
 from .kernels import Mollifier
+from .direct import cell_matrix, recip_vectors
+
+
+def inverse_cell(box):
+    """h^-1 for fractional coordinates s = r h^-1 (rows of h = lattice vectors).  An orthorhombic box gets
+    exactly diag(1/L), so that s = x * (1/L) as reading R4 states."""
+    cell = cell_matrix(box)
+    if np.count_nonzero(cell - np.diag(np.diag(cell))) == 0:
+        return np.diag(1.0 / np.diag(cell))
+    return np.linalg.inv(cell)
 
 
 def stencil(pos, box, grid, w):
@@ -29,9 +39,12 @@ def stencil(pos, box, grid, w):
     u' = s * M - w/2;  i0 = ceil(u');  delta = i0 - u';  z_t = (t + delta) / (w/2) - 1, each
     operation rounded to float64 separately."""
     pos = np.asarray(pos, dtype=np.float64)
-    box = np.asarray(box, dtype=np.float64)
     grid = np.asarray(grid)
-    s = pos * (1.0 / box)
+    Hi = inverse_cell(box)
+    # general cell ("cell tensor Omega", PAPER.md:76): the grid lives in fractional coordinates,
+    # s_d = (r_0 Hi[0][d] + r_1 Hi[1][d]) + r_2 Hi[2][d], products and sums rounded separately in this
+    # order; for an orthorhombic box the two zero terms leave s = x * (1/L) bit for bit
+    s = (pos[:, 0:1] * Hi[0][None, :] + pos[:, 1:2] * Hi[1][None, :]) + pos[:, 2:3] * Hi[2][None, :]
     s = s - np.floor(s)                           # wrap into [0, 1)
     s = np.where(s >= 1.0, 0.0, s)                # guard the rounding case s == 1
     u = s * grid.astype(np.float64) - w / 2.0
@@ -43,28 +56,31 @@ def stencil(pos, box, grid, w):
     return i0, z
 
 
-def window_hat_1d(psi_w, w, h, L, M):
-    """W^_pswf(k_d) = omega lambda_0 psi_0^{c_w}(omega k_d / c_w), omega = w h / 2, at the M
-    signed DFT frequencies of one dimension.  Eq. (22)."""
+def window_hat_1d(psi_w, w, M):
+    """One factor of W^_pswf, Eq. (22), at the M signed DFT indices m of one dimension:
+    lambda_0 psi_0^{c_w}(omega k_d / c_w) with omega k_d = (w h / 2)(2 pi m / L) = pi w m / M -- a function
+    of the index only, in any cell; the lengths omega_d = w h_d / 2 are collected in multiplier()."""
     m = np.fft.fftfreq(M, d=1.0 / M)              # 0,1,..,-1 signed integers
-    kd = 2 * np.pi * m / L
-    omega = w * h / 2.0
-    arg = omega * kd / psi_w.c
-    val = omega * psi_w.lambda0 * psi_w(np.clip(arg, -1, 1))
-    return m, kd, np.where(np.abs(arg) <= 1.0, val, np.nan)
+    arg = np.pi * w * m / (M * psi_w.c)
+    val = psi_w.lambda0 * psi_w(np.clip(arg, -1, 1))
+    return m, np.where(np.abs(arg) <= 1.0, val, np.nan)
 
 
 def multiplier(p, box, grid, w, c, r_c, c_w, zero_mode=True):
     """D_p(m) on the full (Mx,My,Mz) DFT grid (readings R10, R11).  Eq. (25)."""
-    box = np.asarray(box, dtype=np.float64)
+    cell = cell_matrix(box)
     grid = np.asarray(grid)
-    h = box / grid
+    V = float(abs(np.linalg.det(cell)))
+    hvol = V / np.prod(grid)                      # volume of a grid cell (h_x h_y h_z when orthorhombic)
     psi_w = PSWF0(c_w)
     moll = Mollifier(c, r_c)
-    ms, ks, Wh = zip(*[window_hat_1d(psi_w, w, h[d], box[d], grid[d]) for d in range(3)])
-    KX, KY, KZ = np.meshgrid(*ks, indexing="ij")
-    kn = np.sqrt(KX ** 2 + KY ** 2 + KZ ** 2)
-    What = Wh[0][:, None, None] * Wh[1][None, :, None] * Wh[2][None, None, :]
+    ms, Wh = zip(*[window_hat_1d(psi_w, w, grid[d]) for d in range(3)])
+    MX, MY, MZ = np.meshgrid(*ms, indexing="ij")
+    kvec = recip_vectors(cell, np.stack([MX, MY, MZ], axis=-1).reshape(-1, 3))
+    kn = np.sqrt((kvec ** 2).sum(1)).reshape(tuple(grid))
+    # W^ = prod_d omega_d lambda_0 psi(.), prod_d omega_d = (w/2)^3 x (grid-cell volume): the window is a
+    # tensor product in fractional coordinates, its transform carries the Jacobian |det h|
+    What = (w / 2.0) ** 3 * hvol * Wh[0][:, None, None] * Wh[1][None, :, None] * Wh[2][None, None, :]
     nyq = np.zeros(tuple(grid), dtype=bool)
     for d in range(3):
         if grid[d] % 2 == 0:
@@ -81,7 +97,7 @@ def multiplier(p, box, grid, w, c, r_c, c_w, zero_mode=True):
         raise ValueError("window transform used outside its band (grid too coarse for c_w)")
     if zero_mode:
         D[0, 0, 0] = moll.Phi0(p) / What[0, 0, 0] ** 2
-    return D * np.prod(h) / np.prod(grid)
+    return D * hvol / np.prod(grid)
 
 
 def spread(pos, q, box, grid, w, c_w):
@@ -107,13 +123,13 @@ def spread(pos, q, box, grid, w, c_w):
 def gather(phig, pos, box, grid, w, c_w):
     """phi_i^a = sum_g W(x_g - r_i) phi_g^a and its gradient w.r.t. r_i (window derivative)."""
     grid = np.asarray(grid)
-    box = np.asarray(box, dtype=np.float64)
-    h = box / grid
+    Hi = inverse_cell(box)
     psi_w = PSWF0(c_w)
     i0, z = stencil(pos, box, grid, w)
     Wd = psi_w(z)
-    # d/dr_i psi((x_g - r_i)/omega) = -psi'(z)/omega, omega = w h/2
-    dWd = -psi_w.deriv(z, 1) / (w * h[None, :, None] / 2.0)
+    # derivative along the fractional coordinate s_d: z = 2 (t + i0 - s_d M_d + w/2)/w - 1, dz/ds_d = -2 M_d/w
+    # (orthorhombic: d/dr = (1/L) d/ds = -psi'(z)/omega, omega = w h/2); Cartesian gradient below
+    dWd = -psi_w.deriv(z, 1) * (2.0 * grid[None, :, None] / w)
     C = phig.shape[0]
     N = len(i0)
     phi = np.zeros((C, N))
@@ -131,6 +147,8 @@ def gather(phig, pos, box, grid, w, c_w):
             grad[a, j, 0] = np.einsum("i,j,k,ijk->", dx, wy, wz, blk)
             grad[a, j, 1] = np.einsum("i,j,k,ijk->", wx, dy, wz, blk)
             grad[a, j, 2] = np.einsum("i,j,k,ijk->", wx, wy, dz, blk)
+    # d/dr_e = sum_d (ds_d/dr_e) d/ds_d = sum_d Hi[e][d] d/ds_d
+    grad = np.einsum("ed,and->ane", Hi, grad)
     return phi, grad
 
 
@@ -163,7 +181,7 @@ def gridded(pos, q, exponents, box, grid, w, c, r_c, c_w, zero_mode=True, interm
 
 def default_r_c(box, grid, c, eta=0.5):
     """Reading R2: r_c such that max_d h_d = eta pi r_c / c  (Eq. (29))."""
-    h = np.asarray(box, dtype=np.float64) / np.asarray(grid)
+    h = np.linalg.norm(cell_matrix(box), axis=1) / np.asarray(grid)    # |a_d| / M_d
     return float(c * h.max() / (eta * np.pi))
 
 

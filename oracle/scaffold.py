@@ -12,7 +12,15 @@ import itertools
 import numpy as np
 from scipy.special import erfc
 from .kernels import Mollifier
-from .direct import direct_sums
+from .direct import direct_sums, cell_matrix
+
+
+def image_range(cell, r):
+    """Per lattice direction, the largest |n_d| whose image can come within r: ceil(r / width_d) with
+    width_d = V / |a_e x a_f| the distance between the cell faces spanned by the other two vectors."""
+    V = abs(np.linalg.det(cell))
+    width = np.array([V / np.linalg.norm(np.cross(cell[(d + 1) % 3], cell[(d + 2) % 3])) for d in range(3)])
+    return np.ceil(r / width).astype(int)
 
 
 def real_space_complement(pos, q, p, box, moll):
@@ -20,13 +28,13 @@ def real_space_complement(pos, q, p, box, moll):
     L_{p,r_c} vanishes beyond r_c, so only images within r_c are visited."""
     pos = np.asarray(pos, dtype=np.float64)
     q = np.asarray(q, dtype=np.float64)
-    box = np.asarray(box, dtype=np.float64)
-    nmax = np.ceil(moll.r_c / box).astype(int)
+    cell = cell_matrix(box)
+    nmax = image_range(cell, moll.r_c)
     E = 0.0
     d0 = pos[:, None, :] - pos[None, :, :]
     qq = q[:, None] * q[None, :]
     for n in itertools.product(*[range(-k, k + 1) for k in nmax]):
-        d = d0 + np.asarray(n) * box
+        d = d0 + np.asarray(n, dtype=np.float64) @ cell
         r = np.sqrt((d ** 2).sum(-1))
         mask = (r > 0) & (r < moll.r_c)
         if n == (0, 0, 0):
@@ -45,16 +53,16 @@ def real_space_parts(pos, q, exponents, box, c, r_c, fd=1e-6, subset=None):
     ALL atoms) and E is None: the sampled check of large systems."""
     pos = np.asarray(pos, dtype=np.float64)
     q = np.atleast_2d(np.asarray(q, dtype=np.float64))
-    box = np.asarray(box, dtype=np.float64)
+    cell = cell_matrix(box)
     moll = Mollifier(c, r_c)
     N = len(pos)
     phi = np.zeros_like(q)
     F = np.zeros((N, 3))
-    nmax = np.ceil(r_c / box).astype(int)
+    nmax = image_range(cell, r_c)
     rows = np.arange(N) if subset is None else np.asarray(subset)
     d0 = pos[None, :, :] - pos[rows, None, :]       # d0[i, j] = r_j - r_rows[i]
     for n in itertools.product(*[range(-k, k + 1) for k in nmax]):
-        d = d0 + np.asarray(n) * box
+        d = d0 + np.asarray(n, dtype=np.float64) @ cell
         r = np.sqrt((d ** 2).sum(-1))
         mask = (r > 0) & (r < r_c)
         if not mask.any():
@@ -122,13 +130,13 @@ def brute_force_image_sum(pos, q, p, box, nmax):
     """1/2 sum_{|n_d|<=nmax} sum_{i,j}' q_i q_j / |r_ij + n.L|^p  (absolutely convergent for p > 3)."""
     pos = np.asarray(pos, dtype=np.float64)
     q = np.asarray(q, dtype=np.float64)
-    box = np.asarray(box, dtype=np.float64)
+    cell = cell_matrix(box)
     d0 = pos[:, None, :] - pos[None, :, :]
     qq = q[:, None] * q[None, :]
     E = 0.0
     rng = range(-nmax, nmax + 1)
     for n in itertools.product(rng, rng, rng):
-        d = d0 + np.asarray(n) * box
+        d = d0 + np.asarray(n, dtype=np.float64) @ cell
         r2 = (d ** 2).sum(-1)
         mask = r2 > 0
         E += 0.5 * np.sum(qq[mask] * r2[mask] ** (-p / 2.0))

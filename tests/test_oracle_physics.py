@@ -289,3 +289,106 @@ def test_virial_direct_matches_strain_derivative_of_energy():
     assert np.allclose(Wm[0, 2], -W[0, 2], atol=1e-10 * np.abs(W).max())
     assert np.allclose(Wm[1, 2], W[1, 2], atol=1e-10 * np.abs(W).max())
     assert np.allclose(np.diag(Wm), np.diag(W), atol=1e-10 * np.abs(W).max())
+
+
+# ---- general (triclinic) cells: "cell tensor Omega", PAPER.md:76 ------------------------------
+
+_SHEAR = np.array([[1, 0, 0], [1, 1, 0], [0, -1, 1]])     # unimodular: T h spans the same lattice as h
+
+
+def test_madelung_nacl_in_sheared_and_primitive_cells(golden):
+    """The rock-salt Madelung constant from (S65) does not depend on how the lattice is described: the
+    conventional cube re-described by sheared lattice vectors (same lattice, same 8 ions), and the
+    two-ion primitive fcc cell with 60-degree angles."""
+    pos, q, box = _rock_salt()
+    cell = _SHEAR @ np.diag(box)
+    E = scaffold.total_energy(pos, q, 1, cell, 30.0, 1.3)
+    assert abs(-E / 4.0 - golden["madelung_nacl"]) < 2e-9
+    prim = np.array([[1.0, 1.0, 0.0], [0.0, 1.0, 1.0], [1.0, 0.0, 1.0]])
+    E2 = scaffold.total_energy(np.array([[0.0, 0, 0], [1.0, 0, 0]]), np.array([1.0, -1.0]), 1, prim, 30.0, 0.9)
+    assert abs(-E2 - golden["madelung_nacl"]) < 2e-9         # one ion pair: E = -M
+
+
+@pytest.mark.parametrize("p", [1, 3, 6, 8])
+def test_oracle_A_is_invariant_under_relabelling_the_lattice(p):
+    """Oracle A alone: E, phi and F of a random charged system are the same for the box diag(L) and for
+    the sheared description T diag(L) of the same lattice (the mode SET is the same reciprocal lattice,
+    only its integer labels change)."""
+    rng = np.random.default_rng(300 + p)
+    box = np.array([6.0, 7.0, 6.5])
+    pos = rng.uniform(0, 1, (7, 3)) * box
+    q = rng.normal(0, 1, (1, 7))
+    a = direct_sums(pos, q, [p], box, 12.024, 2.0)
+    b = direct_sums(pos, q, [p], _SHEAR @ np.diag(box), 12.024, 2.0)
+    assert abs(a[0] - b[0]) < 1e-12 * abs(a[0])
+    assert np.allclose(a[2], b[2], rtol=0, atol=1e-12 * np.abs(a[2]).max())
+    assert np.allclose(a[3], b[3], rtol=0, atol=1e-12 * np.abs(a[3]).max())
+
+
+def _triclinic_system(seed=11, N=8):
+    rng = np.random.default_rng(seed)
+    cell = np.array([[8.0, 0.0, 0.0], [2.1, 7.5, 0.0], [-1.3, 1.7, 9.0]])
+    pos = rng.uniform(0, 1, (N, 3)) @ cell
+    q = rng.normal(0, 0.7, (3, N))
+    q[0] -= q[0].mean()
+    return pos, q, cell, [1, 4, 6]
+
+
+def test_triclinic_forces_potentials_and_c_oracle():
+    """Triclinic cell: F = -dE/dr and phi = dE/dq by central differences of E; the C routine equals the
+    numpy sums; a lattice translation of one atom changes nothing."""
+    pos, q, cell, ex = _triclinic_system()
+    c, r_c = 12.024, 2.6
+    E, Ech, phi, F = direct_sums(pos, q, ex, cell, c, r_c)
+    h = 1e-5
+    for i, d in ((0, 0), (3, 1), (5, 2)):
+        pp, pm = pos.copy(), pos.copy()
+        pp[i, d] += h
+        pm[i, d] -= h
+        fd = -(direct_sums(pp, q, ex, cell, c, r_c)[0] - direct_sums(pm, q, ex, cell, c, r_c)[0]) / (2 * h)
+        assert abs(fd - F[i, d]) < 1e-7 * np.abs(F).max()
+    qp, qm = q.copy(), q.copy()
+    qp[1, 2] += h
+    qm[1, 2] -= h
+    fdq = (direct_sums(pos, qp, ex, cell, c, r_c)[0] - direct_sums(pos, qm, ex, cell, c, r_c)[0]) / (2 * h)
+    assert abs(fdq - phi[1, 2]) < 1e-7 * np.abs(phi).max()
+    Ec, Echc, phic, Fc = direct_sums_c(pos, q, ex, cell, c, r_c)
+    assert abs(E - Ec) < 1e-13 * abs(E) and np.allclose(F, Fc, atol=1e-13 * np.abs(F).max(), rtol=0)
+    assert np.allclose(phi, phic, atol=1e-13 * np.abs(phi).max(), rtol=0)
+    moved = pos.copy()
+    moved[2] += cell[1] - cell[2]
+    assert abs(direct_sums(moved, q, ex, cell, c, r_c)[0] - E) < 1e-12 * abs(E)
+    assert np.abs(F.sum(0)).max() < 1e-12 * np.abs(F).max()
+
+
+def test_triclinic_total_energy_vs_brute_force_and_invariance():
+    """(S65) in a triclinic cell: p = 6 against the plain image sum, and (c, r_c)-invariance for a charged
+    p = 1 channel (background convention (S73) with V = |det h|)."""
+    pos, q, cell, _ = _triclinic_system(seed=12, N=6)
+    E = scaffold.total_energy(pos, q[1], 6, cell, 24.0, 1.2)
+    nmax = 6
+    brute = scaffold.brute_force_image_sum(pos, q[1], 6, cell, nmax)
+    R = (nmax + 0.5) * 7.0
+    tail = 0.5 * q[1].sum() ** 2 * 4 * np.pi * R ** -3.0 / (3.0 * abs(np.linalg.det(cell)))
+    assert abs(E - brute) < max(2e-6 * abs(E), 3 * abs(tail)), (E, brute, tail)
+    E1 = scaffold.total_energy(pos, q[2], 1, cell, 30.0, 1.1)
+    E2 = scaffold.total_energy(pos, q[2], 1, cell, 26.0, 1.35)
+    assert abs(E1 - E2) < 2e-9 * max(1.0, abs(E1))
+
+
+def test_triclinic_virial_is_the_strain_derivative():
+    """All six components of W_ab = -dE/d(eps_ab) in a triclinic cell by central differences of E under
+    r -> (1 + eps) r, h -> h (1 + eps)^T (symmetric eps)."""
+    from oracle.direct import virial_direct
+    pos, q, cell, ex = _triclinic_system(seed=13, N=6)
+    c, r_c = 12.024, 2.6
+    W = virial_direct(pos, q, ex, cell, c, r_c)
+    assert np.allclose(W, W.T, atol=1e-13)
+    e = 1e-6
+    for a, b in ((0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)):
+        eps = np.zeros((3, 3))
+        eps[a, b] += 0.5
+        eps[b, a] += 0.5
+        Ep = direct_sums(pos @ (np.eye(3) + e * eps).T, q, ex, cell @ (np.eye(3) + e * eps).T, c, r_c)[0]
+        Em = direct_sums(pos @ (np.eye(3) - e * eps).T, q, ex, cell @ (np.eye(3) - e * eps).T, c, r_c)[0]
+        assert abs(-(Ep - Em) / (2 * e) - W[a, b]) < 2e-6 * np.abs(W).max(), (a, b)
