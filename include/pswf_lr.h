@@ -103,6 +103,16 @@ int pswf_lr_plan_create(pswf_lr_plan** plan, const double box[3], const int grid
 int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int grid[3], int w,
                            double c, const int* exponents, int n_channels, const pswf_lr_opts* opts);
 
+/* The same for a general (triclinic) periodic cell -- "positions, species and the cell tensor".
+ * cell[9], row-major: row d is the lattice vector a_d (right-handed, det > 0); r = s h with fractional
+ * s, k_m = 2 pi m h^-T, V = det h.  The grid has M_d points along a_d and the separable PSWF window
+ * acts on the fractional coordinates; |a_d| / M_d takes the place of the grid spacing h_d in Eq. (29)
+ * and in the defaults of r_c and c_window.  Positions, forces and the virial are Cartesian.  A diagonal
+ * cell is the orthorhombic box of pswf_lr_plan_create_ex (same arithmetic).  pswf_lr_execute_real is
+ * limited to orthorhombic cells (PSWF_LR_ERR_GRID_TOO_COARSE otherwise). */
+int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const int grid[3], int w,
+                             double c, const int* exponents, int n_channels, const pswf_lr_opts* opts);
+
 /* One evaluation, asynchronous on `stream` (a cudaStream_t; NULL = default stream).  No host
  * synchronisation and no host<->device copy happens inside (workspaces grow, with a sync, only
  * when n_atoms exceeds the capacity seen so far).

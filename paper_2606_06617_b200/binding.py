@@ -43,7 +43,7 @@ class Info(ctypes.Structure):
                 ("band_limited_fft", ctypes.c_int), ("band_kmax", ctypes.c_int * 3)]
 
 
-EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_execute", "pswf_lr_execute_host",
+EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_plan_create_cell", "pswf_lr_execute", "pswf_lr_execute_host",
            "pswf_lr_submit_host", "pswf_lr_wait_host",
            "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient", "pswf_lr_suggest_parameters", "pswf_lr_set_virial", "pswf_lr_virial",
            "pswf_lr_channel_energies", "pswf_lr_get_info", "pswf_lr_set_profiling", "pswf_lr_stage_ms",
@@ -66,6 +66,9 @@ def lib():
         L.pswf_lr_plan_create.argtypes = [ctypes.POINTER(vp), dp, ctypes.POINTER(ip), ip, ctypes.c_double,
                                           ctypes.POINTER(ip), ip]
         L.pswf_lr_plan_create_ex.argtypes = L.pswf_lr_plan_create.argtypes + [ctypes.POINTER(Opts)]
+        L.pswf_lr_plan_create_cell.argtypes = L.pswf_lr_plan_create_ex.argtypes
+        L.pswf_lr_submit_host.argtypes = [vp, ip, vp, vp, dp, vp, vp]
+        L.pswf_lr_wait_host.argtypes = [vp]
         L.pswf_lr_execute.argtypes = [vp, ip, vp, vp, vp, vp, vp, vp]
         L.pswf_lr_execute_host.argtypes = [vp, ip, vp, vp, dp, vp, vp, vp]
         L.pswf_lr_execute_real.argtypes = [vp, ip, vp, vp, vp, vp, vp, ip, vp]
@@ -127,11 +130,17 @@ class Plan:
         self.precision = {"f32": PSWF_LR_F32, "f64": PSWF_LR_F64}[precision]
         o = Opts(r_c, c_window, self.precision, int(max_atoms), zero_mode, kernel_path, poly_eps,
                  1 if host_only else 0, 1 if debug_spectrum else 0)
-        box_a = (ctypes.c_double * 3)(*[float(b) for b in box])
         grid_a = (ctypes.c_int * 3)(*[int(g) for g in grid])
         ex = (ctypes.c_int * len(exponents))(*[int(p) for p in exponents])
-        _check(L.pswf_lr_plan_create_ex(ctypes.byref(self._h), box_a, grid_a, int(w), float(c), ex,
-                                        len(exponents), ctypes.byref(o)))
+        box_np = np.asarray(box, dtype=np.float64)
+        if box_np.ndim == 2:     # 3x3 cell, rows = lattice vectors
+            cell_a = (ctypes.c_double * 9)(*[float(b) for b in box_np.reshape(9)])
+            _check(L.pswf_lr_plan_create_cell(ctypes.byref(self._h), cell_a, grid_a, int(w), float(c), ex,
+                                              len(exponents), ctypes.byref(o)))
+        else:
+            box_a = (ctypes.c_double * 3)(*[float(b) for b in box_np])
+            _check(L.pswf_lr_plan_create_ex(ctypes.byref(self._h), box_a, grid_a, int(w), float(c), ex,
+                                            len(exponents), ctypes.byref(o)))
         self.n_channels = len(exponents)
         self.grid = [int(g) for g in grid]
 

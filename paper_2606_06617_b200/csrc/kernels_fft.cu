@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(kXYThreads, 1)
 
   // scale by D_p(m) = (h^3 / Mtot) Phi^_p(|k|) / W^(k)^2 inside the ball, zero elsewhere; E_c
   const int slot = P.chan_slot[c];
-  const float kzv = P.kfac[2] * (float)kz;
+  const float fzf = (float)kz;
   const float wz = P.invW2[2][kz];
   const float herm = kz == 0 ? 1.f : 2.f;
   double e = 0.0;
@@ -223,7 +223,9 @@ __global__ void __launch_bounds__(kXYThreads, 1)
     const int fx = ix <= Mx / 2 ? ix : ix - Mx, fy = iy <= My / 2 ? iy : iy - My;
     float2 v = make_float2(0.f, 0.f);
     if (abs(fy) <= X.kmaxy) {
-      const float kx = P.kfac[0] * (float)fx, ky = P.kfac[1] * (float)fy;
+      const float kx = P.recip[0] * (float)fx + P.recip[3] * (float)fy + P.recip[6] * fzf;
+      const float ky = P.recip[1] * (float)fx + P.recip[4] * (float)fy + P.recip[7] * fzf;
+      const float kzv = P.recip[2] * (float)fx + P.recip[5] * (float)fy + P.recip[8] * fzf;
       const float kn = sqrtf(kx * kx + ky * ky + kzv * kzv);
       const float x = kn * P.x_per_k;
       const bool zero_mode = (ix | iy | kz) == 0;
@@ -400,7 +402,7 @@ __global__ void __launch_bounds__(kXYThreads, 1)
   fft_axis_t<NT, M, false, pitch, 1>(s, nkx, lgk, keptx, tw);
 
   const int slot = P.chan_slot[c];
-  const float kzv = P.kfac[2] * (float)kz;
+  const float fzf = (float)kz;
   const float wz = P.invW2[2][kz];
   const float herm = kz == 0 ? 1.f : 2.f;
   double e = 0.0;
@@ -411,7 +413,9 @@ __global__ void __launch_bounds__(kXYThreads, 1)
     const int fx = ix <= M / 2 ? ix : ix - M, fy = iy <= M / 2 ? iy : iy - M;
     float2 v = make_float2(0.f, 0.f);
     if (abs(fy) <= X.kmaxy) {
-      const float kx = P.kfac[0] * (float)fx, ky = P.kfac[1] * (float)fy;
+      const float kx = P.recip[0] * (float)fx + P.recip[3] * (float)fy + P.recip[6] * fzf;
+      const float ky = P.recip[1] * (float)fx + P.recip[4] * (float)fy + P.recip[7] * fzf;
+      const float kzv = P.recip[2] * (float)fx + P.recip[5] * (float)fy + P.recip[8] * fzf;
       const float kn = sqrtf(kx * kx + ky * ky + kzv * kzv);
       const float x = kn * P.x_per_k;
       const bool zero_mode = (ix | iy | kz) == 0;

@@ -38,6 +38,8 @@ namespace pswf {
 namespace {
 
 constexpr int SW = 8;        // stencil slots per dimension
+
+struct HinvF { float m[9]; };   // h^-1 (row e, column d = ds_d/dr_e), kernel parameter
 constexpr int ZSEG = 32;     // cells per z segment: one lane per cell boundary pair
 
 template <int CB> struct VecOf;
@@ -160,7 +162,8 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
     k_gather_rows(int n, int C, int cb0, int Mx, int My, int Mz, int nseg, int nbx, int nby, int recf,
                   const int* __restrict__ start, const float* __restrict__ rec, const float* __restrict__ drec,
                   const int* __restrict__ perm, const typename VecOf<CB>::type* __restrict__ gridt,
-                  float* __restrict__ phi, float* __restrict__ Facc, int accumulate_F) {
+                  float* __restrict__ phi, float* __restrict__ Facc, int accumulate_F,
+                  const __grid_constant__ HinvF Hi) {
   using V = typename VecOf<CB>::type;
   extern __shared__ __align__(16) float s_all[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -255,9 +258,12 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
           if (cb0 + c < C) phi[(size_t)(cb0 + c) * n + perm_l] = pv[c];
       }
       if (Facc) {
+        // the derivative records are along the fractional coordinates: F_e = sum_d hinv[e][d] F^s_d
+        float fx = f.x, fy = f.y, fz = f.z;
+        frac_to_cart(Hi.m, fx, fy, fz);
         float* fp = Facc + 3 * (size_t)perm_l;
-        if (accumulate_F) { fp[0] += f.x; fp[1] += f.y; fp[2] += f.z; }
-        else { fp[0] = f.x; fp[1] = f.y; fp[2] = f.z; }
+        if (accumulate_F) { fp[0] += fx; fp[1] += fy; fp[2] += fz; }
+        else { fp[0] = fx; fp[1] = fy; fp[2] = fz; }
       }
     }
     __syncwarp();
@@ -456,6 +462,8 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, bool hav
   const int recf = stencil_rec_floats(p->C);
   const size_t smem = sizeof(float) * GBX * GBY * (size_t)gather_warp_floats(recf);
   float* gi = (float*)p->d_gridi;
+  HinvF Hi;
+  for (int i = 0; i < 9; ++i) Hi.m[i] = (float)p->hinv[i];
   int pass = 0;
   for (int cb0 = 0; cb0 < p->C; cb0 += 4, ++pass) {
     const int left = p->C - cb0;
@@ -469,7 +477,7 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, bool hav
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \
     kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nbx, nby, recf, p->d_count,        \
                                                (const float*)p->d_rec, (const float*)p->d_drec, p->d_perm,  \
-                                               (const V*)gi, phi, F, acc);                                  \
+                                               (const V*)gi, phi, F, acc, Hi);                              \
     gi += Mtot * CBV;                                                                                       \
   } while (0)
     if (left >= 4) PSWF_GATHER(4, 4);

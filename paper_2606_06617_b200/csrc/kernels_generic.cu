@@ -19,14 +19,11 @@ __global__ void k_bin_count(int n, const T* __restrict__ pos, GridGeom<T> g, int
                             int* __restrict__ key, int* __restrict__ rank) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  int s[3];
+  int s[3], i0[3];
+  double delta[3];
+  stencil_3d(pos + 3 * (size_t)i, g.hinv, g.M, g.w, i0, delta);
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    int i0;
-    double delta;
-    stencil_1d((double)pos[3 * (size_t)i + d], g.invL[d], g.M[d], g.w, i0, delta);
-    s[d] = wrap_index(i0, g.M[d]);
-  }
+  for (int d = 0; d < 3; ++d) s[d] = wrap_index(i0[d], g.M[d]);
   int k = (s[0] * g.M[1] + s[1]) * g.M[2] + s[2];
   key[i] = k;
   rank[i] = atomicAdd(&count[k], 1);
@@ -137,13 +134,13 @@ __global__ void k_scatter(int n, int C, int cap, const T* __restrict__ pos, cons
   if (i >= n) return;
   int dst = start[key[i]] + rank[i];
   perm[dst] = i;
+  int i0[3];
+  double delta[3];
+  stencil_3d(pos + 3 * (size_t)i, g.hinv, g.M, g.w, i0, delta);
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    int i0;
-    double delta;
-    stencil_1d((double)pos[3 * (size_t)i + d], g.invL[d], g.M[d], g.w, i0, delta);
-    si0[(size_t)d * cap + dst] = i0;
-    sdelta[(size_t)d * cap + dst] = (T)delta;
+    si0[(size_t)d * cap + dst] = i0[d];
+    sdelta[(size_t)d * cap + dst] = (T)delta[d];
   }
   for (int c = 0; c < C; ++c) sq[(size_t)c * cap + dst] = q[(size_t)c * n + i];
 }
@@ -219,7 +216,9 @@ __global__ void k_scale(ScaleParams<T> P, Cplx<T>* __restrict__ spec, double* __
     int fz = iz;
     bool nyq = ((P.M[0] % 2 == 0) && ix == P.M[0] / 2) || ((P.M[1] % 2 == 0) && iy == P.M[1] / 2) ||
                ((P.M[2] % 2 == 0) && iz == P.M[2] / 2);
-    T kx = P.kfac[0] * (T)fx, ky = P.kfac[1] * (T)fy, kz = P.kfac[2] * (T)fz;
+    const T kx = P.recip[0] * (T)fx + P.recip[3] * (T)fy + P.recip[6] * (T)fz;
+    const T ky = P.recip[1] * (T)fx + P.recip[4] * (T)fy + P.recip[7] * (T)fz;
+    const T kz = P.recip[2] * (T)fx + P.recip[5] * (T)fy + P.recip[8] * (T)fz;
     T kn = sqrt(kx * kx + ky * ky + kz * kz);
     T x = kn * P.x_per_k;
     is_zero_mode = (ix == 0 && iy == 0 && iz == 0);
@@ -309,7 +308,7 @@ __global__ void k_gather_ref(int n, int C, int cap, GridGeom<T> g, const int* __
     int d = t / w, tt = t - d * w;
     T xi = (T)2 * sdelta[(size_t)d * cap + j] - (T)1;
     wts[wid][d * kMaxW + tt] = horner_panel(g.wcoef, w, tt, g.wdeg, xi);
-    wts[wid][(3 + d) * kMaxW + tt] = horner_panel(g.wdcoef, w, tt, g.wdeg - 1, xi) * g.dxi_dr[d];
+    wts[wid][(3 + d) * kMaxW + tt] = horner_panel(g.wdcoef, w, tt, g.wdeg - 1, xi) * g.dxi_ds[d];
   }
   __syncwarp();
   const int i0x = si0[j], i0y = si0[(size_t)cap + j], i0z = si0[2 * (size_t)cap + j];
@@ -344,6 +343,7 @@ __global__ void k_gather_ref(int n, int C, int cap, GridGeom<T> g, const int* __
     if (lane == 0 && phi) phi[(size_t)c * n + dst] = v;
   }
   if (lane == 0 && F) {
+    frac_to_cart(g.hinv_t, fx, fy, fz);   // the derivative weights are along the fractional coordinates
     F[3 * (size_t)dst + 0] = fx;
     F[3 * (size_t)dst + 1] = fy;
     F[3 * (size_t)dst + 2] = fz;

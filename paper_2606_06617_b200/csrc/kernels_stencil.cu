@@ -127,11 +127,13 @@ __global__ void __launch_bounds__(kRecThreads) k_records(int n, int C, int recf,
       for (int u = 0; u < 4; ++u) qq[u] = c0 + u < C ? __ldg(q + (size_t)(c0 + u) * n + i) : 0.f;
       reinterpret_cast<float4*>(r + 3 * SW)[c0 >> 2] = make_float4(qq[0], qq[1], qq[2], qq[3]);
     }
+    int i0v[3];
+    double deltav[3];
+    stencil_3d(px, g.hinv, g.M, g.w, i0v, deltav);
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-      int i0;
-      double delta;
-      stencil_1d((double)px[d], g.invL[d], g.M[d], g.w, i0, delta);
+      const int i0 = i0v[d];
+      const double delta = deltav[d];
       const int s = wrap_index(i0, g.M[d]);
       const float xi = 2.f * (float)delta - 1.f;
       float v[SW], dv[SW];
@@ -145,7 +147,7 @@ __global__ void __launch_bounds__(kRecThreads) k_records(int n, int C, int recf,
         }
         a = fmaf(a, xi, P.c[0][t]);
         v[t] = a;
-        dv[t] = b * g.dxi_dr[d];
+        dv[t] = b * g.dxi_ds[d];   // derivative along the fractional coordinate; the gather converts
       }
       rotate8(v, s);
       rotate8(dv, s);

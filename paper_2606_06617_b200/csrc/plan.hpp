@@ -37,7 +37,7 @@ struct ScaleParams {
   int chan_slot[kMaxChannels];
   T chan_D0[kMaxChannels];   // multiplier of the m = 0 mode per channel (0 when dropped)
   T slot_pre[kMaxSlots];   // r_c^(3-p) * constant prefactor of each slot
-  T kfac[3];           // 2 pi / L_d
+  T recip[9];          // reciprocal basis 2 pi h^-T: k_e = sum_d m_d recip[3 d + e] (diagonal 2 pi / L_d when orthorhombic)
   T x_per_k;           // r_c / c
   T c;                 // mollifier bandwidth
   T base;              // h_x h_y h_z / M_tot
@@ -51,8 +51,9 @@ template <class T>
 struct GridGeom {
   int M[3];
   int w;
-  double invL[3];      // 1 / L_d   (binning is done in double)
-  T dxi_dr[3];         // d xi / d r_d = -2 / h_d
+  double hinv[9];      // h^-1, s = r h^-1 (binning is done in double, reading R4); diag(1/L_d) when orthorhombic
+  T hinv_t[9];         // the same in plan precision: Cartesian gradient from fractional components
+  T dxi_ds[3];         // d xi / d s_d = -2 M_d
   int wdeg;            // window polynomial degree
   const T* wcoef;      // [(wdeg+1)][w]
   const T* wdcoef;     // [wdeg][w]
@@ -86,7 +87,10 @@ struct pswf_lr_plan {
   // resolved parameters
   int precision = 0, w = 0, C = 0, zero_mode = 0, kernel_path = 0;
   int M[3] = {0, 0, 0};
-  double L[3] = {0, 0, 0}, h[3] = {0, 0, 0};
+  double L[3] = {0, 0, 0}, h[3] = {0, 0, 0};   // |a_d| (edge lengths) and |a_d| / M_d
+  double cell[9] = {0}, hinv[9] = {0};         // lattice vectors (rows) and h^-1; diagonal when orthorhombic
+  double volume = 0;                           // |det h|
+  bool triclinic = false;
   double c = 0, r_c = 0, c_w = 0, eta = 0, poly_eps = 0;
   int chan_p[pswf::kMaxChannels] = {0};
   int chan_slot[pswf::kMaxChannels] = {0};

@@ -126,8 +126,11 @@ GridGeom<T> make_geom(const pswf_lr_plan* p) {
   GridGeom<T> g;
   for (int d = 0; d < 3; ++d) {
     g.M[d] = p->M[d];
-    g.invL[d] = 1.0 / p->L[d];
-    g.dxi_dr[d] = (T)(-2.0 / p->h[d]);
+    g.dxi_ds[d] = (T)(-2.0 * p->M[d]);
+  }
+  for (int i = 0; i < 9; ++i) {
+    g.hinv[i] = p->hinv[i];
+    g.hinv_t[i] = (T)p->hinv[i];
   }
   g.w = p->w;
   g.wdeg = p->wt.degree;
@@ -156,14 +159,20 @@ template <class T>
 ScaleParams<T> make_scale(const pswf_lr_plan* p) {
   ScaleParams<T> P;
   memset(&P, 0, sizeof(P));
-  double hv = 1, mt = 1;
+  double mt = 1, ltab = 1;
   for (int d = 0; d < 3; ++d) {
     P.M[d] = p->M[d];
-    P.kfac[d] = (T)(2 * kPi / p->L[d]);
     P.invW2[d] = (const T*)p->d_invW2[d];
-    hv *= p->h[d];
     mt *= p->M[d];
+    ltab *= p->L[d];
   }
+  // reciprocal basis 2 pi h^-T: k_e = sum_d m_d recip[3 d + e], recip[3 d + e] = 2 pi hinv[e][d]
+  for (int d = 0; d < 3; ++d)
+    for (int e = 0; e < 3; ++e) P.recip[3 * d + e] = (T)(2 * kPi * p->hinv[3 * e + d]);
+  // D_p(m) = (V / Mtot^2) Phi^ / W^2 with W^ = prod_d omega_d lambda_0 psi(.), prod_d omega_d = (w/2)^3 V / Mtot.
+  // The 1-D tables carry omega_d = w |a_d| / (2 M_d); in a skewed cell prod |a_d| > V, corrected here.
+  const double vcorr = (ltab / p->volume) * (ltab / p->volume);
+  const double hv = p->volume / mt * vcorr;
   P.Mzh = p->M[2] / 2 + 1;
   P.C = p->C;
   P.nslots = (int)p->distinct_p.size();
@@ -340,7 +349,28 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
                            const int* exponents, int n_channels, const pswf_lr_opts* opts) {
   if (!plan) return PSWF_LR_ERR_INVALID_ARG;
   *plan = nullptr;
-  if (!box || !grid || !exponents) return PSWF_LR_ERR_INVALID_ARG;
+  if (!box) return PSWF_LR_ERR_INVALID_ARG;
+  const double cell[9] = {box[0], 0, 0, 0, box[1], 0, 0, 0, box[2]};
+  return pswf_lr_plan_create_cell(plan, cell, grid, w, c, exponents, n_channels, opts);
+}
+
+int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const int grid[3], int w, double c,
+                             const int* exponents, int n_channels, const pswf_lr_opts* opts) {
+  if (!plan) return PSWF_LR_ERR_INVALID_ARG;
+  *plan = nullptr;
+  if (!cell || !grid || !exponents) return PSWF_LR_ERR_INVALID_ARG;
+  // lattice vectors a_d = rows of the cell; |a_d| plays the role of the box length L_d wherever only the
+  // grid spacing along a lattice direction matters (Eq. (29), band limits, 1-D window tables)
+  double box[3], det;
+  {
+    const double* h = cell;
+    det = h[0] * (h[4] * h[8] - h[5] * h[7]) - h[1] * (h[3] * h[8] - h[5] * h[6]) + h[2] * (h[3] * h[7] - h[4] * h[6]);
+    for (int d = 0; d < 3; ++d) {
+      box[d] = std::sqrt(h[3 * d] * h[3 * d] + h[3 * d + 1] * h[3 * d + 1] + h[3 * d + 2] * h[3 * d + 2]);
+      if (!std::isfinite(box[d])) return PSWF_LR_ERR_INVALID_ARG;
+    }
+    if (!(det > 0) || !(det > 1e-6 * box[0] * box[1] * box[2])) return PSWF_LR_ERR_INVALID_ARG;   // right-handed, not degenerate
+  }
   if (n_channels < 1 || n_channels > kMaxChannels) return PSWF_LR_ERR_INVALID_ARG;
   if (w < 2 || w > kMaxW || (w % 2) != 0) return PSWF_LR_ERR_INVALID_ARG;
   if (!(c >= 2.0 && c <= 60.0)) return PSWF_LR_ERR_INVALID_ARG;
@@ -386,6 +416,22 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       p->L[d] = box[d];
       p->h[d] = box[d] / grid[d];
       hmax = std::max(hmax, p->h[d]);
+    }
+    p->volume = det;
+    p->triclinic = false;
+    for (int i = 0; i < 9; ++i) {
+      p->cell[i] = cell[i];
+      if (i % 4 != 0 && cell[i] != 0.0) p->triclinic = true;
+    }
+    if (!p->triclinic) {   // exactly 1/L: the binning of an orthorhombic box is s = x * (1/L) (reading R4)
+      for (int i = 0; i < 9; ++i) p->hinv[i] = 0.0;
+      for (int d = 0; d < 3; ++d) p->hinv[4 * d] = 1.0 / cell[4 * d];
+    } else {               // adjugate / determinant
+      const double* h = cell;
+      const double adj[9] = {h[4] * h[8] - h[5] * h[7], h[2] * h[7] - h[1] * h[8], h[1] * h[5] - h[2] * h[4],
+                             h[5] * h[6] - h[3] * h[8], h[0] * h[8] - h[2] * h[6], h[2] * h[3] - h[0] * h[5],
+                             h[3] * h[7] - h[4] * h[6], h[1] * h[6] - h[0] * h[7], h[0] * h[4] - h[1] * h[3]};
+      for (int i = 0; i < 9; ++i) p->hinv[i] = adj[i] / det;
     }
     // reading R2: default r_c puts eta = 0.5 in Eq. (29)
     p->r_c = o.r_c > 0 ? o.r_c : c * hmax / (0.5 * kPi);
@@ -455,24 +501,25 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
       for (int d = 0; d < 3; ++d) {
         p->real_R[d] = (int)std::floor(p->r_c / p->h[d]) + 1;
         if (!(p->r_c < 0.5 * p->L[d])) p->real_ok = false;
+        if (p->triclinic) p->real_ok = false;   // the pair kernel's minimum image is per Cartesian axis
       }
       // count modes in the ball (half spectrum), for info / roofline bytes
       long long cnt = 0;
       const double kc2 = (c / p->r_c) * (c / p->r_c);
       for (int ix = 0; ix < p->M[0]; ++ix) {
-        int fx = ix <= p->M[0] / 2 ? ix : ix - p->M[0];
+        const int fx = ix <= p->M[0] / 2 ? ix : ix - p->M[0];
         if ((p->M[0] % 2 == 0) && ix == p->M[0] / 2) continue;
-        double kx = 2 * kPi * fx / p->L[0];
         for (int iy = 0; iy < p->M[1]; ++iy) {
-          int fy = iy <= p->M[1] / 2 ? iy : iy - p->M[1];
+          const int fy = iy <= p->M[1] / 2 ? iy : iy - p->M[1];
           if ((p->M[1] % 2 == 0) && iy == p->M[1] / 2) continue;
-          double ky = 2 * kPi * fy / p->L[1];
-          double rem = kc2 - kx * kx - ky * ky;
-          if (rem <= 0) continue;
           for (int iz = 0; iz <= p->M[2] / 2; ++iz) {
             if ((p->M[2] % 2 == 0) && iz == p->M[2] / 2) continue;
-            double kz = 2 * kPi * iz / p->L[2];
-            if (kz * kz < rem) ++cnt;
+            double k2 = 0;
+            for (int e = 0; e < 3; ++e) {   // k_e = 2 pi sum_d m_d hinv[e][d]
+              const double ke = 2 * kPi * (fx * p->hinv[3 * e] + fy * p->hinv[3 * e + 1] + iz * p->hinv[3 * e + 2]);
+              k2 += ke * ke;
+            }
+            if (k2 < kc2) ++cnt;   // (the m = 0 entry is counted: it carries the zero-mode constant)
           }
         }
       }

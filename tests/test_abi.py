@@ -195,3 +195,28 @@ def test_suggested_parameters_meet_the_tolerance(eps):
     assert eF <= 2 * eps / 3 and eE <= 2 * eps / 3
     if w > 4:
         assert err(w - 2)[1] > 0.5 * eps / 3      # a narrower window would (nearly) exhaust the spreading share
+
+
+def test_plan_create_cell_validation_and_info():
+    """pswf_lr_plan_create_cell: left-handed or degenerate cells are refused; |a_d| / M_d is the spacing that
+    enters Eq. (29) and the default r_c; a diagonal cell gives the orthorhombic plan's parameters."""
+    ok = dict(grid=[16] * 3, w=6, c=12.024, exponents=[1], host_only=True)
+
+    def code(cell):
+        try:
+            binding.Plan(np.asarray(cell, float), **ok).destroy()
+            return 0
+        except binding.PswfLrError as e:
+            return e.code
+    assert code([[10, 0, 0], [2, 9, 0], [1, -1, 11]]) == 0
+    assert code([[10, 0, 0], [0, -9, 0], [0, 0, 11]]) == binding.ERR_INVALID_ARG       # left-handed
+    assert code([[10, 0, 0], [20, 0, 0], [0, 0, 11]]) == binding.ERR_INVALID_ARG       # degenerate
+    assert code([[10, 0, 0], [0, float("nan"), 0], [0, 0, 11]]) == binding.ERR_INVALID_ARG
+    a = binding.Plan([10.0, 12.0, 9.0], **ok)
+    b = binding.Plan(np.diag([10.0, 12.0, 9.0]), **ok)
+    ia, ib = a.info(), b.info()
+    assert ia["r_c"] == ib["r_c"] and ia["c_window"] == ib["c_window"] and ia["modes_in_ball"] == ib["modes_in_ball"]
+    t = binding.Plan(np.array([[10.0, 0, 0], [6.0, 8.0, 0], [0, 0, 9.0]]), **ok)      # |a_2| = 10
+    assert abs(t.info()["r_c"] - 12.024 * (10.0 / 16) / (0.5 * np.pi)) < 1e-12
+    for p in (a, b, t):
+        p.destroy()

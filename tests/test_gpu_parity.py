@@ -103,6 +103,60 @@ def test_exponents_8_and_10_fp32_vs_oracle_A(kernel_path):
     check_vs(out, oracle_A(wl, out["info"]["r_c"]), TOL_E32, TOL_F32, label="p=8,10 f32 vs A path%d" % kernel_path)
 
 
+# ---- general (triclinic) cells, PAPER.md:76 ------------------------------------------------------
+
+def _triclinic_workload(N, grid, w, precision, seed=91, C=3):
+    rng = np.random.default_rng(seed)
+    cell = np.array([[20.0, 0.0, 0.0], [4.5, 19.0, 0.0], [-3.0, 3.5, 21.0]])
+    pos = rng.uniform(-0.3, 1.3, (N, 3)) @ cell          # some atoms outside the cell: wrapped internally
+    q = rng.normal(0, 0.5, (C, N))
+    q[0] -= q[0].mean()
+    if precision == "f32":
+        pos = pos.astype(np.float32).astype(np.float64)
+        q = q.astype(np.float32).astype(np.float64)
+    return dict(pos=pos, q=q, exponents=[1, 6, 3][:C], box=cell, grid=grid, w=w, c=12.024, precision=precision)
+
+
+@pytest.mark.parametrize("kernel_path", [0, 1])
+def test_triclinic_fp64_vs_oracle_B(kernel_path):
+    """Triclinic cell, fp64: the same discretisation on the CPU (grid in fractional coordinates) to 1e-10."""
+    wl = _triclinic_workload(80, [20, 18, 22], 6, "f64")
+    out = run_gpu(wl, kernel_path=kernel_path)
+    i = out["info"]
+    ref = G.gridded(wl["pos"], wl["q"], wl["exponents"], wl["box"], wl["grid"], wl["w"], wl["c"], i["r_c"],
+                    i["c_window"])
+    check_vs(out, ref, TOL_64, TOL_64, label="triclinic f64 vs B")
+
+
+def test_triclinic_fp64_w16_vs_oracle_A():
+    wl = _triclinic_workload(60, [22, 20, 24], 16, "f64")
+    out = run_gpu(wl)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), 1e-9, 1e-9, label="triclinic f64 w16 vs A")
+
+
+@pytest.mark.parametrize("kernel_path,grid", [(0, [32, 32, 32]), (0, [24, 32, 40]), (1, [32, 32, 32])])
+def test_triclinic_fp32_vs_oracle_A(kernel_path, grid):
+    """fp32 at north_star's gates in a triclinic cell: cell-sorted spread / gather kernels, band-limited
+    transform path (32^3) and dense transform path (24 x 32 x 40), reference kernels."""
+    wl = _triclinic_workload(4000, grid, 8, "f32")
+    out = run_gpu(wl, kernel_path=kernel_path)
+    if kernel_path == 0:
+        assert out["info"]["fast_stencil"] == 1
+        assert out["info"]["band_limited_fft"] == (1 if grid == [32, 32, 32] else 0)
+    check_vs(out, oracle_A(wl, out["info"]["r_c"]), TOL_E32, TOL_F32, label="triclinic f32 vs A %s" % grid)
+
+
+def test_diagonal_cell_equals_box():
+    """pswf_lr_plan_create_cell with a diagonal cell is the orthorhombic plan: same energies and forces."""
+    wl = workloads.make(2, n_atoms=900)
+    a = run_gpu(wl)
+    wl2 = dict(wl)
+    wl2["box"] = np.diag(wl["box"])
+    b = run_gpu(wl2)
+    assert abs(a["E"] - b["E"]) <= 1e-6 * abs(a["E"])
+    assert rel(b["F"], a["F"]) < 1e-5 and rel(b["phi"], a["phi"]) < 1e-5
+
+
 # ---- configs 2, 3, 5: fp32 vs the definition ---------------------------------------------------
 
 @pytest.mark.parametrize("kernel_path", [0, 1])
@@ -607,6 +661,25 @@ def test_virial_reciprocal_vs_oracle():
         W_ref = virial_direct(pp, qq, wl["exponents"], box, wl["c"], plan.info()["r_c"], grid=grid)
         err = np.abs(W - W_ref).max() / np.abs(W_ref).max()
         print("virial %s: max rel err %.2e" % (precision, err))
+        assert err <= tol
+        plan.destroy()
+
+
+def test_virial_triclinic_all_components_vs_oracle():
+    """Triclinic cell: all six components (the off-diagonal ones are no longer zero by symmetry of the
+    mode set) against the oracle's k-sum virial, itself pinned by strain derivatives in a triclinic cell."""
+    from oracle.direct import virial_direct
+    for precision, w, tol in [("f64", 16, 1e-9), ("f32", 8, 1e-4)]:
+        wl = _triclinic_workload(60, [24, 24, 32], w, precision, seed=92)
+        plan = make_plan(wl)
+        plan.set_virial(True)
+        run_gpu(wl, plan=plan)
+        W = _virial(plan)
+        W_ref = virial_direct(wl["pos"], wl["q"], wl["exponents"], wl["box"], wl["c"], plan.info()["r_c"],
+                              grid=wl["grid"])
+        assert np.abs(W_ref[0, 1]) > 1e-3 * np.abs(W_ref).max()
+        err = np.abs(W - W_ref).max() / np.abs(W_ref).max()
+        print("triclinic virial %s: max rel err %.2e" % (precision, err))
         assert err <= tol
         plan.destroy()
 
