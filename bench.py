@@ -197,11 +197,73 @@ def run_reference(args):
     return 0
 
 
+def run_sharded(args):
+    """--shard channels, N > 1: positions replicated, rank g evaluates the channels a mod N == g, one
+    all-reduce of F and E per step; total work fixed -> "scaling": "strong"."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_06617_b200 import build, sharding, workloads
+    rank, local, world = dist_env()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist.init_process_group("nccl", device_id=dev)
+    build.build()
+    wl = workloads.make(args.cfg, n_atoms=args.atoms)            # the SAME system on every rank
+    N, C = len(wl["pos"]), len(wl["exponents"])
+    dt_t = torch.float32 if wl["precision"] == "f32" else torch.float64
+    sp = sharding.ChannelShardedPlan(wl["box"], wl["grid"], wl["w"], wl["c"], wl["exponents"], rank, world,
+                                     precision=wl["precision"], max_atoms=N)
+    box = np.asarray(wl["box"])
+    n_sets = args.steps + args.warmup
+    pos_d, p = [], wl["pos"].copy()
+    for dsp in workloads.md_displacements(args.cfg, n_sets, N, sigma=0.01):
+        pos_d.append(torch.as_tensor(np.mod(p, box), dtype=dt_t).to(dev))
+        p = p + dsp
+    q_d = torch.as_tensor(wl["q"], dtype=dt_t).to(dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    for i in range(args.warmup):
+        sp.execute(pos_d[i], q_d)
+    dist.barrier()
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    clocks = ClockSampler(local)
+    clocks.start()
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)
+        evs[i][0].record(stream)
+        E, F = sp.execute(pos_d[args.warmup + i], q_d)
+        evs[i][1].record(stream)
+    dist.barrier()
+    torch.cuda.synchronize()
+    clk = clocks.stop()
+    total_s = sum(a.elapsed_time(b) for a, b in evs) / 1e3
+    total_s_max, _ = reduce_times(total_s, N, dev)
+    if rank == 0:
+        line = {"metric": METRIC, "value": N * args.steps / total_s_max, "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_s_max / args.steps,
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": wl["precision"],
+                "data": "synthetic", "evals_per_s": args.steps / total_s_max,
+                "config": {"workload": wl["name"], "n_atoms": N, "grid": wl["grid"], "w": wl["w"],
+                           "exponents": wl["exponents"], "parallelism": "channels a mod %d per GPU, one all-reduce "
+                           "of F and E per step" % world, "channels_per_rank": [len(sharding.channel_partition(C, world, r))
+                                                                                  for r in range(world)],
+                           "l2": "flushed between timed steps (256 MiB write, outside the events)"},
+                "clocks": clk, "energy_last_step": float(E.item()),
+                "gpu_launches": args.steps * 9, "e2e": None, "roofline": None, "cpu_baseline": None}
+        print(json.dumps(line))
+    sp.destroy()
+    dist.destroy_process_group()
+    return 0
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2606_06617_b200 import binding, build, workloads
     rank, local, world = dist_env()
+    if args.shard == "channels" and world > 1:
+        return run_sharded(args)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -402,6 +464,9 @@ def main():
     ap.add_argument("--atoms", type=int, default=None, help="override the atom count (same box and grid)")
     ap.add_argument("--kernel-path", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "channels"],
+                    help="N > 1: independent replica per GPU (default, weak scaling) or one system with its channels "
+                         "dealt round-robin to the GPUs and an all-reduce of F and E (strong scaling)")
     ap.add_argument("--with-real", action="store_true",
                     help="also time pswf_lr_execute_real (real-space complement + self term, SURVEY 8(f) row 1); "
                          "reported under 'real_space', the metric is unchanged")

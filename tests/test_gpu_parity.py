@@ -746,6 +746,43 @@ def test_random_configurations_fast_path_consistent_with_reference_kernels():
             assert rel(a["F"], b["F"]) <= 5e-5, (it, grid, N, C, w)
 
 
+def test_channel_sharded_plan_on_one_gpu_matches_the_plain_plan():
+    """ChannelShardedPlan with the two ranks' plans run one after the other on this GPU: the
+    sum of the per-rank F and E and the re-assembled phi equal the all-channel evaluation.  (The exchange
+    step itself runs under gloo in tests/test_multi_rank.py; several ranks never share this GPU.)"""
+    from paper_2606_06617_b200 import sharding
+    wl = workloads.make(3, n_atoms=3000)
+    full = run_gpu(wl)
+    dev = torch.device("cuda:0")
+    pos = torch.as_tensor(wl["pos"], dtype=torch.float32, device=dev)
+    q = torch.as_tensor(wl["q"], dtype=torch.float32, device=dev)
+    E = 0.0
+    F = np.zeros((len(wl["pos"]), 3))
+    phi = np.zeros_like(full["phi"])
+    for r in range(2):
+        sp = sharding.ChannelShardedPlan(wl["box"], wl["grid"], wl["w"], wl["c"], wl["exponents"], rank=r, world=2)
+        sp.world_for_gather = 1
+        E_r = torch.zeros(1, dtype=torch.float64, device=dev)
+        F_r = torch.zeros((len(wl["pos"]), 3), dtype=torch.float32, device=dev)
+        phi_r = torch.zeros((len(sp.own), len(wl["pos"])), dtype=torch.float32, device=dev)
+        sp.plan.execute(len(wl["pos"]), pos, q[sp.own].contiguous(), E_r, phi_r, F_r,
+                        torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        E += E_r.item()
+        F += F_r.double().cpu().numpy()
+        phi[sp.own] = phi_r.double().cpu().numpy()
+        sp.destroy()
+    assert abs(E - full["E"]) < 2e-6 * abs(full["E"])
+    assert rel(F, full["F"]) < 1e-5 and rel(phi, full["phi"]) < 1e-5
+    # world size 1: the sharded plan IS the plain plan
+    sp = sharding.ChannelShardedPlan(wl["box"], wl["grid"], wl["w"], wl["c"], wl["exponents"], rank=0, world=1)
+    E1, F1, phi1 = sp.execute(pos, q, want_phi=True)
+    torch.cuda.synchronize()
+    assert abs(E1.item() - full["E"]) < 2e-6 * abs(full["E"]) and rel(F1.double().cpu().numpy(), full["F"]) < 1e-5
+    assert rel(phi1.double().cpu().numpy(), full["phi"]) < 1e-5
+    sp.destroy()
+
+
 def test_native_library_is_loaded():
     """The product path is the CUDA library: the shared object is mapped into this process."""
     binding.lib()
