@@ -29,12 +29,13 @@ __global__ void k_bin_count(int n, const T* __restrict__ pos, GridGeom<T> g, int
   rank[i] = atomicAdd(&count[k], 1);
 }
 
-// Exclusive scan of count[0..n) in place in ONE pass (decoupled look-back): a tile of 4096 counts per
+// Exclusive scan of count[0..n) in place in ONE pass (decoupled look-back): a tile of 16384 counts per
 // CTA; tiles are handed out by a ticket counter, so every tile a CTA waits for is already running.
 // state[0] = ticket counter, state[1 + t] = (status << 32) | value of tile t with status 1 = the
 // tile's own sum, 2 = inclusive prefix up to and including the tile; zeroed before each launch.
-constexpr int kScanThreads = 512;
-constexpr int kScanItems = 8;
+constexpr int kScanThreads = 1024;
+constexpr int kScanItems = 16;   // 16384 counts per tile: 128 tiles at 128^3, one wave, a 4x shorter look-back chain than 4096
+int scan_tile_size() { return kScanThreads * kScanItems; }
 
 __global__ void __launch_bounds__(kScanThreads) k_scan_lookback(int n, int* __restrict__ data,
                                                                 unsigned long long* __restrict__ state,
@@ -48,9 +49,11 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_lookback(int n, int* __re
   int v[kScanItems];
   int sum = 0;
   if (base + kScanItems <= n) {
-    const int4 a = *reinterpret_cast<const int4*>(data + base);
-    const int4 b = *reinterpret_cast<const int4*>(data + base + 4);
-    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+#pragma unroll
+    for (int j = 0; j < kScanItems; j += 4) {
+      const int4 a = *reinterpret_cast<const int4*>(data + base + j);
+      v[j] = a.x; v[j + 1] = a.y; v[j + 2] = a.z; v[j + 3] = a.w;
+    }
   } else {
 #pragma unroll
     for (int j = 0; j < kScanItems; ++j) v[j] = (base + j < n) ? data[base + j] : 0;
@@ -113,8 +116,9 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_lookback(int n, int* __re
     int o[kScanItems];
 #pragma unroll
     for (int j = 0; j < kScanItems; ++j) { o[j] = run; run += v[j]; }
-    *reinterpret_cast<int4*>(data + base) = make_int4(o[0], o[1], o[2], o[3]);
-    *reinterpret_cast<int4*>(data + base + 4) = make_int4(o[4], o[5], o[6], o[7]);
+#pragma unroll
+    for (int j = 0; j < kScanItems; j += 4)
+      *reinterpret_cast<int4*>(data + base + j) = make_int4(o[j], o[j + 1], o[j + 2], o[j + 3]);
   } else {
 #pragma unroll
     for (int j = 0; j < kScanItems; ++j) {

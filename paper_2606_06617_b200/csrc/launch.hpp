@@ -7,6 +7,7 @@ namespace pswf {
 template <class T>
 void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, bool scatter,
                      cudaStream_t st);
+int scan_tile_size();   // counts per tile of the single-pass scan (sizes its state array)
 template <class T>
 void launch_spread_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, cudaStream_t st);
 template <class T>

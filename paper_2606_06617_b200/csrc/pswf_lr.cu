@@ -549,7 +549,7 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
       if (!rc) rc = dev_alloc(&p->d_spec, 2 * rs * Mhalf * p->C, &b);
       if (!rc && stencil_path_supported(p)) rc = dev_alloc(&p->d_gridi, gather_grid_bytes(p), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_count, sizeof(int) * (Mtot + 1), &b);
-      p->n_scan_blocks = (int)((Mtot + 4095) / 4096);
+      p->n_scan_blocks = (int)((Mtot + scan_tile_size() - 1) / scan_tile_size());
       if (!rc) rc = dev_alloc((void**)&p->d_scan_state, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
       if (!rc) rc = dev_alloc((void**)&p->d_Ereal, sizeof(double), &b);
