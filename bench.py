@@ -116,7 +116,7 @@ def measured_peaks():
 
 def profiled_traffic(kernel):
     """DRAM bytes per launch of a kernel from the committed ncu --set full capture (profiles/), or None."""
-    path = os.path.join(ROOT, "profiles", "r1f_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
     try:
         return int(json.load(open(path))["dram_bytes_per_launch"][kernel])
     except Exception:
@@ -158,9 +158,26 @@ def cpu_baseline(wl, r_c, seconds_target=15.0):
     t0 = time.perf_counter()
     direct_sums_c(pos[:n_big], q[:, :n_big], wl["exponents"], wl["box"], wl["c"], r_c, grid=wl["grid"])
     dt3 = time.perf_counter() - t0
-    return {"value": n_big / dt3, "unit": UNIT, "cores": c_threads(), "kind": "oracle",
-            "sample": "oracle A (direct k-sum, float64, oracle/direct_sum.c): E, phi, F of the first %d atoms "
-                      "of the workload over all %d half-space modes, %.1f s" % (n_big, K, dt3)}
+    out = {"value": n_big / dt3, "unit": UNIT, "cores": c_threads(), "kind": "oracle",
+           "sample": "oracle A (direct k-sum, float64, oracle/direct_sum.c): E, phi, F of the first %d atoms "
+                     "of the workload over all %d half-space modes, %.1f s" % (n_big, K, dt3)}
+    # oracle B: the same gridded algorithm on the CPU (like-for-like), on a bounded sample of the atoms
+    # over the FULL grid; the multipliers D_p (plan-time, independent of the atoms) are built once, untimed
+    from oracle import gridded as G
+    n_b = int(min(len(pos), 100000))
+    c_w = G.default_c_w(wl["w"])
+    mult, tm = {}, {}
+    G.gridded_c(pos[:2000], q[:, :2000], wl["exponents"], wl["box"], wl["grid"], wl["w"], wl["c"], r_c, c_w,
+                multipliers=mult)
+    G.gridded_c(pos[:n_b], q[:, :n_b], wl["exponents"], wl["box"], wl["grid"], wl["w"], wl["c"], r_c, c_w,
+                timings=tm, multipliers=mult)
+    out["gridded"] = {"value": n_b / tm["total"], "unit": UNIT, "cores": G.c_threads(), "kind": "oracle",
+                      "seconds": {k: round(v, 3) for k, v in tm.items()},
+                      "sample": "oracle B (spread / FFT / multiply / inverse FFT / gather in float64: numpy + "
+                                "oracle/gridded_sum.c) on the first %d atoms of the workload over the full %s grid, "
+                                "%.1f s; the grid-sized steps do not shrink with the sample, so this UNDERSTATES "
+                                "the full-size rate" % (n_b, "x".join(str(g) for g in wl["grid"]), tm["total"])}
+    return out
 
 
 def run_reference(args):
@@ -310,12 +327,14 @@ def run_ours(args):
     clocks = ClockSampler(local)
     clocks.start()
     barrier()
+    launches0 = plan.info()
     for i in range(args.steps):
         flush.fill_(i & 0xFF)                       # L2 flush between timed iterations (not timed)
         evs[i][0].record(stream)
         plan.execute(N, pos_d[args.warmup + i], q_d, E_d, phi_d, F_d, sp)
         evs[i][1].record(stream)
     barrier()
+    launches1 = plan.info()
     clk = clocks.stop()
     step_ms = [a.elapsed_time(b) for a, b in evs]
     total_s = sum(step_ms) / 1e3
@@ -393,11 +412,11 @@ def run_ours(args):
     roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": ach / alu_peak,
                 "traffic": profiled_traffic(dom) if (args.cfg == 4 and args.atoms is None and args.kernel_path == 0) else None,
-                "traffic_source": "profiles/r1f_ncu_full.md (dram__bytes_read+write of one launch, config 4)",
+                "traffic_source": "profiles/r2_ncu_full.md (dram__bytes_read+write of one launch, config 4)",
                 "alg_flops": flops_alg[dom], "alg_bytes": bytes_alg[dom],
                 "peak_source": "148 SM x 128 FMA/clk x 2 x %.0f MHz (DESIGN.md §6)" % sm_max,
-                "time_source": "CUDA events around the %s stage on the execute stream (for gather: the 12 us "
-                               "transposing interleave + k_gather_rows), mean over the timed steps" % dom,
+                "time_source": "CUDA events around the %s stage on the execute stream (one kernel launch per channel "
+                               "group), mean over the timed steps" % dom,
                 "hbm_achieved_gbs": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9,
                 "hbm_frac": bytes_alg[dom] / (stage_ms[dom] * 1e-3) / 1e9 / peak_gbs}
     stages = {k: {"ms": stage_ms[k], "alg_bytes": bytes_alg[k],
@@ -412,11 +431,10 @@ def run_ours(args):
     if not args.no_cpu_baseline:
         cb = cpu_baseline(wl, info["r_c"])
 
-    # this library's own kernels per evaluation (cuFFT's 6 kernels and 3 memsets not counted):
-    # fast: bin_count, scan, perm, records, spread, scale, finalize, interleave, gather (C <= 4)
-    # ref:  bin_count, scan, scatter, spread_ref, scale, finalize, gather_ref
-    groups = (C + 3) // 4
-    launches_per_step = {"ref": 7, "fast": 6 + 3 * groups}["fast" if args.kernel_path == 0 else "ref"]
+    # launches inside the timed region, counted by the library at its launch sites (pswf_lr_info)
+    own_launches = launches1["own_kernel_launches"] - launches0["own_kernel_launches"]
+    if args.kernel_path == 0 and wl["precision"] == "f32":
+        assert info["fast_stencil"] == 1, "bench: the cell-sorted fp32 kernels did not run"
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -435,7 +453,12 @@ def run_ours(args):
                 "blocking_call": {"value": atoms_all * args.steps / e2e_sync_s_max, "unit": UNIT,
                                   "ms_per_step": 1e3 * e2e_sync_s_max / args.steps,
                                   "api": "pswf_lr_execute_host (copy-in, evaluation, copy-out in series)"}},
-        "gpu_launches": args.steps * launches_per_step,
+        "gpu_launches": own_launches,
+        "launches": {"own_kernels": own_launches, "memsets": launches1["memsets"] - launches0["memsets"],
+                     "cufft_execs": launches1["cufft_execs"] - launches0["cufft_execs"],
+                     "note": "counted by the library at its launch sites during the %d timed steps" % args.steps},
+        "paths": {"fast_stencil": info["fast_stencil"], "band_limited_fft": info["band_limited_fft"],
+                  "band_kmax": info["band_kmax"]},
         "clocks": clk,
         "roofline": roofline,
         "stages": stages,

@@ -90,6 +90,9 @@ typedef struct {
   int band_limited_fft;  /* 1: z transforms + fused (x,y) transform / scale kernel (fp32, Mx and My      */
                          /*    powers of two <= 256, kernel_path = 0, virial off); 0: dense 3-D cuFFT    */
   int band_kmax[3];      /* band-limited path: kept DFT indices |m_d| <= band_kmax[d]                    */
+  long long own_kernel_launches; /* kernels of this library launched by the plan since creation (counted  */
+  long long memsets;             /* at the launch sites), cudaMemsetAsync calls, and cuFFT executions      */
+  long long cufft_execs;         /* (each a few cuFFT kernels; 0 on the band-limited path with pow-2 Mz)    */
 } pswf_lr_info;
 
 /* Create a plan.  box[3]: edge lengths; grid[3]: M_x,M_y,M_z (each >= w, product < 2^31);

@@ -90,7 +90,8 @@ def multiplier(p, box, grid, w, c, r_c, c_w, zero_mode=True):
     inside = (kn * r_c < c) & ~nyq
     inside[0, 0, 0] = False
     Ph = np.zeros(tuple(grid))
-    Ph[inside] = moll.Phi_hat(p, kn[inside])
+    kn_u, inv = np.unique(kn[inside], return_inverse=True)    # Phi^ depends on |k| only
+    Ph[inside] = moll.Phi_hat(p, kn_u)[inv]
     with np.errstate(invalid="ignore"):
         D = np.where(inside, Ph / What ** 2, 0.0)
     if np.isnan(D).any():
@@ -188,3 +189,83 @@ def default_r_c(box, grid, c, eta=0.5):
 def default_c_w(w, eta=0.5):
     """Reading R3: window bandwidth c_w = w (3.55 - 1.55 eta)."""
     return float(w * (3.55 - 1.55 * eta))
+
+
+# ---------------------------------------------------------------------------------
+# The same evaluation with the two atom loops in plain C (oracle/gridded_sum.c), for the large
+# configurations; stencil, window values, multiplier and FFTs are the numpy code above.
+# ---------------------------------------------------------------------------------
+_LIBG = None
+
+
+def build_c(force=False):
+    """Compile oracle/gridded_sum.c -> oracle/liboracle_gridded.so (gcc -O2 -fopenmp)."""
+    import os
+    import subprocess
+    here = os.path.dirname(os.path.abspath(__file__))
+    src, out = os.path.join(here, "gridded_sum.c"), os.path.join(here, "liboracle_gridded.so")
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-std=c11", "-o", out, src])
+    return out
+
+
+def _libg():
+    global _LIBG
+    if _LIBG is None:
+        import ctypes
+        _LIBG = ctypes.CDLL(build_c())
+        _LIBG.oracle_gridded_threads.restype = ctypes.c_int
+    return _LIBG
+
+
+def c_threads():
+    return int(_libg().oracle_gridded_threads())
+
+
+def gridded_c(pos, q, exponents, box, grid, w, c, r_c, c_w, zero_mode=True, timings=None, multipliers=None):
+    """gridded() with spread() and gather() replaced by their plain-C transcriptions.  Same returns
+    (E, E_channels, phi, F).  `timings`, if a dict, receives the seconds spent per step.  `multipliers`
+    may carry {p: D_p} from an earlier call with the same cell and parameters (they depend on neither
+    positions nor charges: the plan-time part of the method) and is filled in otherwise."""
+    import ctypes
+    import time
+    t0 = time.perf_counter()
+    q = np.ascontiguousarray(np.atleast_2d(np.asarray(q, dtype=np.float64)))
+    C, N = q.shape
+    grid_a = np.ascontiguousarray(grid, dtype=np.int64)
+    Hi = inverse_cell(box)
+    psi_w = PSWF0(c_w)
+    i0, z = stencil(pos, box, grid_a, w)
+    i0 = np.ascontiguousarray(i0, dtype=np.int64)
+    Wd = np.ascontiguousarray(psi_w(z))                                   # (N,3,w)
+    dWd = np.ascontiguousarray(-psi_w.deriv(z, 1) * (2.0 * grid_a[None, :, None] / w))
+    t1 = time.perf_counter()
+    P = lambda a, t=ctypes.POINTER(ctypes.c_double): a.ctypes.data_as(t)
+    PI = ctypes.POINTER(ctypes.c_int64)
+    rho = np.zeros((C,) + tuple(int(g) for g in grid_a))
+    _libg().oracle_spread(ctypes.c_long(N), ctypes.c_int(C), ctypes.c_int(w), P(grid_a, PI), P(i0, PI), P(Wd), P(q),
+                          P(rho))                                           # (i)
+    t2 = time.perf_counter()
+    rho_hat = np.fft.fftn(rho, axes=(1, 2, 3))                             # (ii)
+    phig = np.empty_like(rho)
+    Dcache = multipliers if multipliers is not None else {}
+    t_mult = 0.0
+    for a, p in enumerate(exponents):
+        if int(p) not in Dcache:
+            tm0 = time.perf_counter()
+            Dcache[int(p)] = multiplier(int(p), box, grid_a, w, c, r_c, c_w, zero_mode)
+            t_mult += time.perf_counter() - tm0
+        phig[a] = np.fft.ifftn(Dcache[int(p)] * rho_hat[a]).real * np.prod(grid_a)   # (iii) + inverse
+    t3 = time.perf_counter()
+    phi = np.empty((C, N))
+    grad = np.empty((C, N, 3))
+    _libg().oracle_gather(ctypes.c_long(N), ctypes.c_int(C), ctypes.c_int(w), P(grid_a, PI), P(i0, PI), P(Wd), P(dWd),
+                          P(np.ascontiguousarray(phig)), P(phi), P(grad))
+    grad = np.einsum("ed,and->ane", Hi, grad)
+    F = -np.einsum("an,and->nd", q, grad)
+    E_ch = 0.5 * np.einsum("an,an->a", q, phi)
+    t4 = time.perf_counter()
+    if timings is not None:
+        timings.update(window=t1 - t0, spread=t2 - t1, fft_scale=t3 - t2 - t_mult, multipliers=t_mult,
+                       gather=t4 - t3, total=t4 - t0)
+    return float(E_ch.sum()), E_ch, phi, F

@@ -40,7 +40,9 @@ class Info(ctypes.Structure):
                 ("window_degree", ctypes.c_int), ("kernel_degree", ctypes.c_int),
                 ("kernel_panels", ctypes.c_int), ("modes_in_ball", ctypes.c_longlong),
                 ("workspace_bytes", ctypes.c_longlong), ("fast_stencil", ctypes.c_int),
-                ("band_limited_fft", ctypes.c_int), ("band_kmax", ctypes.c_int * 3)]
+                ("band_limited_fft", ctypes.c_int), ("band_kmax", ctypes.c_int * 3),
+                ("own_kernel_launches", ctypes.c_longlong), ("memsets", ctypes.c_longlong),
+                ("cufft_execs", ctypes.c_longlong)]
 
 
 EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_plan_create_cell", "pswf_lr_execute", "pswf_lr_execute_host",

@@ -658,6 +658,7 @@ void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t 
   X.Mzh = p->M[2] / 2 + 1;
   const size_t sm = xy_smem_bytes(X.Mx, X.My);
   const dim3 grid((unsigned)(p->fused_kmax[2] + 1), (unsigned)p->C);
+  p->n_kernels += 1;
   float2* dump = nullptr;
   if (p->debug_dump_spectrum) {
     const size_t Mhalf = (size_t)p->M[0] * p->M[1] * X.Mzh;
@@ -703,6 +704,7 @@ int z_tile(int My) {
 void launch_z_forward(pswf_lr_plan* p, cudaStream_t st) {
   const int C = p->C, Mx = p->M[0], My = p->M[1], YT = z_tile(My);
   const unsigned nb = (unsigned)(C * Mx * (My / YT));
+  p->n_kernels += 1;
 #define PSWF_ZF(NZ) \
   case NZ: k_z_forward<NZ><<<nb, kZThreads, 0, st>>>(C, Mx, My, YT, p->fused_kmax[2], (const float*)p->d_grid, (float2*)p->d_spec); break;
   switch (p->M[2]) { PSWF_ZF(8) PSWF_ZF(16) PSWF_ZF(32) PSWF_ZF(64) PSWF_ZF(128) PSWF_ZF(256) default: break; }
@@ -720,6 +722,7 @@ void launch_z_inverse_interleaved(pswf_lr_plan* p, cudaStream_t st) {
   for (int cb0 = 0; cb0 < C; cb0 += 4) {
     const int left = C - cb0;
     const int cbv = left >= 3 ? 4 : left, nch = std::min(left, 4);
+    p->n_kernels += 1;
 #define PSWF_ZIL(NZ, CBV)                                                                                         \
   k_z_inverse_il<NZ, CBV><<<nb, kZThreads, 0, st>>>(C, cb0, nch, Mx, My, YT, p->fused_kmax[2], (const float2*)p->d_spec2, \
                                                     (typename ZVec<CBV>::type*)gi)
@@ -739,6 +742,7 @@ void launch_z_inverse_interleaved(pswf_lr_plan* p, cudaStream_t st) {
 void launch_z_inverse(pswf_lr_plan* p, cudaStream_t st) {
   const int C = p->C, Mx = p->M[0], My = p->M[1], YT = z_tile(My);
   const unsigned nb = (unsigned)(C * Mx * (My / YT));
+  p->n_kernels += 1;
 #define PSWF_ZI(NZ) \
   case NZ: k_z_inverse<NZ><<<nb, kZThreads, 0, st>>>(C, Mx, My, YT, p->fused_kmax[2], (const float2*)p->d_spec2, (float*)p->d_grid); break;
   switch (p->M[2]) { PSWF_ZI(8) PSWF_ZI(16) PSWF_ZI(32) PSWF_ZI(64) PSWF_ZI(128) PSWF_ZI(256) default: break; }

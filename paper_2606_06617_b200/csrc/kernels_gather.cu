@@ -472,6 +472,7 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, bool hav
 #define PSWF_GATHER(CBV, NCH)                                                                               \
   do {                                                                                                      \
     using V = typename VecOf<CBV>::type;                                                                    \
+    p->n_kernels += have_il ? 1 : 2;                                                                        \
     if (!have_il) k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);            \
     auto kern = k_gather_rows<CBV, GBX, GBY, NCTA>;                                                         \
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \

@@ -362,6 +362,8 @@ void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const Gri
                      cudaStream_t st) {
   const int Mtot = p->M[0] * p->M[1] * p->M[2];
   cudaMemsetAsync(p->d_count, 0, sizeof(int) * ((size_t)Mtot + 1), st);
+  p->n_memsets += 2;
+  p->n_kernels += (n > 0 ? 1 : 0) + 1 + ((n > 0 && scatter) ? 1 : 0);
   if (n > 0)
     k_bin_count<T><<<(n + 255) / 256, 256, 0, st>>>(n, pos, g, p->d_count, p->d_key, p->d_rank);
   cudaMemsetAsync(p->d_scan_state, 0, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), st);
@@ -376,6 +378,8 @@ template <class T>
 void launch_spread_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, cudaStream_t st) {
   const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
   cudaMemsetAsync(p->d_grid, 0, sizeof(T) * Mtot * p->C, st);
+  p->n_memsets += 1;
+  p->n_kernels += n > 0 ? 1 : 0;
   if (n > 0)
     k_spread_ref<T><<<(n + 7) / 8, 256, 0, st>>>(n, p->C, p->cap_atoms, g, p->d_si0, (const T*)p->d_sdelta,
                                                   (const T*)p->d_sq, (T*)p->d_grid);
@@ -386,6 +390,7 @@ void launch_scale(pswf_lr_plan* p, const ScaleParams<T>& P, bool want_E, cudaStr
   const size_t Mhalf = (size_t)P.M[0] * P.M[1] * P.Mzh;
   const int threads = 256;
   const unsigned nb = (unsigned)((Mhalf + threads - 1) / threads);
+  p->n_kernels += 1;
   if (p->virial)
     k_scale<T, true><<<nb, threads, 0, st>>>(P, (Cplx<T>*)p->d_spec, p->d_Ech, want_E ? 1 : 0, p->d_virial);
   else
@@ -393,11 +398,13 @@ void launch_scale(pswf_lr_plan* p, const ScaleParams<T>& P, bool want_E, cudaStr
 }
 
 void launch_finalize_energy(pswf_lr_plan* p, double* E, cudaStream_t st) {
+  p->n_kernels += 1;
   k_finalize_energy<<<1, 32, 0, st>>>(p->C, p->d_Ech, E);
 }
 
 template <class T>
 void launch_gather_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, T* phi, T* F, cudaStream_t st) {
+  p->n_kernels += n > 0 ? 1 : 0;
   if (n > 0)
     k_gather_ref<T><<<(n + 7) / 8, 256, 0, st>>>(n, p->C, p->cap_atoms, g, p->d_si0, (const T*)p->d_sdelta,
                                                   (const T*)p->d_sq, p->d_perm, (const T*)p->d_grid, phi, F);

@@ -229,6 +229,8 @@ template <class T>
 void launch_real_space(pswf_lr_plan* p, int n, const T* pos, const RealGeom<T>& g, const RealParams<T>& P, double* E,
                        T* phi, T* F, int accumulate, cudaStream_t st) {
   cudaMemsetAsync(p->d_Ereal, 0, sizeof(double), st);
+  p->n_memsets += 1;
+  p->n_kernels += (n > 0 ? 2 : 0) + (E ? 1 : 0);
   // virial: added to the plan's accumulator when accumulate is set (after pswf_lr_execute), else restarted
   double* wacc = p->virial ? p->d_virial : nullptr;
   if (wacc && !accumulate) cudaMemsetAsync(wacc, 0, sizeof(double) * 6, st);

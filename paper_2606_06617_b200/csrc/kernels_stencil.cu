@@ -620,6 +620,7 @@ struct SpreadLaunch {
     const size_t sm = smem_bytes(cap, recf);
     auto kern = k_spread_os<WY, WZ, CB, NCTA>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    p->n_kernels += 1;
     kern<<<(unsigned)(npy * npz * nseg), S::NT + 32, sm, st>>>(Mx, My, Mz, nseg, npy, npz, cap, recf, cb0, p->d_count,
                                                          (const float*)p->d_rec, (float*)p->d_grid);
   }
@@ -638,6 +639,7 @@ struct SpreadLaunch {
     nseg = std::max(1, std::min(nseg, p->M[0] / SW));
     const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
     cudaMemsetAsync(p->d_grid, 0, sizeof(float) * Mtot * p->C, st);   // the RED-merged planes start from zero
+    p->n_memsets += 1;
     int cb0 = 0;
     while (cb0 < p->C) {
       const int left = p->C - cb0;
@@ -674,6 +676,7 @@ void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const floa
                             cudaStream_t st) {
   if (n <= 0) return;
   const int recf = stencil_rec_floats(p->C);
+  p->n_kernels += 2;
   k_perm<<<(n + 255) / 256, 256, 0, st>>>(n, p->d_count, p->d_key, p->d_rank, p->d_perm);
   const size_t sm = sizeof(float) * kRecThreads * (size_t)recf;
   const unsigned nb = (unsigned)((n + kRecThreads - 1) / kRecThreads);

@@ -147,6 +147,8 @@ struct pswf_lr_plan {
   cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
   long long n_submitted = 0, n_waited = 0;
   int last_n_atoms = 0;
+  // launch accounting (pswf_lr_info): this library's own kernels, memsets, cuFFT executions since creation
+  long long n_kernels = 0, n_memsets = 0, n_cufft = 0;
   // cuFFT
   cufftHandle fft_fwd = 0, fft_inv = 0;
   bool have_fft = false;

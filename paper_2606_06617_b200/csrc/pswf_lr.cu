@@ -224,9 +224,11 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
       launch_z_forward(p, st);
     } else {
       CUFFT_TRY(cufftSetStream(p->fft_zf, st));
+      p->n_cufft++;
       CUFFT_TRY(cufftExecR2C(p->fft_zf, (cufftReal*)p->d_grid, (cufftComplex*)p->d_spec));
     }
   } else {
+    p->n_cufft++;
     CUFFT_TRY(cufftSetStream(p->fft_fwd, st));
     if (sizeof(T) == 4)
       CUFFT_TRY(cufftExecR2C(p->fft_fwd, (cufftReal*)p->d_grid, (cufftComplex*)p->d_spec));
@@ -237,6 +239,7 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   // a3
   cudaMemsetAsync(p->d_Ech, 0, sizeof(double) * p->C, st);
   if (p->virial) cudaMemsetAsync(p->d_virial, 0, sizeof(double) * 6, st);
+  p->n_memsets += p->virial ? 2 : 1;
   if constexpr (kIsF32) {
     if (fused) launch_xy_scale(p, P, st);
   }
@@ -254,10 +257,12 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
       if (p->fused_z && (!il || p->debug_dump_spectrum)) {
         launch_z_inverse(p, st);
       } else if (!p->fused_z) {
+        p->n_cufft++;
         CUFFT_TRY(cufftSetStream(p->fft_zi, st));
         CUFFT_TRY(cufftExecC2R(p->fft_zi, (cufftComplex*)p->d_spec2, (cufftReal*)p->d_grid));
       }
     } else {
+      p->n_cufft++;
       CUFFT_TRY(cufftSetStream(p->fft_inv, st));
       if (sizeof(T) == 4)
         CUFFT_TRY(cufftExecC2R(p->fft_inv, (cufftComplex*)p->d_spec, (cufftReal*)p->d_grid));
@@ -817,6 +822,9 @@ int pswf_lr_get_info(const pswf_lr_plan* p, pswf_lr_info* info) {
   info->fast_stencil = (!p->host_only && p->kernel_path == 0 && stencil_path_supported(p)) ? 1 : 0;
   info->band_limited_fft = (p->fused_fft && !p->virial) ? 1 : 0;
   for (int d = 0; d < 3; ++d) info->band_kmax[d] = p->fused_kmax[d];
+  info->own_kernel_launches = p->n_kernels;
+  info->memsets = p->n_memsets;
+  info->cufft_execs = p->n_cufft;
   return 0;
 }
 
