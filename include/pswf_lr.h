@@ -138,7 +138,7 @@ int pswf_lr_execute_host(pswf_lr_plan* plan, int n_atoms, const void* pos, const
 /* Pipelined form of pswf_lr_execute_host for streams of independent evaluations (batches of frames,
  * ensemble members, or an MD loop whose next positions do not wait for these forces): submit enqueues
  * the host->device copies, the evaluation and the device->host copies on three streams owned by the
- * plan and returns at once; at most TWO submissions may be in flight (two staging slots), a third
+ * plan and returns at once; at most THREE submissions may be in flight (three staging slots), a fourth
  * returns PSWF_LR_ERR_BUSY.  pswf_lr_wait_host blocks until the OLDEST outstanding submission has
  * delivered E, phi and F to its host buffers.  With pinned host buffers the copy-in of submission
  * k+1, the evaluation of k and the copy-out of k-1 overlap (PCIe is full duplex), so the sustained

@@ -136,15 +136,16 @@ struct pswf_lr_plan {
   void* d_sq = nullptr;           // real [C][cap]
   void* d_rec = nullptr;          // fast path: per-atom weight records
   void* d_drec = nullptr;         // fast path: per-atom derivative-weight records (gather)
-  // host-buffer entry points: two staging slots (slot 0 serves pswf_lr_execute_host; submit / wait
-  // alternate between both so that copy-in, evaluation and copy-out of consecutive submissions overlap)
-  void* d_pos_in[2] = {nullptr, nullptr};
-  void* d_q_in[2] = {nullptr, nullptr};
-  void* d_phi_out[2] = {nullptr, nullptr};
-  void* d_F_out[2] = {nullptr, nullptr};
-  double* d_E_out[2] = {nullptr, nullptr};
+  // host-buffer entry points: three staging slots (slot 0 serves pswf_lr_execute_host; submit / wait
+  // cycle through them so that copy-in, evaluation and copy-out of consecutive submissions overlap)
+  static constexpr int kHostSlots = 3;
+  void* d_pos_in[kHostSlots] = {};
+  void* d_q_in[kHostSlots] = {};
+  void* d_phi_out[kHostSlots] = {};
+  void* d_F_out[kHostSlots] = {};
+  double* d_E_out[kHostSlots] = {};
   cudaStream_t s_in = nullptr, s_comp = nullptr, s_out = nullptr;
-  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+  cudaEvent_t ev_in[kHostSlots] = {}, ev_comp[kHostSlots] = {}, ev_out[kHostSlots] = {};
   long long n_submitted = 0, n_waited = 0;
   int last_n_atoms = 0;
   // launch accounting (pswf_lr_info): this library's own kernels, memsets, cuFFT executions since creation

@@ -65,7 +65,8 @@ int dev_alloc(void** ptr, size_t bytes, long long* total) {
 void free_atoms(pswf_lr_plan* p) {
   void** ptrs[] = {&p->d_spos, (void**)&p->d_key, (void**)&p->d_rank, (void**)&p->d_perm, (void**)&p->d_si0, &p->d_sdelta,
                    &p->d_sq,          &p->d_rec,          &p->d_drec,         &p->d_pos_in[0],    &p->d_q_in[0],     &p->d_phi_out[0],
-                   &p->d_F_out[0],    &p->d_pos_in[1],    &p->d_q_in[1],      &p->d_phi_out[1],   &p->d_F_out[1]};
+                   &p->d_F_out[0],    &p->d_pos_in[1],    &p->d_q_in[1],      &p->d_phi_out[1],   &p->d_F_out[1],
+                   &p->d_pos_in[2],   &p->d_q_in[2],      &p->d_phi_out[2],   &p->d_F_out[2]};
   for (void** q : ptrs) {
     if (*q) cudaFree(*q);
     *q = nullptr;
@@ -660,35 +661,37 @@ int pswf_lr_execute_host(pswf_lr_plan* p, int n, const void* pos, const void* q,
   return 0;
 }
 
-// Pipelined host-buffer evaluation.  Submission k uses staging slot k % 2:
-//   copy-in stream:   [wait: evaluation k-2 done with the slot]  H2D pos, q            -> ev_in
-//   compute stream:   [wait: ev_in, copy-out k-2 done with the slot]  the evaluation     -> ev_comp
+// Pipelined host-buffer evaluation.  Submission k uses staging slot k % 3:
+//   copy-in stream:   [wait: evaluation k-3 done with the slot]  H2D pos, q            -> ev_in
+//   compute stream:   [wait: ev_in, copy-out k-3 done with the slot]  the evaluation     -> ev_comp
 //   copy-out stream:  [wait: ev_comp]  D2H E, phi, F                                    -> ev_out
-// so with pinned host buffers H2D(k+1), evaluation(k) and D2H(k-1) run at the same time.
+// so with pinned host buffers H2D(k+1), evaluation(k) and D2H(k-1) run at the same time; the third slot lets
+// the copy-in run a whole step ahead (with two, an evaluation waited ~0.1 ms for its inputs at config 4).
 int pswf_lr_submit_host(pswf_lr_plan* p, int n, const void* pos, const void* q, double* E, void* phi, void* F) {
   if (!p || n < 0) return PSWF_LR_ERR_INVALID_ARG;
   if (n > 0 && (!pos || !q)) return PSWF_LR_ERR_INVALID_ARG;
   if (p->host_only) return PSWF_LR_ERR_CUDA;
-  if (p->n_submitted - p->n_waited >= 2) return PSWF_LR_ERR_BUSY;
+  constexpr int NS = pswf_lr_plan::kHostSlots;
+  if (p->n_submitted - p->n_waited >= NS) return PSWF_LR_ERR_BUSY;
   DeviceGuard guard(p);
   if (!guard.ok) return PSWF_LR_ERR_CUDA;
   if (n > p->cap_atoms && p->n_submitted != p->n_waited) return PSWF_LR_ERR_BUSY;   // growing reallocates
   int rc = ensure_capacity(p, n);
   if (rc) return rc;
-  rc = ensure_host_staging(p, 2);
+  rc = ensure_host_staging(p, NS);
   if (rc) return rc;
   if (!p->s_in) {
     CUDA_TRY(cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking));
     CUDA_TRY(cudaStreamCreateWithFlags(&p->s_comp, cudaStreamNonBlocking));
     CUDA_TRY(cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking));
-    for (int s = 0; s < 2; ++s) {
+    for (int s = 0; s < NS; ++s) {
       CUDA_TRY(cudaEventCreateWithFlags(&p->ev_in[s], cudaEventDisableTiming));
       CUDA_TRY(cudaEventCreateWithFlags(&p->ev_comp[s], cudaEventDisableTiming));
       CUDA_TRY(cudaEventCreateWithFlags(&p->ev_out[s], cudaEventDisableTiming));
     }
   }
-  const int s = (int)(p->n_submitted & 1);
-  const bool reuse = p->n_submitted >= 2;
+  const int s = (int)(p->n_submitted % NS);
+  const bool reuse = p->n_submitted >= NS;
   const size_t rs = real_size(p);
   if (reuse) CUDA_TRY(cudaStreamWaitEvent(p->s_in, p->ev_comp[s], 0));
   if (n > 0) {
@@ -716,7 +719,7 @@ int pswf_lr_wait_host(pswf_lr_plan* p) {
   if (!p) return PSWF_LR_ERR_INVALID_ARG;
   if (p->host_only) return PSWF_LR_ERR_CUDA;
   if (p->n_submitted == p->n_waited) return PSWF_LR_ERR_INVALID_ARG;   // nothing in flight
-  const int s = (int)(p->n_waited & 1);
+  const int s = (int)(p->n_waited % pswf_lr_plan::kHostSlots);
   CUDA_TRY(cudaEventSynchronize(p->ev_out[s]));
   p->n_waited++;
   return 0;
@@ -975,7 +978,7 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   DeviceGuard guard(p);
   cudaDeviceSynchronize();
   free_atoms(p);
-  for (int s = 0; s < 2; ++s) {
+  for (int s = 0; s < pswf_lr_plan::kHostSlots; ++s) {
     if (p->d_E_out[s]) cudaFree(p->d_E_out[s]);
     if (p->ev_in[s]) cudaEventDestroy(p->ev_in[s]);
     if (p->ev_comp[s]) cudaEventDestroy(p->ev_comp[s]);

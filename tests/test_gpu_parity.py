@@ -415,8 +415,8 @@ def test_execute_host_matches_execute():
 
 
 def test_pipelined_host_submissions_match_execute():
-    """pswf_lr_submit_host / pswf_lr_wait_host: five different systems through the two staging slots
-    give what the blocking call gives; a third submission in flight is refused, and so is a blocking
+    """pswf_lr_submit_host / pswf_lr_wait_host: five different systems through the three staging slots
+    give what the blocking call gives; a fourth submission in flight is refused, and so is a blocking
     call while submissions are in flight; workspace accounting survives a capacity growth."""
     wl = workloads.make(2)
     n, C = len(wl["pos"]), 2
@@ -439,16 +439,17 @@ def test_pipelined_host_submissions_match_execute():
         ref.append((E.item(), phi.double().numpy().copy(), F.double().numpy().copy()))
     w0 = plan.info()["workspace_bytes"]
     for k in range(5):
-        if k >= 2:
+        if k >= 3:
             plan.wait_host()
         plan.submit_host(n, systems[k][0], systems[k][1], *outs[k])
-        if k == 1:
+        if k == 2:
             with pytest.raises(binding.PswfLrError) as e3:
                 plan.submit_host(n, systems[k][0], systems[k][1], *outs[k])
             assert e3.value.code == -7
             with pytest.raises(binding.PswfLrError) as e4:
                 plan.execute_host(n, systems[k][0], systems[k][1], *outs[k], sp)
             assert e4.value.code == -7
+    plan.wait_host()
     plan.wait_host()
     plan.wait_host()
     with pytest.raises(binding.PswfLrError):
@@ -459,7 +460,7 @@ def test_pipelined_host_submissions_match_execute():
         assert rel(F.double().numpy(), ref[k][2]) < 1e-5 and rel(phi.double().numpy(), ref[k][1]) < 1e-5
     # second staging slot was added; nothing else may have changed
     w1 = plan.info()["workspace_bytes"]
-    assert 0 < w1 - w0 <= 2 * (n * (3 + C) * 4 * 2 + 64) + 4096
+    assert 0 < w1 - w0 <= 2 * 2 * (n * (3 + C) * 4 * 2 + 64) + 4096     # two more staging slots
     plan.destroy()
 
 
