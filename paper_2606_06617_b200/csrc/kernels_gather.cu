@@ -16,12 +16,11 @@
 //    z == k (mod 8).  The weight records hold wz and dwz/dz ROTATED by the atom's cell index mod 8,
 //    so the z contraction is sum_k wzr[k] * win[k] with static register indices: one copy of the
 //    atom code, no unrolled window rotation;
-//  * the potential grid is first copied from cuFFT's planar layout [C][x][y][z] into a transposed,
-//    channel-interleaved one [z][x][y][CB] (k_interleave_t, L2-resident), so that a z-plane is
-//    contiguous and one 16-byte load per footprint point refreshes the slot that left the window
-//    for all channels.  The plane of the NEXT step is loaded one step ahead into scratch registers
-//    and the one after that is touched in L1, so that empty cells do not expose load latency;
-//    neighbouring rows of the CTA share 7/8 of their footprint in L1;
+//  * the potential grid is read in a transposed, channel-interleaved layout [z][x][y][CB], so that a
+//    z-plane is contiguous and one 16-byte load per footprint point refreshes the slot that left the
+//    window for all channels.  The band-limited transform path writes that layout directly
+//    (k_z_inverse_il, kernels_fft.cu); after the dense path k_interleave_t copies it from cuFFT's planar
+//    [C][x][y][z] (L2-resident).  Neighbouring rows of the CTA share 7/8 of their footprint in L1;
 //  * the lanes of a segment fetch the cell boundaries of its 32 cells at once, skip leading /
 //    trailing empty cells and return at once when the segment holds no atoms (vacuum of
 //    configuration 5);
@@ -114,10 +113,6 @@ __device__ __forceinline__ float reduce8(float (&v)[8], int lane) {
   v[0] += __shfl_xor_sync(0xffffffffu, v[0], 2);
   v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
   return v[0];
-}
-
-__device__ __forceinline__ void prefetch_l1(const void* p) {
-  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
 }
 
 // Packed FP32 pairs (sm_100a FFMA2: one instruction, two IEEE fused multiply-adds per lane; ptxas

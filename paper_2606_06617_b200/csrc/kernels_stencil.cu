@@ -16,8 +16,11 @@
 //  * the record holds the three weight vectors ROTATED by the atom's cell index mod 8, so a thread
 //    reads wy at offset (y & 7), wz at (z0 & 7) and multiplies slot k by wxr[k]: no per-atom index
 //    arithmetic, no register rotation, no unrolled plane loop;
-//  * when a plane leaves the window its slot is stored once with plain coalesced stores: no
-//    zero-fill of the grid, no atomics, deterministic summation order.
+//  * the x range is cut into segments that form one wave of CTAs; when a plane leaves the window its slot
+//    is stored once with plain coalesced stores, except the 7 planes a segment shares with each
+//    neighbour, which are merged with red.global.add.v2.f32 into the grid (zero-filled by a memset before
+//    the launch).  No shared-memory atomics.  In-cell atom order comes from atomicAdd ranks and the seam
+//    planes from RED, so results are NOT bitwise reproducible from run to run (differences ~1e-7).
 //
 // Requirements of this path (host-checked): fp32, even w <= 8 (narrower windows are zero padded to 8
 // slots), M_d a multiple of 8 and >= 16.
@@ -696,10 +699,9 @@ void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const floa
 
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {
   (void)n;
-  // 16 x 32 column patches (8 warps), two CTAs per SM: measured 396 us against 407 us for 16 x 16
-  // patches x 3 CTAs and 444 us for 16 x 16 x 4 CTAs at configuration 4
-  // 16 x 16 column patches: 4 consumer warps + 1 producer warp, three CTAs per SM (136 registers).
-  // Measured at configuration 4: 364 us; 16 x 32 patches x 2 CTAs (113 registers) 418 us.
+  // 16 x 16 column patches: 4 consumer warps + 1 producer warp, three CTAs per SM (<= 128 registers).
+  // Measured at configuration 4 (round 2): 300 us.  Rejected: 16 x 32 patches x 2 CTAs (113-register cap:
+  // spills), 16 x 16 x 4 CTAs, 136 registers x 2 CTAs.
   SpreadLaunch<2, 2, 3>::all_channels(p, st);
 }
 
