@@ -719,9 +719,10 @@ void launch_z_inverse_interleaved(pswf_lr_plan* p, cudaStream_t st) {
   const unsigned nb = (unsigned)(Mx * (My / YT));
   const size_t Mtot = (size_t)Mx * My * p->M[2];
   float* gi = (float*)p->d_gridi;
-  for (int cb0 = 0; cb0 < C; cb0 += 4) {
-    const int left = C - cb0;
-    const int cbv = left >= 3 ? 4 : left, nch = std::min(left, 4);
+  const int G = p->gather_group;
+  for (int cb0 = 0; cb0 < C; cb0 += G) {
+    const int left = std::min(G, C - cb0);
+    const int cbv = left >= 3 ? 4 : left, nch = left;
     p->n_kernels += 1;
 #define PSWF_ZIL(NZ, CBV)                                                                                         \
   k_z_inverse_il<NZ, CBV><<<nb, kZThreads, 0, st>>>(C, cb0, nch, Mx, My, YT, p->fused_kmax[2], (const float2*)p->d_spec2, \

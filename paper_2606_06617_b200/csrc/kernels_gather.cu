@@ -27,6 +27,7 @@
 //  * per atom: z contraction with value and derivative weights in one pass (2 x 8 x 2 FFMA per
 //    channel per lane), combination with the (x,y) weights, 9-shuffle transpose-reduce of
 //    (phi_a, F_x, F_y, F_z), scattered store to the caller's atom order.
+#include <algorithm>
 #include <type_traits>
 
 #include "kernels_common.cuh"
@@ -363,37 +364,47 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
         retire();   // the previous atom's reduction: independent of everything below, interleaved by ptxas
         float fx = 0.f, fy = 0.f, fz = 0.f;
         if constexpr (CB % 2 == 0) {
-          // channel pairs (c, c+1): {S_c, S_c+1} += w * {win_c, win_c+1}, one FFMA2 each
-          f32x2 fx2 = 0ull, fy2 = 0ull, fz2 = 0ull;
+          // channel pairs (c, c+1): {S_c, S_c+1} += w * {win_c, win_c+1}, one FFMA2 each.  The force needs
+          // only sum_c q_c S_c: the charge-weighted sums T are formed BEFORE the (x,y) weights are applied
+          // (4 FFMA2 per pair + 6 scalar FMAs instead of 9 FFMA2 per pair + unpacking)
+          f32x2 T00 = 0ull, T01 = 0ull, T10 = 0ull, T11 = 0ull;
+          // all channel pairs in one pass over the 8 planes: 4 (CB = 2) or 8 (CB = 4) independent FFMA2 chains
+          // in round-robin order, so that a chain's next link issues 8 or 16 cycles after the previous one
+          constexpr int NP = CB / 2;
+          f32x2 S00[NP], S10[NP], S01[NP], S11[NP];
 #pragma unroll
-          for (int c = 0; c < CB; c += 2) {
-            // four chains {S0, S1} x {point 0, point 1} in round-robin order (the volatile asm keeps
-            // it): 16 accumulator registers would not fit beside the 64-register window
-            f32x2 S00 = 0ull, S10 = 0ull, S01 = 0ull, S11 = 0ull;
+          for (int h = 0; h < NP; ++h) { S00[h] = 0ull; S10[h] = 0ull; S01[h] = 0ull; S11[h] = 0ull; }
 #pragma unroll
-            for (int k = 0; k < SW; ++k) {
-              const f32x2 ga = win[k][0][c / 2], gb = win[k][1][c / 2];
-              const f32x2 wk = pack2(wz[k], wz[k]), dk = pack2(dz[k], dz[k]);
-              S00 = ffma2v(ga, wk, S00);
-              S10 = ffma2v(ga, dk, S10);
-              S01 = ffma2v(gb, wk, S01);
-              S11 = ffma2v(gb, dk, S11);
+          for (int k = 0; k < SW; ++k) {
+            const f32x2 wk = pack2(wz[k], wz[k]), dk = pack2(dz[k], dz[k]);
+#pragma unroll
+            for (int h = 0; h < NP; ++h) {
+              const f32x2 ga = win[k][0][h], gb = win[k][1][h];
+              S00[h] = ffma2v(ga, wk, S00[h]);
+              S10[h] = ffma2v(ga, dk, S10[h]);
+              S01[h] = ffma2v(gb, wk, S01[h]);
+              S11[h] = ffma2v(gb, dk, S11[h]);
             }
-            const f32x2 xy0 = pack2(xy[0], xy[0]), xy1 = pack2(xy[1], xy[1]);
-            f32x2 val = ffma2(S01, xy1, ffma2(S00, xy0, 0ull));
-            f32x2 gz = ffma2(S11, xy1, ffma2(S10, xy0, 0ull));
-            f32x2 gx = ffma2(S01, pack2(dxy[1], dxy[1]), ffma2(S00, pack2(dxy[0], dxy[0]), 0ull));
-            f32x2 gy = ffma2(S01, pack2(xdy[1], xdy[1]), ffma2(S00, pack2(xdy[0], xdy[0]), 0ull));
-            const f32x2 q2 = pack2(qv[c], qv[c + 1]);
-            fx2 = ffma2(q2, gx, fx2);
-            fy2 = ffma2(q2, gy, fy2);
-            fz2 = ffma2(q2, gz, fz2);
-            unpack2(val, pend[c], pend[c + 1]);
+          }
+          const f32x2 xy0 = pack2(xy[0], xy[0]), xy1 = pack2(xy[1], xy[1]);
+#pragma unroll
+          for (int h = 0; h < NP; ++h) {
+            const f32x2 val = ffma2(S01[h], xy1, ffma2(S00[h], xy0, 0ull));
+            const f32x2 q2 = pack2(qv[2 * h], qv[2 * h + 1]);
+            T00 = ffma2(q2, S00[h], T00);
+            T01 = ffma2(q2, S01[h], T01);
+            T10 = ffma2(q2, S10[h], T10);
+            T11 = ffma2(q2, S11[h], T11);
+            unpack2(val, pend[2 * h], pend[2 * h + 1]);
           }
           float a, b;
-          unpack2(fx2, a, b); fx = -(a + b);
-          unpack2(fy2, a, b); fy = -(a + b);
-          unpack2(fz2, a, b); fz = -(a + b);
+          unpack2(T00, a, b); const float t00 = a + b;
+          unpack2(T01, a, b); const float t01 = a + b;
+          unpack2(T10, a, b); const float t10 = a + b;
+          unpack2(T11, a, b); const float t11 = a + b;
+          fx = -fmaf(dxy[1], t01, dxy[0] * t00);
+          fy = -fmaf(xdy[1], t01, xdy[0] * t00);
+          fz = -fmaf(xy[1], t11, xy[0] * t10);
         } else {
 #pragma unroll
         for (int c = 0; c < CB; ++c) {
@@ -439,8 +450,9 @@ size_t gather_grid_bytes(const pswf_lr_plan* p) {
   // interleaved copy of the potential grid: channel groups of 4 (last group 1, 2 or 4 wide)
   const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
   size_t fl = 0;
-  for (int cb0 = 0; cb0 < p->C; cb0 += 4) {
-    const int left = p->C - cb0;
+  const int G = p->gather_group;
+  for (int cb0 = 0; cb0 < p->C; cb0 += G) {
+    const int left = std::min(G, p->C - cb0);
     fl += Mtot * (left >= 3 ? 4 : left);
   }
   return fl * sizeof(float);
@@ -460,26 +472,27 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, bool hav
   HinvF Hi;
   for (int i = 0; i < 9; ++i) Hi.m[i] = (float)p->hinv[i];
   int pass = 0;
-  for (int cb0 = 0; cb0 < p->C; cb0 += 4, ++pass) {
-    const int left = p->C - cb0;
+  const int G = p->gather_group;
+  for (int cb0 = 0; cb0 < p->C; cb0 += G, ++pass) {
+    const int left = std::min(G, p->C - cb0);
     const int acc = pass > 0 ? 1 : 0;
     const float* planar = (const float*)p->d_grid + (size_t)cb0 * Mtot;
-#define PSWF_GATHER(CBV, NCH)                                                                               \
+#define PSWF_GATHER(CBV, NCH, NCTAV)                                                                        \
   do {                                                                                                      \
     using V = typename VecOf<CBV>::type;                                                                    \
     p->n_kernels += have_il ? 1 : 2;                                                                        \
     if (!have_il) k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);            \
-    auto kern = k_gather_rows<CBV, GBX, GBY, NCTA>;                                                         \
+    auto kern = k_gather_rows<CBV, GBX, GBY, NCTAV>;                                                         \
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \
     kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nbx, nby, recf, p->d_count,        \
                                                (const float*)p->d_rec, (const float*)p->d_drec, p->d_perm,  \
                                                (const V*)gi, phi, F, acc, Hi);                              \
     gi += Mtot * CBV;                                                                                       \
   } while (0)
-    if (left >= 4) PSWF_GATHER(4, 4);
-    else if (left == 3) PSWF_GATHER(4, 3);
-    else if (left == 2) PSWF_GATHER(2, 2);
-    else PSWF_GATHER(1, 1);
+    if (left >= 4) PSWF_GATHER(4, 4, NCTA);
+    else if (left == 3) PSWF_GATHER(4, 3, NCTA);
+    else if (left == 2) PSWF_GATHER(2, 2, 6);
+    else PSWF_GATHER(1, 1, 6);
 #undef PSWF_GATHER
   }
 }

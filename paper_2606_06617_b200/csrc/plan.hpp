@@ -159,6 +159,7 @@ struct pswf_lr_plan {
   int fused_kmax[3] = {0, 0, 0};  // kept signed DFT indices per dimension: |f| <= kmax (never Nyquist)
   cufftHandle fft_zf = 0, fft_zi = 0;
   void* d_spec2 = nullptr;        // cplx [Mz/2+1][C][Mx][My]; planes beyond the band stay zero
+  int gather_group = 4;           // channels per gather pass / interleaved grid group (4, or 2: narrower register window)
   bool debug_dump_spectrum = false;
   void* d_spec_dump = nullptr;    // cplx [C][Mx][My][Mz/2+1] dense copy of the scaled modes (test hook)
   // profiling

@@ -2,6 +2,7 @@
 // execute (bin/sort -> spread -> FFT -> scale+reduce -> inverse FFT -> gather), destroy.
 // See include/pswf_lr.h for the contract and the PAPER.md passages behind each step.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <type_traits>
