@@ -280,20 +280,8 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   };
 
   // walk the non-empty cells of the segment; the window advances to each of them in one go
-  unsigned rem = mask;        // non-empty cells not yet visited
-  bool first_cell = true;
-  while (rem != 0u) {
-    const int cur = __ffs(rem) - 1;   // current cell, relative to Z0
-    rem &= rem - 1u;
-    // advance the window from cell curA to cell an: the planes max(curA+8, an) .. an+7 replace the ones
-    // that left it (all 8 at the start of a row or after a gap).  Slot k takes the plane
-    // p_k = an + ((k - an) & 7) if that plane is new.  ptxas guards all refill loads with ONE
-    // scoreboard, so any form that branches between the planes of an advance fetches them one L2
-    // round trip after the other (decoded wait masks, 25% of the stall samples in profiles/r1e):
-    // one or two planes go through a switch over the first slot with the second plane predicated,
-    // longer advances are eight predicated loads in one straight-line block.
-    {
-      const int an = Z0 + cur, first_new = max(curA + SW, an);
+  auto advance_to = [&](const int an) {
+      const int first_new = max(curA + SW, an);
       const int cnt = an + SW - first_new;      // 1 .. 8 new planes
       if (cnt <= 2) {
         const int z = first_new >= Mz ? first_new - Mz : first_new;
@@ -327,16 +315,10 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
         }
       }
       curA = an;
-    }
-    if (first_cell) {   // this segment's records were staged before the window loads were issued
-      cp_async_wait_all();
-      __syncwarp();
-      first_cell = false;
-    }
-    {
-      const int jlo = __shfl_sync(0xffffffffu, jlo_l, cur);
-      const int jhi = __shfl_sync(0xffffffffu, jhi_l, cur);
-      for (int j = jlo; j < jhi; ++j) {
+  };
+  // one atom: S = slot of the NEWEST plane of the window; the z contraction visits it last
+  auto atom = [&](const int j, auto Sc) {
+      constexpr int S = decltype(Sc)::value;
         if (j - js >= kStage) {   // staging buffer exhausted (dense rows): write results, stage the next atoms
           retire();
           pend_row = kStage;
@@ -375,7 +357,9 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
 #pragma unroll
           for (int h = 0; h < NP; ++h) { S00[h] = 0ull; S10[h] = 0ull; S01[h] = 0ull; S11[h] = 0ull; }
 #pragma unroll
-          for (int k = 0; k < SW; ++k) {
+          for (int kk = 0; kk < SW; ++kk) {
+            constexpr int k0 = (S + 1) & 7;
+            const int k = (k0 + kk) & 7;
             const f32x2 wk = pack2(wz[k], wz[k]), dk = pack2(dz[k], dz[k]);
 #pragma unroll
             for (int h = 0; h < NP; ++h) {
@@ -433,8 +417,23 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
         for (int c = CB; c < 4; ++c) pend[c] = 0.f;
         pend[4] = fx; pend[5] = fy; pend[6] = fz; pend[7] = 0.f;
         pend_row = j - js;
-      }
+  };
+  {
+  unsigned rem = mask;        // non-empty cells not yet visited
+  bool first_cell = true;
+  while (rem != 0u) {
+    const int cur = __ffs(rem) - 1;   // current cell, relative to Z0
+    rem &= rem - 1u;
+    advance_to(Z0 + cur);
+    if (first_cell) {   // this segment's records were staged before the window loads were issued
+      cp_async_wait_all();
+      __syncwarp();
+      first_cell = false;
     }
+    const int jlo = __shfl_sync(0xffffffffu, jlo_l, cur);
+    const int jhi = __shfl_sync(0xffffffffu, jhi_l, cur);
+    for (int j = jlo; j < jhi; ++j) atom(j, std::integral_constant<int, 7>());
+  }
   }
   retire();
   flush(jend - js);
