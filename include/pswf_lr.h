@@ -93,6 +93,8 @@ typedef struct {
   long long own_kernel_launches; /* kernels of this library launched by the plan since creation (counted  */
   long long memsets;             /* at the launch sites), cudaMemsetAsync calls, and cuFFT executions      */
   long long cufft_execs;         /* (each a few cuFFT kernels; 0 on the band-limited path with pow-2 Mz)    */
+  long long graph_replays;       /* evaluations replayed from a cached CUDA graph (their launches are      */
+                                 /* included in the three counts above)                                    */
 } pswf_lr_info;
 
 /* Create a plan.  box[3]: edge lengths; grid[3]: M_x,M_y,M_z (each >= w, product < 2^31);
@@ -124,6 +126,9 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
  *   E    device, double[1]: total energy, Eq. (26) (accumulated in double); may be NULL
  *   phi  device, real[n_channels][n_atoms], phi_i^a = dE/dq_i^a; may be NULL
  *   F    device, real[n_atoms][3], F_i = -dE/dr_i; may be NULL
+ * Repeated calls with the same arguments (the same device buffers, as in an MD loop) are captured into a
+ * CUDA graph on the second call and replayed afterwards; calls made while `stream` is itself being captured
+ * launch plainly into the caller's capture.
  * Outputs are in the caller's atom order.  If phi and F are both NULL the inverse FFT and the
  * gather are skipped (the paper's energy-only path).  n_atoms = 0 is legal. */
 int pswf_lr_execute(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, void* E,

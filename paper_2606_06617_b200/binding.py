@@ -42,7 +42,7 @@ class Info(ctypes.Structure):
                 ("workspace_bytes", ctypes.c_longlong), ("fast_stencil", ctypes.c_int),
                 ("band_limited_fft", ctypes.c_int), ("band_kmax", ctypes.c_int * 3),
                 ("own_kernel_launches", ctypes.c_longlong), ("memsets", ctypes.c_longlong),
-                ("cufft_execs", ctypes.c_longlong)]
+                ("cufft_execs", ctypes.c_longlong), ("graph_replays", ctypes.c_longlong)]
 
 
 EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_plan_create_cell", "pswf_lr_execute", "pswf_lr_execute_host",

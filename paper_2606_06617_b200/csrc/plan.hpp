@@ -150,6 +150,21 @@ struct pswf_lr_plan {
   int last_n_atoms = 0;
   // launch accounting (pswf_lr_info): this library's own kernels, memsets, cuFFT executions since creation
   long long n_kernels = 0, n_memsets = 0, n_cufft = 0;
+  // launch sequences of pswf_lr_execute cached as CUDA graphs, keyed by the call's arguments (an MD loop
+  // passes the same device buffers every step); invalidated when workspaces are reallocated
+  struct GraphEntry {
+    int n = -1;
+    const void *pos = nullptr, *q = nullptr;
+    void *E = nullptr, *phi = nullptr, *F = nullptr;
+    bool virial = false;
+    cudaGraphExec_t exec = nullptr;
+    long long kernels = 0, memsets = 0, cufft = 0;   // launches one replay stands for
+    long long last_use = 0;
+  };
+  static constexpr int kGraphEntries = 4;
+  GraphEntry graphs[kGraphEntries];
+  bool use_graphs = true;
+  long long graph_clock = 0, n_graph_replays = 0;
   // cuFFT
   cufftHandle fft_fwd = 0, fft_inv = 0;
   bool have_fft = false;
