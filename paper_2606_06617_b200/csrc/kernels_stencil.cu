@@ -448,23 +448,36 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
       if (lane < NROW) s_row[tb * 32 + lane] = ri;
     }
     __syncwarp();
-#pragma unroll 6
-    for (int t = lane; t < NROW * NB; t += 32) {
+    // all of the lane's table entries are requested before the first one is used: ONE L2 round trip for
+    // the plane (with the loads issued in batches of six the producer needed three, and its ~6.6 us per
+    // plane ADDED to the consumers' time: spread = 140 us + 161 us x N / 1e6 at the config-4 grid)
+    constexpr int kEnt = (NROW * NB + 31) / 32;
+    int got[kEnt];
+#pragma unroll
+    for (int k = 0; k < kEnt; ++k) {
+      const int t = lane + 32 * k;
       const int r = t / NB, b = t - r * NB;
       const int syu = Y0 - (SW - 1) + r;
-      int val = 0;
-      if (syu < My) {
+      got[k] = 0;
+      if (t < NROW * NB && syu < My) {
         const int sy = syu < 0 ? syu + My : syu;
         const int* rs = start + ((size_t)sx * My + sy) * Mz;
-        const int4 ri = s_row[tb * 32 + r];
-        if (b < nAc) {
-          val = __ldg(rs + Mz - nAc + b) - ri.x;
-        } else {
-          const int bb = min(b, ncell) - nAc;
-          val = ri.y + __ldg(rs + zb0 + bb) - ri.z;
-        }
+        got[k] = b < nAc ? __ldg(rs + Mz - nAc + b) : __ldg(rs + zb0 + min(b, ncell) - nAc);
       }
-      s_L[(tb * NROW + r) * NB + b] = val;
+    }
+#pragma unroll
+    for (int k = 0; k < kEnt; ++k) {
+      const int t = lane + 32 * k;
+      const int r = t / NB, b = t - r * NB;
+      const int syu = Y0 - (SW - 1) + r;
+      if (t < NROW * NB) {
+        int val = 0;
+        if (syu < My) {
+          const int4 ri = s_row[tb * 32 + r];
+          val = b < nAc ? got[k] - ri.x : ri.y + got[k] - ri.z;
+        }
+        s_L[(tb * NROW + r) * NB + b] = val;
+      }
     }
   };
 
