@@ -425,32 +425,24 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
   const int oy = SW + (y & 7), oz = 2 * SW + (z0 & 7);
   const size_t Mtot = (size_t)Mx * My * Mz;
 
-  // Cell-boundary table of plane pl (producer warp).  Step 1: lane r fetches row r's run bases (4
-  // independent loads per lane, all rows at once).  Step 2: one load per table entry, unrolled so that
-  // several L2 round trips are in flight.  (Measured neutral against re-deriving the bases per entry:
-  // the consumers' waits on the full barrier come from their own imbalance -- the slowest of the four
-  // warps gates the empty barrier -- not from the producer.)
+  // Cell-boundary table of plane pl (producer warp): lane r fetches row r's run bases (4 loads), every
+  // lane its share of the 23 x 24 table entries (one load each).
   auto build_plane = [&](int pl) {
     const int tb = pl % NTAB;
     const int sx = X0 + pl;
-    {
-      const int syu = Y0 - (SW - 1) + lane;
-      int4 ri = make_int4(0, 0, 0, 0);
-      if (lane < NROW && syu < My) {
-        const int sy = syu < 0 ? syu + My : syu;
-        const int* rs = start + ((size_t)sx * My + sy) * Mz;
-        const int gA0 = nAc ? __ldg(rs + Mz - nAc) : 0;
-        const int eA = nAc ? __ldg(rs + Mz) : 0;
-        const int gB0 = __ldg(rs + zb0);
-        const int eB = __ldg(rs + zb0 + nBc);
-        ri = make_int4(gA0, eA - gA0, gB0, eB - gB0);
-      }
-      if (lane < NROW) s_row[tb * 32 + lane] = ri;
+    // every load of the plane -- the lane's row bases and its table entries -- is requested before the
+    // first result is used: ONE L2 round trip per plane (the producer's time per plane adds to the
+    // consumers': spread = 140 us + 161 us x N / 1e6 at the config-4 grid with three round trips)
+    const int syu_l = Y0 - (SW - 1) + lane;
+    const bool row_ok = lane < NROW && syu_l < My;
+    int gA0 = 0, eA = 0, gB0 = 0, eB = 0;
+    if (row_ok) {
+      const int sy = syu_l < 0 ? syu_l + My : syu_l;
+      const int* rs = start + ((size_t)sx * My + sy) * Mz;
+      if (nAc) { gA0 = __ldg(rs + Mz - nAc); eA = __ldg(rs + Mz); }
+      gB0 = __ldg(rs + zb0);
+      eB = __ldg(rs + zb0 + nBc);
     }
-    __syncwarp();
-    // all of the lane's table entries are requested before the first one is used: ONE L2 round trip for
-    // the plane (with the loads issued in batches of six the producer needed three, and its ~6.6 us per
-    // plane ADDED to the consumers' time: spread = 140 us + 161 us x N / 1e6 at the config-4 grid)
     constexpr int kEnt = (NROW * NB + 31) / 32;
     int got[kEnt];
 #pragma unroll
@@ -465,6 +457,8 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
         got[k] = b < nAc ? __ldg(rs + Mz - nAc + b) : __ldg(rs + zb0 + min(b, ncell) - nAc);
       }
     }
+    if (lane < NROW) s_row[tb * 32 + lane] = row_ok ? make_int4(gA0, eA - gA0, gB0, eB - gB0) : make_int4(0, 0, 0, 0);
+    __syncwarp();
 #pragma unroll
     for (int k = 0; k < kEnt; ++k) {
       const int t = lane + 32 * k;
