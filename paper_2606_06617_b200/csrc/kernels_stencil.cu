@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(kRecThreads) k_records(int n, int C, int recf,
 // plane, or -- when a single row holds more atoms than the staging buffer -- the atoms [a0, a1) of
 // the one row r0 (indices local to the row).
 struct RoundDesc {
-  int p;          // cell plane within the segment (0 .. NP-1); NP = finished
+  int p;          // cell plane, counted through the CTA's segments (a segment's planes are pb .. pe-1)
   int r0, r1;     // rows of the plane handled by this round
   int a0, a1;     // atom sub-range of a single-row round (0, INT_MAX otherwise)
   int total;      // atoms staged
@@ -385,7 +385,7 @@ template <int WY, int WZ, int CB, int NCTA>
 // register-saving copies in the atom loop, but 136 registers x 160 threads run as TWO CTAs per SM:
 // 353 us against 300 us.)
 __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
-    k_spread_os(int Mx, int My, int Mz, int nseg, int npy, int npz, int cap, int recf, int cb0,
+    k_spread_os(int Mx, int My, int Mz, int npy, int npz, int cap, int recf, int cb0,
                 const int* __restrict__ start, const float* __restrict__ rec, float* __restrict__ grid) {
   using S = SpreadShape<WY, WZ>;
   constexpr int NROW = S::NROW, NB = S::NB, NT = S::NT;
@@ -401,35 +401,50 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
   float* s_rec = reinterpret_cast<float*>(smem + S::kHeader + S::kTables + S::kRuns);     // [2][cap * recf]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  int bid = blockIdx.x;
-  const int pz = bid % npz; bid /= npz;
-  const int py = bid % npy; bid /= npy;
-  // this CTA's cell planes: the atoms are PARTITIONED over the x segments (no halo is re-read); the
-  // 7 output planes a segment shares with each neighbour are merged in global memory by RED
-  const int X0 = (int)((long long)bid * Mx / nseg), X1 = (int)((long long)(bid + 1) * Mx / nseg);
-  const int NP = X1 - X0;
-  const int Y0 = py * S::TY, Z0 = pz * S::TZ;
+  // This CTA's share of the work: the npy * npz patches x Mx cell planes, patch-major, are cut into
+  // gridDim.x equal ranges (one wave: every SM holds NCTA CTAs of the same length -- with whole segments
+  // per patch, 64 patches x 6 segments left 60 of 148 SMs a CTA short).  A range that crosses a patch
+  // boundary is one segment per patch, worked off one after the other.  The atoms are PARTITIONED over the segments
+  // (no halo is re-read); the 7 output planes a segment shares with each neighbour are merged in global
+  // memory by RED.
+  const int gtot = npy * npz * Mx;
+  const int g0 = (int)((long long)blockIdx.x * gtot / gridDim.x), g1 = (int)((long long)(blockIdx.x + 1) * gtot / gridDim.x);
+  const int nsg = (g1 - 1) / Mx - g0 / Mx + 1;   // 1, or 2 across a patch boundary (more only when patches outnumber CTAs)
+  int X0, NP, pb, pe, Y0, Z0, nAc, zb0, nBc, ncell;
   // cells of a row: sz_u = Z0-7 .. Z0+TZ-1; those below 0 wrap to the end of the row (run A)
-  const int nAc = Z0 < SW - 1 ? SW - 1 - Z0 : 0;
-  const int zb0 = Z0 - (SW - 1) + nAc;
-  const int nBc = min(S::NCELL - nAc, Mz - zb0);
-  const int ncell = nAc + nBc;
+  auto set_segment = [&](int sg) {
+    const int patch = g0 / Mx + sg;
+    const int lo = max(g0, patch * Mx), hi = min(g1, (patch + 1) * Mx);
+    X0 = lo - patch * Mx; NP = hi - lo;
+    pb = lo - g0; pe = pb + NP;          // running plane indices: table slots and barrier phases carry over
+    Y0 = (patch / npz) * S::TY; Z0 = (patch % npz) * S::TZ;
+    nAc = Z0 < SW - 1 ? SW - 1 - Z0 : 0;
+    zb0 = Z0 - (SW - 1) + nAc;
+    nBc = min(S::NCELL - nAc, Mz - zb0);
+    ncell = nAc + nBc;
+  };
+  set_segment(0);
 
   // this thread's two columns
   const int wy_ = warp / WZ, wz_ = warp % WZ;
   const int ly = lane >> 2, lzp = lane & 3;
-  const int y = Y0 + wy_ * 8 + ly, z0 = Z0 + wz_ * 8 + 2 * lzp;
-  const bool lane_ok = y < My && z0 < Mz;
+  int y, z0;
+  bool lane_ok;
+  auto set_columns = [&] {
+    y = Y0 + wy_ * 8 + ly; z0 = Z0 + wz_ * 8 + 2 * lzp;
+    lane_ok = y < My && z0 < Mz;
+  };
+  set_columns();
   const int rlo = wy_ * 8 + ly;          // first of the 8 rows (s_y = y-7 .. y) this thread reads
   const int clo = wz_ * 8 + 2 * lzp;     // boundary index of cell s_z = z0-7
-  const int oy = SW + (y & 7), oz = 2 * SW + (z0 & 7);
+  const int oy = SW + ly, oz = 2 * SW + 2 * lzp;   // patch origins are multiples of 8
   const size_t Mtot = (size_t)Mx * My * Mz;
 
   // Cell-boundary table of plane pl (producer warp): lane r fetches row r's run bases (4 loads), every
   // lane its share of the 23 x 24 table entries (one load each).
   auto build_plane = [&](int pl) {
     const int tb = pl % NTAB;
-    const int sx = X0 + pl;
+    const int sx = X0 + (pl - pb);
     // every load of the plane -- the lane's row bases and its table entries -- is requested before the
     // first result is used: ONE L2 round trip per plane (the producer's time per plane adds to the
     // consumers': spread = 140 us + 161 us x N / 1e6 at the config-4 grid with three round trips)
@@ -480,7 +495,7 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
     RoundDesc nd;
     nd.p = pn; nd.r0 = rn0; nd.r1 = NROW; nd.a0 = 0; nd.a1 = INT_MAX; nd.total = 0; nd.flush = 1;
     nd.np = pn + 1; nd.nr = 0; nd.na = 0;
-    if (pn < NP) {
+    if (pn < pe) {
       const int tb = pn % NTAB;
       const bool mine = lane >= rn0 && lane < NROW;
       int tot = mine ? s_L[(tb * NROW + lane) * NB + NB - 1] : 0;
@@ -528,10 +543,6 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
           bulk_g2s(dst + (size_t)(a_hi - a_lo) * recf, rec + (size_t)(ri.z + b_lo) * recf,
                    (uint32_t)(b_hi - b_lo) * recf * 4u, &full[nb]);
       }
-    } else {          // past the last plane: the terminal descriptor
-      if (lane == 0) s_desc[nb] = nd;
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&full[nb]);
     }
     return nd;
   };
@@ -547,16 +558,24 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
     //      Table slot (p+1) % NTAB last served plane p-NS, whose rounds were all released before the
     //      empty barrier of the first round of plane p could be passed (NS staging buffers: the
     //      producer is at most NS rounds ahead, and every plane in between holds at least one round).
-    build_plane(0);
-    __syncwarp();
-    int pn = 0, rn = 0, an = 0;
-    for (int n = 0;; ++n) {
-      const int nb = n % NS;
-      if (n >= NS) mbar_wait(&empty[nb], ((n / NS) - 1) & 1);
-      const RoundDesc nd = build_round(pn, rn, an, nb);
-      if (nd.p >= NP) break;
-      if (nd.r0 == 0 && nd.a0 == 0 && nd.p + 1 < NP) { build_plane(nd.p + 1); __syncwarp(); }
-      pn = nd.np; rn = nd.nr; an = nd.na;
+    //      The round counter n and the plane counter run on through the CTA's segments; a segment's
+    //      last round is the one that completes plane pe-1 (every plane has at least one round), so no
+    //      terminal descriptor is needed.  At a segment's first plane the slot pb % NTAB last served
+    //      plane pb-NTAB, released for the same reason.
+    int n = 0;
+    for (int sg = 0; sg < nsg; ++sg) {
+      if (sg) set_segment(sg);
+      build_plane(pb);
+      __syncwarp();
+      int pn = pb, rn = 0, an = 0;
+      for (;; ++n) {
+        const int nb = n % NS;
+        if (n >= NS) mbar_wait(&empty[nb], ((n / NS) - 1) & 1);
+        const RoundDesc nd = build_round(pn, rn, an, nb);
+        if (nd.r0 == 0 && nd.a0 == 0 && nd.p + 1 < pe) { build_plane(nd.p + 1); __syncwarp(); }
+        pn = nd.np; rn = nd.nr; an = nd.na;
+        if (pn >= pe) { ++n; break; }
+      }
     }
     return;
   }
@@ -570,11 +589,11 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
       for (int c = 0; c < CB; ++c) acc[k][u][c] = 0ull;
 
   // ---- consumer warps: free-running, coupled to the producer (and to nothing else) by the barriers
+  int sg = 0;
   for (int n = 0;; ++n) {
     const int cur = n % NS;
     mbar_wait(&full[cur], (n / NS) & 1);
     const RoundDesc d = s_desc[cur];
-    if (d.p >= NP) break;
     // ---- this thread's atoms of the round ----
     {
       const int tb = d.p % NTAB;
@@ -589,9 +608,9 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
     // ---- plane complete: its slot leaves the window; after the last cell plane so do the 7 planes
     //      beyond it.  Planes shared with a neighbouring segment are added (RED), the others stored.
     if (d.flush && lane_ok) {
-      const int nfl = d.p == NP - 1 ? SW : 1;
+      const int nfl = d.p == pe - 1 ? SW : 1;
       for (int i = 0; i < nfl; ++i) {
-        const int pl = d.p + i;
+        const int pl = d.p - pb + i;
         int P = X0 + pl; if (P >= Mx) P -= Mx;
         const bool shared = pl < SW - 1 || pl >= NP;
         float* gp = grid + (size_t)cb0 * Mtot + ((size_t)P * My + y) * Mz + z0;
@@ -615,6 +634,11 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
         }
       }
     }
+    if (d.flush && d.p == pe - 1) {   // the segment's last round: on to the CTA's second segment, if any
+      if (++sg == nsg) break;
+      set_segment(sg);
+      set_columns();
+    }
   }
 }
 
@@ -624,14 +648,14 @@ struct SpreadLaunch {
   static size_t smem_bytes(int cap, int recf) { return S::kHeader + S::kTables + S::kRuns + S::kStages * (size_t)cap * recf * 4; }
 
   template <int CB>
-  static void run(pswf_lr_plan* p, int nseg, int cap, int recf, int cb0, cudaStream_t st) {
+  static void run(pswf_lr_plan* p, int ncta, int cap, int recf, int cb0, cudaStream_t st) {
     const int Mx = p->M[0], My = p->M[1], Mz = p->M[2];
     const int npy = (My + S::TY - 1) / S::TY, npz = (Mz + S::TZ - 1) / S::TZ;
     const size_t sm = smem_bytes(cap, recf);
     auto kern = k_spread_os<WY, WZ, CB, NCTA>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     p->n_kernels += 1;
-    kern<<<(unsigned)(npy * npz * nseg), S::NT + 32, sm, st>>>(Mx, My, Mz, nseg, npy, npz, cap, recf, cb0, p->d_count,
+    kern<<<(unsigned)ncta, S::NT + 32, sm, st>>>(Mx, My, Mz, npy, npz, cap, recf, cb0, p->d_count,
                                                          (const float*)p->d_rec, (float*)p->d_grid);
   }
 
@@ -641,12 +665,12 @@ struct SpreadLaunch {
     const size_t budget = (size_t)(227 * 1024) / NCTA - 1024;
     int cap = (int)((budget - S::kHeader - S::kTables - S::kRuns) / (S::kStages * (size_t)recf * 4));
     cap &= ~7;
-    // x segments: ONE wave of CTAs.  The atoms are partitioned over the segments, so short segments
-    // cost no extra arithmetic, only RED traffic for the 7 shared planes; a second, partly filled
-    // wave would cost a full segment time (512 CTAs on 444 slots; profiles/r1b).
+    // ONE full wave of CTAs, each with the same number of (patch, cell plane) pairs.  The atoms are
+    // partitioned over the segments, so short segments cost no extra arithmetic, only RED traffic for the
+    // 7 shared planes; a second, partly filled wave would cost a full segment time (512 CTAs on 444 slots;
+    // profiles/r1b).  Never less than 8 planes per CTA.
     const int npatch = ((p->M[1] + S::TY - 1) / S::TY) * ((p->M[2] + S::TZ - 1) / S::TZ);
-    int nseg = NCTA * p->sm_count / npatch;
-    nseg = std::max(1, std::min(nseg, p->M[0] / SW));
+    const int nseg = std::max(1, std::min(NCTA * p->sm_count, npatch * (p->M[0] / SW)));
     const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
     cudaMemsetAsync(p->d_grid, 0, sizeof(float) * Mtot * p->C, st);   // the RED-merged planes start from zero
     p->n_memsets += 1;
