@@ -187,17 +187,20 @@ struct SpreadShape {
   static constexpr int TY = 8 * WY, TZ = 8 * WZ;
   static constexpr int NROW = TY + 7, NCELL = TZ + 7, NB = TZ + 8;
   static constexpr int NT = 32 * WY * WZ;
-  // staging buffers in flight, and cell-boundary tables (kStages + 1: plane p+1 is built while rounds
-  // of plane p+1-kStages may still be read).  Three stages were measured: the smaller buffers split
-  // every plane into two rounds and the spread went from 329 to 405 us.
+  // Staging buffers in flight: two, each as large as shared memory allows -- a cell plane whose atoms do
+  // not fit one buffer is split into two rounds, and every round costs the consumers a run-descriptor pass
+  // and a barrier (three smaller buffers split every plane: 329 -> 405 us, round 1).  Cell-boundary tables:
+  // two, handed back to the producer by the consumers (tabfree barriers) as soon as they have built the run
+  // descriptors of a plane's last round; a third table cost 11 records of each buffer.
   static constexpr int kStages = 2;
-  static constexpr int kTabs = kStages + 1;
+  static constexpr int kTabs = 2;
   static constexpr int kOffDesc = 64, kOffRowoff = 192, kOffRow = kOffRowoff + kStages * 32 * 4;
   static constexpr int kHeader = kOffRow + kTabs * 32 * 16;   // mbar | desc | rowoff | rowinfo
   static constexpr int kTables = kTabs * NROW * NB * 4;
-  static constexpr int kRuns = (SW + 1) * NT * 8;   // per thread: 8 packed run descriptors of the current round (+1: prefetch past the last)
+  static constexpr int kRuns = SW * NT * 8;   // per thread: 8 packed run descriptors of the current round (the prefetch past the
+                                               // last one reads the first staged records: in bounds, never used)
   static_assert(NROW <= 32, "one lane per row in the round builder");
-  static_assert(kOffDesc + kStages * sizeof(RoundDesc) <= kOffRowoff && 2 * kStages * 8 <= kOffDesc, "header");
+  static_assert(kOffDesc + kStages * sizeof(RoundDesc) <= kOffRowoff && (2 * kStages + kTabs) * 8 <= kOffDesc, "header");
 };
 
 // Packed FP32 pairs (sm_100a FFMA2: one instruction, two IEEE fused multiply-adds per lane -- the FLOP
@@ -393,6 +396,7 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
   constexpr int NS = S::kStages, NTAB = S::kTabs;
   uint64_t* full = reinterpret_cast<uint64_t*>(smem);                 // [NS] records of a round have landed
   uint64_t* empty = full + NS;                                        // [NS] all consumer warps are done with them
+  uint64_t* tabfree = empty + NS;                                     // [NTAB] ... with a plane's cell-boundary table
   RoundDesc* s_desc = reinterpret_cast<RoundDesc*>(smem + S::kOffDesc);   // [NS]
   int* s_rowoff = reinterpret_cast<int*>(smem + S::kOffRowoff);       // [NS][32]
   int4* s_row = reinterpret_cast<int4*>(smem + S::kOffRow);            // [NTAB][32]  {gA0, nA, gB0, nB}
@@ -473,6 +477,7 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
       }
     }
     if (lane < NROW) s_row[tb * 32 + lane] = row_ok ? make_int4(gA0, eA - gA0, gB0, eB - gB0) : make_int4(0, 0, 0, 0);
+    if (pl >= NTAB) mbar_wait(&tabfree[tb], ((pl / NTAB) - 1) & 1);   // plane pl-NTAB's table has been read
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < kEnt; ++k) {
@@ -549,19 +554,18 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
 
   if (tid == 0) {
     for (int i = 0; i < NS; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], WY * WZ); }
+    for (int i = 0; i < NTAB; ++i) mbar_init(&tabfree[i], WY * WZ);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
   if (warp == WY * WZ) {
     // ---- producer warp: cell-boundary tables one plane ahead, rounds two ahead of the consumers.
-    //      Table slot (p+1) % NTAB last served plane p-NS, whose rounds were all released before the
-    //      empty barrier of the first round of plane p could be passed (NS staging buffers: the
-    //      producer is at most NS rounds ahead, and every plane in between holds at least one round).
+    //      Table slot (p+1) % NTAB last served plane p+1-NTAB; build_plane waits for the consumers to
+    //      hand it back (tabfree) after its loads are in flight.
     //      The round counter n and the plane counter run on through the CTA's segments; a segment's
     //      last round is the one that completes plane pe-1 (every plane has at least one round), so no
-    //      terminal descriptor is needed.  At a segment's first plane the slot pb % NTAB last served
-    //      plane pb-NTAB, released for the same reason.
+    //      terminal descriptor is needed.
     int n = 0;
     for (int sg = 0; sg < nsg; ++sg) {
       if (sg) set_segment(sg);
@@ -601,6 +605,10 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
       const int r_hi = lane_ok ? min(rlo + SW, d.r1) : r_beg;
       const int total =
           build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32, d.a0, d.a1);
+      if (d.flush) {   // the plane's last round: its cell-boundary table goes back to the producer
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tabfree[tb]);
+      }
       walk_atoms<CB>(acc, s_run, NT, total, s_rec + (size_t)cur * cap * recf, recf, cb0, oy, oz);
     }
     __syncwarp();
@@ -662,7 +670,7 @@ struct SpreadLaunch {
   static void all_channels(pswf_lr_plan* p, cudaStream_t st) {
     const int recf = stencil_rec_floats(p->C);
     // staging capacity: NCTA CTAs per SM
-    const size_t budget = (size_t)(227 * 1024) / NCTA - 1024;
+    const size_t budget = (size_t)(228 * 1024) / NCTA - 1024;   // 228 KB per SM, 1 KB of it reserved per CTA
     int cap = (int)((budget - S::kHeader - S::kTables - S::kRuns) / (S::kStages * (size_t)recf * 4));
     cap &= ~7;
     // ONE full wave of CTAs, each with the same number of (patch, cell plane) pairs.  The atoms are
