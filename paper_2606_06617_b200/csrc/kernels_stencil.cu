@@ -252,26 +252,26 @@ __device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) {
 // one (v4 spent a third of its warp instructions there; profiles/r1f).  Returns the thread's atom
 // count of the round.
 __device__ __forceinline__ int build_runs(uint2* runs, const int NT, const int r_beg, const int r_hi, const int* Lp,
-                                          const int NB, const int* ro, const int a0, const int a1) {
+                                          const int NB, const int NROWS, const int* ro, const int a0, const int a1) {
   int total = 0;
   uint2* out = runs;
+  // branch-free: every lane handles 8 row slots; a row outside [r_beg, r_hi) or without atoms for this
+  // thread stores its descriptor too, but does not advance `out`, so the next one overwrites it
 #pragma unroll
   for (int i = 0; i < SW; ++i) {
     const int rr = r_beg + i;
-    if (rr < r_hi) {
-      const int2 a = *reinterpret_cast<const int2*>(Lp + rr * NB);
-      const int2 b = *reinterpret_cast<const int2*>(Lp + rr * NB + SW);
-      const int off = ro[rr] - a0;      // staged position of the row's atom 0
-      const int j = off + max(a.x, a0);
-      const int jend = off + min(b.y, a1);
-      const int ja = min(max(off + a.y, 0), 0xffff);
-      const int jb = min(max(off + b.x, 0), 0xffff);
-      if (jend > j) {
-        *out = make_uint2((unsigned)j | ((unsigned)jend << 16), (unsigned)ja | ((unsigned)jb << 16));
-        out += NT;
-        total += jend - j;
-      }
-    }
+    const int rc = min(rr, NROWS - 1);   // (clamped: stays inside the table; masked below)
+    const int2 a = *reinterpret_cast<const int2*>(Lp + rc * NB);
+    const int2 b = *reinterpret_cast<const int2*>(Lp + rc * NB + SW);
+    const int off = ro[rc] - a0;      // staged position of the row's atom 0
+    const int j = off + max(a.x, a0);
+    const int jend = off + min(b.y, a1);
+    const int ja = min(max(off + a.y, 0), 0xffff);
+    const int jb = min(max(off + b.x, 0), 0xffff);
+    const bool ne = rr < r_hi && jend > j;
+    *out = make_uint2((unsigned)j | ((unsigned)jend << 16), (unsigned)ja | ((unsigned)jb << 16));
+    out += ne ? NT : 0;
+    total += ne ? jend - j : 0;
   }
   return total;
 }
@@ -604,7 +604,7 @@ __global__ void __launch_bounds__(32 * WY * WZ + 32, NCTA)
       const int r_beg = max(rlo, d.r0);
       const int r_hi = lane_ok ? min(rlo + SW, d.r1) : r_beg;
       const int total =
-          build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, s_rowoff + cur * 32, d.a0, d.a1);
+          build_runs(s_run, NT, r_beg, r_hi, s_L + (size_t)tb * NROW * NB + clo, NB, NROW, s_rowoff + cur * 32, d.a0, d.a1);
       if (d.flush) {   // the plane's last round: its cell-boundary table goes back to the producer
         __syncwarp();
         if (lane == 0) mbar_arrive(&tabfree[tb]);
