@@ -676,9 +676,10 @@ struct SpreadLaunch {
     // ONE full wave of CTAs, each with the same number of (patch, cell plane) pairs.  The atoms are
     // partitioned over the segments, so short segments cost no extra arithmetic, only RED traffic for the
     // 7 shared planes; a second, partly filled wave would cost a full segment time (512 CTAs on 444 slots;
-    // profiles/r1b).  Never less than 8 planes per CTA.
+    // profiles/r1b).  On small grids down to one cell plane per CTA: the planes of a CTA are a latency
+    // chain of ~2.5 us each (42 -> 15 us at configuration 2 against 8 planes per CTA).
     const int npatch = ((p->M[1] + S::TY - 1) / S::TY) * ((p->M[2] + S::TZ - 1) / S::TZ);
-    const int nseg = std::max(1, std::min(NCTA * p->sm_count, npatch * (p->M[0] / SW)));
+    const int nseg = std::max(1, std::min(NCTA * p->sm_count, npatch * p->M[0]));
     const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
     cudaMemsetAsync(p->d_grid, 0, sizeof(float) * Mtot * p->C, st);   // the RED-merged planes start from zero
     p->n_memsets += 1;
