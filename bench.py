@@ -123,6 +123,15 @@ def profiled_traffic(kernel):
         return None
 
 
+def profiled_unit(key):
+    """A unit's busy fraction in the committed ncu --set full capture (profiles/r2_traffic.json), or None."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    try:
+        return float(json.load(open(path))["unit_busy"][key])
+    except Exception:
+        return None
+
+
 def algorithmic_bytes(N, C, M, B=4):
     """SURVEY.md §8(d) / DESIGN.md §6: bytes each stage must move per evaluation."""
     Mtot = M[0] * M[1] * M[2]
@@ -465,6 +474,13 @@ def run_ours(args):
                   "gbs": (bytes_alg[k] / (stage_ms[k] * 1e-3) / 1e9) if stage_ms[k] > 0 else None,
                   "hbm_frac": (bytes_alg[k] / (stage_ms[k] * 1e-3) / 1e9 / peak_gbs) if stage_ms[k] > 0 else None}
               for k in binding.STAGE_NAMES}
+    for k in ("spread", "gather"):      # the stencil stages also against the FP32 peak
+        if stage_ms[k] > 0:
+            stages[k]["alg_flops"] = flops_alg[k]
+            stages[k]["alu_frac"] = flops_alg[k] / (stage_ms[k] * 1e-3) / 1e12 / alu_peak
+    if args.cfg == 4 and args.atoms is None and args.kernel_path == 0:
+        # busiest unit of the spread in the committed ncu capture: the shared-memory data pipe
+        stages["spread"]["smem_pipe_frac_profiled"] = profiled_unit("spread_smem_pipe_frac")
     pipeline_bytes = sum(bytes_alg.values())
     ms_per_step = 1e3 * total_s_max / args.steps
 
