@@ -113,8 +113,8 @@ int pswf_lr_plan_create_ex(pswf_lr_plan** plan, const double box[3], const int g
  * s, k_m = 2 pi m h^-T, V = det h.  The grid has M_d points along a_d and the separable PSWF window
  * acts on the fractional coordinates; |a_d| / M_d takes the place of the grid spacing h_d in Eq. (29)
  * and in the defaults of r_c and c_window.  Positions, forces and the virial are Cartesian.  A diagonal
- * cell is the orthorhombic box of pswf_lr_plan_create_ex (same arithmetic).  pswf_lr_execute_real is
- * limited to orthorhombic cells (PSWF_LR_ERR_GRID_TOO_COARSE otherwise). */
+ * cell is the orthorhombic box of pswf_lr_plan_create_ex (same arithmetic).  pswf_lr_execute_real
+ * takes the minimum image in fractional coordinates there (see its r_c condition). */
 int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const int grid[3], int w,
                              double c, const int* exponents, int n_channels, const pswf_lr_opts* opts);
 
@@ -165,8 +165,9 @@ int pswf_lr_wait_host(pswf_lr_plan* plan);
  *   pswf_lr_execute(...); pswf_lr_execute_real(..., 1, stream);
  * returns the complete energy, potentials and forces of (S65).  Asynchronous on `stream`; it re-sorts
  * the atoms (the plan's sort buffers are shared with pswf_lr_execute: same-stream use only).
- * Fails with PSWF_LR_ERR_GRID_TOO_COARSE when r_c >= L_d / 2 in some dimension (only the minimum
- * image of a pair is visited). */
+ * Fails with PSWF_LR_ERR_GRID_TOO_COARSE when r_c is not below half the distance between opposite cell
+ * faces in every lattice direction (L_d / 2 in an orthorhombic box; V / |a_e x a_f| / 2 in a general
+ * cell): only the minimum image of a pair is visited. */
 int pswf_lr_execute_real(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, void* E,
                          void* phi, void* F, int accumulate, void* stream);
 

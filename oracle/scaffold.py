@@ -50,7 +50,8 @@ def real_space_parts(pos, q, exponents, box, c, r_c, fd=1e-6, subset=None):
         F_i = -dE/dr_i, with dL/dr by central differences of L (step fd): the scaffold has no
               closed-form derivative of its own, and none is needed at 1e-8 relative accuracy.
     With `subset` (atom indices) only those atoms' phi and F are computed (rows of the pair sum against
-    ALL atoms) and E is None: the sampled check of large systems."""
+    ALL atoms) and E is None: the sampled check of large systems.
+    The image loops cover ceil(r_c / width) cells around positions INSIDE the cell: wrap them first."""
     pos = np.asarray(pos, dtype=np.float64)
     q = np.atleast_2d(np.asarray(q, dtype=np.float64))
     cell = cell_matrix(box)

@@ -11,8 +11,10 @@
 // neighbours of an atom within r_c are, for every (dx, dy) cell-row offset, one contiguous run of
 // the sorted arrays (two when the z range wraps).  One warp per sorted atom, all channels; each
 // distinct exponent's polynomial is evaluated once per pair and shared by its channels.
-// Requirement (host-checked): r_c < L_d / 2 (minimum image).  Cell search radius
-// R_d = floor(r_c / h_d) + 1; a dimension with 2 R_d + 1 >= M_d is searched whole.
+// Requirement (host-checked): r_c < half the distance between opposite cell faces (minimum image; L_d / 2 in
+// an orthorhombic box).  Cell search radius R_d = floor(r_c / h_d) + 1 with h_d the distance between
+// neighbouring grid planes; a dimension with 2 R_d + 1 >= M_d is searched whole.  General cells (R-cell,
+// DESIGN.md §2): fractional coordinates, minimum image there, converted with the lattice vectors.
 #include "kernels_common.cuh"
 #include "launch.hpp"
 
@@ -28,6 +30,17 @@ __global__ void __launch_bounds__(256) k_sorted_pos(int n, int cap, const T* __r
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   const int i = perm[j];
+  if (g.tri) {   // wrapped fractional coordinates
+    const double r[3] = {(double)pos[3 * (size_t)i], (double)pos[3 * (size_t)i + 1], (double)pos[3 * (size_t)i + 2]};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      double s = r[0] * g.hinv[d] + r[1] * g.hinv[3 + d] + r[2] * g.hinv[6 + d];
+      s -= floor(s);
+      if (s >= 1.0) s = 0.0;
+      spos[(size_t)d * cap + j] = (T)s;
+    }
+    return;
+  }
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     double s = (double)pos[3 * (size_t)i + d] * g.invL[d];
@@ -144,9 +157,11 @@ __global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, Rea
         const int dx = ri / ny, dy = ri - dx * ny;
         const T ax = nx == Mx ? (T)0 : (T)max(abs(dx - g.R[0]) - 1, 0) * g.h[0];
         const T ay = ny == My ? (T)0 : (T)max(abs(dy - g.R[1]) - 1, 0) * g.h[1];
-        const T rem2 = rc2 - ax * ax - ay * ay;
+        // orthorhombic: the per-axis lower bounds add in quadrature; general cell: each bounds |r| on its own
+        // (|r| >= |ds_d| x plane distance), so a row is dropped only when one of them reaches r_c
+        const T rem2 = g.tri ? (ax < P.r_c && ay < P.r_c ? rc2 : (T)0) : rc2 - ax * ax - ay * ay;
         if (rem2 > (T)0) {
-          const int Rz = min(g.R[2], (int)(sqrt(rem2) * g.inv_hz) + 1);
+          const int Rz = g.tri ? g.R[2] : min(g.R[2], (int)(sqrt(rem2) * g.inv_hz) + 1);
           const int* row = start + ((size_t)wrap_index(x0 + dx, Mx) * My + wrap_index(y0 + dy, My)) * Mz;
           int z0 = allz ? 0 : cz - Rz, z1 = allz ? Mz : cz + Rz + 1;
           if (z0 < 0) { k2 = row[z0 + Mz]; k3 = row[Mz]; z0 = 0; }
@@ -163,9 +178,16 @@ __global__ void __launch_bounds__(128) k_real_pairs_q(int n, int C, int cap, Rea
           T ddx = 0, ddy = 0, ddz = 0, r2 = 0;
           if (k < kend && k != j) {
             ddx = spos[k] - xj; ddy = spos[(size_t)cap + k] - yj; ddz = spos[2 * (size_t)cap + k] - zj;
-            ddx -= g.L[0] * rint(ddx * (T)g.invL[0]);
-            ddy -= g.L[1] * rint(ddy * (T)g.invL[1]);
-            ddz -= g.L[2] * rint(ddz * (T)g.invL[2]);
+            if (g.tri) {
+              const T sx = ddx - rint(ddx), sy = ddy - rint(ddy), sz = ddz - rint(ddz);
+              ddx = sx * g.hm[0] + sy * g.hm[3] + sz * g.hm[6];
+              ddy = sx * g.hm[1] + sy * g.hm[4] + sz * g.hm[7];
+              ddz = sx * g.hm[2] + sy * g.hm[5] + sz * g.hm[8];
+            } else {
+              ddx -= g.L[0] * rint(ddx * (T)g.invL[0]);
+              ddy -= g.L[1] * rint(ddy * (T)g.invL[1]);
+              ddz -= g.L[2] * rint(ddz * (T)g.invL[2]);
+            }
             r2 = ddx * ddx + ddy * ddy + ddz * ddz;
             acc = r2 < rc2 && r2 > (T)0;
           }

@@ -66,8 +66,14 @@ struct RealGeom {
   int R[3];            // cell search radius per dimension: floor(r_c / h_d) + 1
   double invL[3];
   T L[3];
-  T h[3];              // grid spacing (cell size of the sort)
+  T h[3];              // cell size of the sort: distance between neighbouring grid planes (h_d in an orthorhombic box)
   T inv_hz;
+  // general cells (tri != 0): positions are kept as wrapped FRACTIONAL coordinates, the minimum image is taken
+  // there (valid for r_c < half the smallest distance between opposite cell faces, host-checked) and
+  // converted with the lattice vectors hm[3 d + e] (row d = vector a_d)
+  int tri;
+  double hinv[9];      // h^-1: s_d = sum_e r_e hinv[3 e + d]
+  T hm[9];
 };
 template <class T>
 struct RealParams {
@@ -106,6 +112,7 @@ struct pswf_lr_plan {
   pswf::WindowPoly wpoly;         // fast path copy of wt (float, zero padded)
   pswf::RealTable rt;             // real-space complement numerators N_p, S_p(0)
   int real_R[3] = {0, 0, 0};      // cell search radius of the pair kernel
+  double real_h[3] = {0, 0, 0};   // distance between neighbouring grid planes (h_d in an orthorhombic box)
   bool real_ok = false;           // r_c < L_d / 2 and 2 R_d + 1 <= M_d in every dimension
   void* d_rcoef = nullptr;
   void* d_rdcoef = nullptr;

@@ -304,9 +304,14 @@ int execute_real_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, 
     rg.R[d] = p->real_R[d];
     rg.invL[d] = 1.0 / p->L[d];
     rg.L[d] = (T)p->L[d];
-    rg.h[d] = (T)p->h[d];
+    rg.h[d] = (T)p->real_h[d];
   }
-  rg.inv_hz = (T)(1.0 / p->h[2]);
+  rg.inv_hz = (T)(1.0 / p->real_h[2]);
+  rg.tri = p->triclinic ? 1 : 0;
+  for (int i = 0; i < 9; ++i) {
+    rg.hinv[i] = p->hinv[i];
+    rg.hm[i] = (T)p->cell[i];
+  }
   P.C = p->C;
   P.nslots = (int)p->distinct_p.size();
   P.panels = p->rt.panels;
@@ -506,9 +511,13 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
       p->rt = fit_real(rm, p->distinct_p, panels, p->poly_eps, kMaxKernelDegree);
       p->real_ok = true;
       for (int d = 0; d < 3; ++d) {
-        p->real_R[d] = (int)std::floor(p->r_c / p->h[d]) + 1;
-        if (!(p->r_c < 0.5 * p->L[d])) p->real_ok = false;
-        if (p->triclinic) p->real_ok = false;   // the pair kernel's minimum image is per Cartesian axis
+        // distance between opposite cell faces: 1 / |column d of h^-1| (= L_d in an orthorhombic box)
+        double width = p->L[d];
+        if (p->triclinic)
+          width = 1.0 / std::sqrt(p->hinv[d] * p->hinv[d] + p->hinv[3 + d] * p->hinv[3 + d] + p->hinv[6 + d] * p->hinv[6 + d]);
+        p->real_h[d] = width / p->M[d];
+        p->real_R[d] = (int)std::floor(p->r_c / p->real_h[d]) + 1;
+        if (!(p->r_c < 0.5 * width)) p->real_ok = false;   // minimum image
       }
       // count modes in the ball (half spectrum), for info / roofline bytes
       long long cnt = 0;

@@ -661,6 +661,59 @@ def test_real_space_complement_vs_scaffold(precision, tol):
     plan.destroy()
 
 
+@pytest.mark.parametrize("precision,tol", [("f64", 1e-9), ("f32", 2e-5)])
+def test_real_space_complement_triclinic_vs_scaffold(precision, tol):
+    """The real-space row in a general cell: minimum image in fractional coordinates, cell
+    search over the grid planes of the skewed cell.  Against the scaffold's plain image loops."""
+    from oracle.scaffold import real_space_parts
+    rng = np.random.default_rng(23)
+    cell = np.array([[13.0, 0.0, 0.0], [3.5, 12.0, 0.0], [-2.5, 3.0, 14.0]])
+    grid, w, r_c = [24, 24, 32], 6, 4.4
+    N = 160
+    pos = rng.uniform(-0.4, 1.4, (N, 3)) @ cell          # atoms outside the cell too
+    q = rng.normal(0, 1, (4, N))
+    if precision == "f32":
+        pos = pos.astype(np.float32).astype(np.float64)
+        q = q.astype(np.float32).astype(np.float64)
+    wl = dict(pos=pos, q=q, exponents=[1, 3, 6, 8], box=cell, grid=grid, w=w, c=12.024, precision=precision)
+    plan = make_plan(wl, r_c=r_c)
+    E, phi, F = _run_real(wl, plan)
+    # the scaffold visits the images ceil(r_c / width) around positions INSIDE the cell: wrap them for it
+    frac = pos @ np.linalg.inv(cell)
+    pos_in = (frac - np.floor(frac)) @ cell
+    E_ref, phi_ref, F_ref = real_space_parts(pos_in, q, wl["exponents"], cell, wl["c"], r_c)
+    print("real triclinic %s: eps_E=%.2e eps_phi=%.2e eps_F=%.2e" % (precision, abs(E - E_ref) / abs(E_ref),
+                                                                    rel(phi, phi_ref), rel(F, F_ref)))
+    assert abs(E - E_ref) <= tol * abs(E_ref)
+    assert rel(phi, phi_ref) <= tol
+    assert rel(F, F_ref) <= max(tol, 1e-7)
+    assert np.abs(phi - phi_ref).max() <= 8 * tol * np.abs(phi_ref).max()
+    plan.destroy()
+
+
+def test_full_decomposition_triclinic_independent_of_splitting():
+    """(S65) in a triclinic cell from the GPU alone: reciprocal + real-space - self is the plain periodic
+    inverse-power energy, so it must not depend on (c, r_c).  A neutral p = 1 channel and a charged p = 6
+    channel (zero mode (S78)); fp64, w = 16, bands as in the oracle's own invariance pin."""
+    rng = np.random.default_rng(29)
+    cell = np.array([[9.0, 0.0, 0.0], [2.0, 8.5, 0.0], [-1.5, 1.0, 9.5]])
+    N = 40
+    pos = rng.uniform(0, 1, (N, 3)) @ cell
+    q = rng.normal(0, 1, (2, N))
+    q[0] -= q[0].mean()
+    res = []
+    for c, r_c in ((26.0, 3.0), (30.0, 3.9)):
+        wl = dict(pos=pos, q=q, exponents=[1, 6], box=cell, grid=[56, 56, 60], w=16, c=c, precision="f64")
+        plan = make_plan(wl, r_c=r_c)
+        res.append(_run_real(wl, plan, accumulate_after_recip=True))
+        plan.destroy()
+    (E1, phi1, F1), (E2, phi2, F2) = res
+    print("triclinic S65: E = %.12f / %.12f, dF = %.2e, dphi = %.2e" % (E1, E2, rel(F1, F2), rel(phi1, phi2)))
+    assert abs(E1 - E2) <= 1e-7 * abs(E1)
+    assert rel(F1, F2) <= 1e-6
+    assert rel(phi1, phi2) <= 1e-6
+
+
 def test_real_space_large_system_sampled_fp32():
     """The thread-per-atom variant of the pair kernel (n >= 65536): 70,000 atoms at 0.1 A^-3, sampled
     atoms against the scaffold's rows over ALL atoms (fp32 gates)."""
@@ -790,6 +843,34 @@ def test_virial_real_space_vs_strain_derivative_of_scaffold():
     _run_real(wl, plan, accumulate_after_recip=True)
     W_tot = _virial(plan)
     assert np.abs(W_tot - (W_rec + W)).max() <= 1e-11 * np.abs(W_tot).max()
+    plan.destroy()
+
+
+def test_virial_real_space_triclinic_all_components():
+    """Pair virial in a triclinic cell: W_ab = -dE/d(eps_ab) of the scaffold's real-space energy under the
+    symmetric strain r -> r (1 + eps), h -> h (1 + eps) (central differences), all six components."""
+    from oracle.scaffold import real_space_parts
+    rng = np.random.default_rng(27)
+    cell = np.array([[13.0, 0.0, 0.0], [3.5, 12.0, 0.0], [-2.5, 3.0, 14.0]])
+    N, r_c = 70, 4.4
+    pos = rng.uniform(0, 1, (N, 3)) @ cell
+    q = rng.normal(0, 1, (2, N))
+    ex = [1, 6]
+    wl = dict(pos=pos, q=q, exponents=ex, box=cell, grid=[24, 24, 32], w=8, c=12.024, precision="f64")
+    plan = make_plan(wl, r_c=r_c)
+    plan.set_virial(True)
+    _run_real(wl, plan)
+    W = _virial(plan)
+    assert np.abs(W - W.T).max() <= 1e-12 * np.abs(W).max()
+    for a_, b_ in [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]:
+        e = 1e-6
+        eps = np.zeros((3, 3))
+        eps[a_, b_] += 0.5 * e
+        eps[b_, a_] += 0.5 * e
+        sp, sm = np.eye(3) + eps, np.eye(3) - eps
+        fd = -(real_space_parts(pos @ sp, q, ex, cell @ sp, 12.024, r_c)[0]
+               - real_space_parts(pos @ sm, q, ex, cell @ sm, 12.024, r_c)[0]) / (2 * e)
+        assert abs(fd - W[a_, b_]) <= 1e-6 * np.abs(W).max(), (a_, b_, fd, W[a_, b_])
     plan.destroy()
 
 
