@@ -49,7 +49,8 @@ typedef enum {
   PSWF_LR_ERR_ALLOC = -4,
   PSWF_LR_ERR_CUDA = -5,
   PSWF_LR_ERR_CUFFT = -6,
-  PSWF_LR_ERR_BUSY = -7                  /* host submissions in flight: pswf_lr_wait_host first    */
+  PSWF_LR_ERR_BUSY = -7,                 /* host submissions in flight: pswf_lr_wait_host first    */
+  PSWF_LR_ERR_TOO_LARGE = -8             /* size beyond the static scratch of a no-allocation call  */
 } pswf_lr_status;
 
 enum { PSWF_LR_F32 = 0, PSWF_LR_F64 = 1 };
@@ -203,6 +204,29 @@ int pswf_lr_stage_ms(pswf_lr_plan* plan, double ms[PSWF_LR_N_STAGES], int* n_exe
  * Only meaningful when the intermediate still exists (call right after execute; the real grid is
  * overwritten by the inverse FFT, so what = 0 needs an execute with phi = F = NULL). */
 int pswf_lr_debug_copy(pswf_lr_plan* plan, int what, void* dst, void* stream);
+
+/* Test hook: copy the cell starts of the most recent execute -- the exclusive scan of the atoms-per-cell
+ * counts of step a0 (cell key = stencil cell (s_x, s_y, s_z), z fastest), with the
+ * atom count in the last entry -- to a caller's DEVICE buffer int[Mx*My*Mz + 1]. */
+int pswf_lr_debug_cell_starts(pswf_lr_plan* plan, int* dst, void* stream);
+
+/* NO-ALLOCATION entry point, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): the exclusive scan of step a0 (cell counts -> cell starts, the
+ * kernel the plans use) without a plan.  Its scratch -- the tile states of the single-pass scan -- lives in
+ * a file-scope device array of the library (8200 bytes, held by every GPU that loads the library until the
+ * process exits) instead of a cudaMalloc'd workspace.  The call performs no cudaMalloc / cudaFree and calls
+ * no allocating library routine.
+ *   counts: DEVICE pointer (current device), int[n + 1], 16-byte aligned.  In place: on return (stream
+ *           order) counts[i] = counts_in[0] + ... + counts_in[i-1] for 0 <= i <= n, i.e. counts[n] = total
+ *           (what counts[n] held on entry is ignored).  The total must fit in an int.
+ *   n:      0 <= n <= PSWF_LR_SCAN_STATIC_MAX (2^24: a 256^3 grid); beyond it PSWF_LR_ERR_TOO_LARGE and
+ *           nothing is launched.  NULL or misaligned counts, n < 0: PSWF_LR_ERR_INVALID_ARG.
+ * Asynchronous on `stream`; no host synchronisation.  The scratch is SHARED by all calls of the process on
+ * that GPU and keeps the previous call's contents (the call clears what it uses first): calls that overlap
+ * on the GPU -- two streams, two host threads -- race; serialise them.  The first call on a device resolves
+ * the array's device address (cudaGetSymbolAddress): make it once before capturing a graph. */
+enum { PSWF_LR_SCAN_STATIC_MAX = 1 << 24 };
+int pswf_lr_exclusive_scan_static(int* counts, int n, void* stream);
 
 /* Host-side evaluation of the plan's fitted tables (tests compare them with the oracle):
  *   window:  W(z) and dW/dz for z in [-1,1) from the panel polynomials

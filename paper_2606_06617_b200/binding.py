@@ -19,6 +19,7 @@ STAGE_NAMES = ("bin_sort", "spread", "fft_forward", "scale_reduce", "fft_inverse
 
 ERR_INVALID_ARG, ERR_UNSUPPORTED_EXPONENT, ERR_GRID_TOO_COARSE, ERR_ALLOC, ERR_CUDA, ERR_CUFFT = \
     -1, -2, -3, -4, -5, -6
+ERR_BUSY, ERR_TOO_LARGE = -7, -8
 
 
 class PswfLrError(RuntimeError):
@@ -49,7 +50,7 @@ EXPORTS = ("pswf_lr_plan_create", "pswf_lr_plan_create_ex", "pswf_lr_plan_create
            "pswf_lr_submit_host", "pswf_lr_wait_host",
            "pswf_lr_execute_real", "pswf_lr_eval_real", "pswf_lr_self_coefficient", "pswf_lr_suggest_parameters", "pswf_lr_set_virial", "pswf_lr_virial",
            "pswf_lr_channel_energies", "pswf_lr_get_info", "pswf_lr_set_profiling", "pswf_lr_stage_ms",
-           "pswf_lr_debug_copy", "pswf_lr_eval_window", "pswf_lr_eval_kernel", "pswf_lr_destroy",
+           "pswf_lr_debug_copy", "pswf_lr_debug_cell_starts", "pswf_lr_exclusive_scan_static", "pswf_lr_eval_window", "pswf_lr_eval_kernel", "pswf_lr_destroy",
            "pswf_lr_error_string", "pswf_lr_version")
 
 _lib = None
@@ -85,6 +86,8 @@ def lib():
         L.pswf_lr_set_profiling.argtypes = [vp, ip]
         L.pswf_lr_stage_ms.argtypes = [vp, dp, ctypes.POINTER(ip)]
         L.pswf_lr_debug_copy.argtypes = [vp, ip, vp, vp]
+        L.pswf_lr_debug_cell_starts.argtypes = [vp, vp, vp]
+        L.pswf_lr_exclusive_scan_static.argtypes = [vp, ip, vp]
         L.pswf_lr_eval_window.argtypes = [vp, ip, dp, dp, dp]
         L.pswf_lr_eval_kernel.argtypes = [vp, ip, ip, dp, dp]
         L.pswf_lr_destroy.argtypes = [vp]
@@ -110,6 +113,15 @@ def _ptr(t):
     if isinstance(t, np.ndarray):
         return ctypes.c_void_p(t.ctypes.data)
     return ctypes.c_void_p(t.data_ptr())
+
+
+SCAN_STATIC_MAX = 1 << 24
+
+
+def exclusive_scan_static(counts, n, stream=None):
+    """pswf_lr_exclusive_scan_static: in-place exclusive scan of the int32 device tensor counts[n + 1]
+    (counts[n] receives the total) with the library's static scratch; allocates nothing."""
+    _check(lib().pswf_lr_exclusive_scan_static(_ptr(counts), int(n), ctypes.c_void_p(stream or 0)))
 
 
 def suggest_parameters(box, eps_tot, r_c):
@@ -242,6 +254,9 @@ class Plan:
 
     def debug_copy(self, what, dst, stream=None):
         _check(lib().pswf_lr_debug_copy(self._h, int(what), _ptr(dst), ctypes.c_void_p(stream or 0)))
+
+    def debug_cell_starts(self, dst, stream=None):
+        _check(lib().pswf_lr_debug_cell_starts(self._h, _ptr(dst), ctypes.c_void_p(stream or 0)))
 
     def set_profiling(self, enabled):
         _check(lib().pswf_lr_set_profiling(self._h, 1 if enabled else 0))

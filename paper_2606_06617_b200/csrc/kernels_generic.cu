@@ -4,6 +4,8 @@
 // any channel count); the fp64 path and kernel_path = 1 always use them.  The tiled fp32
 // kernels in kernels_stencil.cu / kernels_gather.cu replace sort-scatter, spread and gather on the
 // default path.
+#include <atomic>
+
 #include "kernels_common.cuh"
 #include "kernels_scale.cuh"
 #include "launch.hpp"
@@ -127,6 +129,48 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_lookback(int n, int* __re
     }
   }
   if (tile == 0 && threadIdx.x == 0) data[total_slot] = total;
+}
+
+// ------------------------------------------------------------------------------------------------
+// No-allocation variant of the scan (pswf_lr_exclusive_scan_static, include/pswf_lr.h): the tile state
+// lives in a file-scope device array instead of the plan's cudaMalloc'd d_scan_state.  8200 bytes, held by
+// every GPU that loads the library until the process exits.  All calls share it: calls that overlap on
+// the GPU (two streams) race.
+// ------------------------------------------------------------------------------------------------
+constexpr int kScanStaticTiles = PSWF_LR_SCAN_STATIC_MAX / (kScanThreads * kScanItems);   // 1024 tiles of 16384 counts
+static_assert(kScanStaticTiles * kScanThreads * kScanItems == PSWF_LR_SCAN_STATIC_MAX, "whole tiles");
+static __device__ __align__(256) unsigned long long g_scan_state_static[kScanStaticTiles + 1];
+
+// the inclusive prefix of the last tile is the total
+__global__ void k_scan_total(const unsigned long long* __restrict__ state, int ntiles, int* __restrict__ out) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) *out = (int)(unsigned int)state[ntiles];
+}
+
+// In host code g_scan_state_static is a host-side stand-in, not a device address: the address the kernels
+// get comes from cudaGetSymbolAddress, looked up once per device with that device current (no allocation).
+int launch_scan_static(int* data, int n, cudaStream_t st) {
+  constexpr int kDevs = 64;
+  static std::atomic<unsigned long long*> cache[kDevs];
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PSWF_LR_ERR_CUDA; }
+  unsigned long long* state = (dev >= 0 && dev < kDevs) ? cache[dev].load() : nullptr;
+  if (!state) {
+    if (cudaGetSymbolAddress((void**)&state, g_scan_state_static) != cudaSuccess || !state) {
+      cudaGetLastError();
+      return PSWF_LR_ERR_CUDA;
+    }
+    if (dev >= 0 && dev < kDevs) cache[dev].store(state);
+  }
+  const int ntiles = (n + kScanThreads * kScanItems - 1) / (kScanThreads * kScanItems);
+  // the array keeps the previous call's ticket counter and tile states: all of what this call uses restarts at zero
+  if (cudaMemsetAsync(state, 0, sizeof(unsigned long long) * ((size_t)ntiles + 1), st) != cudaSuccess) {
+    cudaGetLastError();
+    return PSWF_LR_ERR_CUDA;
+  }
+  k_scan_lookback<<<ntiles, kScanThreads, 0, st>>>(n, data, state, n, 0);
+  k_scan_total<<<1, 32, 0, st>>>(state, ntiles, data + n);
+  if (cudaGetLastError() != cudaSuccess) return PSWF_LR_ERR_CUDA;
+  return 0;
 }
 
 template <class T>

@@ -8,6 +8,7 @@ template <class T>
 void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, bool scatter,
                      cudaStream_t st);
 int scan_tile_size();   // counts per tile of the single-pass scan (sizes its state array)
+int launch_scan_static(int* data, int n, cudaStream_t st);   // 1 <= n <= PSWF_LR_SCAN_STATIC_MAX; no allocation
 template <class T>
 void launch_spread_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, cudaStream_t st);
 template <class T>

@@ -1,6 +1,7 @@
 // C ABI of libpswf_lr: plan creation (host-side PSWF solve + Horner tables + cuFFT plans),
 // execute (bin/sort -> spread -> FFT -> scale+reduce -> inverse FFT -> gather), destroy.
 // See include/pswf_lr.h for the contract and the PAPER.md passages behind each step.
+#include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -348,6 +349,7 @@ const char* pswf_lr_error_string(int code) {
     case PSWF_LR_ERR_CUDA: return "CUDA error (no usable device, or a kernel/launch failed)";
     case PSWF_LR_ERR_CUFFT: return "cuFFT error";
     case PSWF_LR_ERR_BUSY: return "busy: host submissions in flight (call pswf_lr_wait_host first)";
+    case PSWF_LR_ERR_TOO_LARGE: return "size beyond the static scratch of a no-allocation entry point (PSWF_LR_SCAN_STATIC_MAX)";
   }
   return "unknown error";
 }
@@ -968,6 +970,27 @@ int pswf_lr_debug_copy(pswf_lr_plan* p, int what, void* dst, void* stream) {
   }
   CUDA_TRY(cudaMemcpyAsync(dst, src, nb, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
   return 0;
+}
+
+int pswf_lr_debug_cell_starts(pswf_lr_plan* p, int* dst, void* stream) {
+  if (!p || !dst) return PSWF_LR_ERR_INVALID_ARG;
+  if (p->host_only) return PSWF_LR_ERR_CUDA;
+  DeviceGuard guard(p);
+  const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
+  CUDA_TRY(cudaMemcpyAsync(dst, p->d_count, sizeof(int) * (Mtot + 1), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return 0;
+}
+
+int pswf_lr_exclusive_scan_static(int* counts, int n, void* stream) {
+  if (!counts || n < 0) return PSWF_LR_ERR_INVALID_ARG;
+  if (n > PSWF_LR_SCAN_STATIC_MAX) return PSWF_LR_ERR_TOO_LARGE;   // beyond the static tile-state array
+  if (((uintptr_t)counts & 15u) != 0) return PSWF_LR_ERR_INVALID_ARG;   // the scan reads and writes 16-byte vectors
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n == 0) {
+    CUDA_TRY(cudaMemsetAsync(counts, 0, sizeof(int), st));
+    return 0;
+  }
+  return launch_scan_static(counts, n, st);
 }
 
 int pswf_lr_eval_window(const pswf_lr_plan* p, int n, const double* z, double* W, double* dW) {
