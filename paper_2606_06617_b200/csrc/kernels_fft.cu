@@ -90,6 +90,31 @@ struct Dft<8, INV> {
   }
 };
 
+template <bool INV>
+struct Dft<16, INV> {
+  static __device__ __forceinline__ void run(float2 (&v)[16]) {
+    float2 e[8] = {v[0], v[2], v[4], v[6], v[8], v[10], v[12], v[14]};
+    float2 o[8] = {v[1], v[3], v[5], v[7], v[9], v[11], v[13], v[15]};
+    Dft<8, INV>::run(e);
+    Dft<8, INV>::run(o);
+    // W16^k = exp(-+ 2 pi i k / 16), k = 1 .. 7 (upper sign: forward)
+    const float h = 0.70710678118654752f, c1 = 0.92387953251128674f, s1 = 0.38268343236508977f;
+    const float sg = INV ? 1.f : -1.f;
+    o[1] = cmul(o[1], make_float2(c1, sg * s1));
+    o[2] = cmul(o[2], make_float2(h, sg * h));
+    o[3] = cmul(o[3], make_float2(s1, sg * c1));
+    o[4] = rot90<INV>(o[4]);
+    o[5] = cmul(o[5], make_float2(-s1, sg * c1));
+    o[6] = cmul(o[6], make_float2(-h, sg * h));
+    o[7] = cmul(o[7], make_float2(-c1, sg * s1));
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      v[k] = cadd(e[k], o[k]);
+      v[k + 8] = csub(e[k], o[k]);
+    }
+  }
+};
+
 // One radix-R pass over `npen` pencils of length N.  Element n of pencil p is s[pen(p) * sp + n * sn];
 // consecutive threads take consecutive pencils (conflict-free for sp = 1, and for sp = pitch = My + 1).
 // Forward (decimation in frequency): the block of length L splits into R sub-blocks of length L / R,
@@ -281,8 +306,8 @@ template <> struct Rad<8>   { static constexpr int n = 1, r0 = 8, r1 = 1, r2 = 1
 template <> struct Rad<16>  { static constexpr int n = 2, r0 = 4, r1 = 4, r2 = 1; };
 template <> struct Rad<32>  { static constexpr int n = 2, r0 = 8, r1 = 4, r2 = 1; };
 template <> struct Rad<64>  { static constexpr int n = 2, r0 = 8, r1 = 8, r2 = 1; };
-template <> struct Rad<128> { static constexpr int n = 3, r0 = 8, r1 = 4, r2 = 4; };
-template <> struct Rad<256> { static constexpr int n = 3, r0 = 8, r1 = 8, r2 = 4; };
+template <> struct Rad<128> { static constexpr int n = 2, r0 = 16, r1 = 8, r2 = 1; };   // two shared-memory passes instead of three (8, 4, 4)
+template <> struct Rad<256> { static constexpr int n = 2, r0 = 16, r1 = 16, r2 = 1; };
 
 __host__ __device__ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
 
@@ -493,11 +518,16 @@ __global__ void __launch_bounds__(kZThreads)
   }
   {
     const float* src = grid + (((size_t)c * Mx + x) * My + y0) * NZ;   // YT contiguous pencils
-    for (int i = tid; i < YT * NZ; i += NT) {
-      const int y = i / NZ, n = i % NZ;
-      const float v = __ldg(src + i);
-      float* d = reinterpret_cast<float*>(s + (y >> 1) * pitch + n);
-      d[y & 1] = v;
+    // pencils 2q (real part) and 2q+1 (imaginary part), four z at a time: two 16-byte loads, four complex stores
+    for (int i = tid; i < npen * (NZ / 4); i += NT) {
+      const int q = i / (NZ / 4), n = (i % (NZ / 4)) * 4;
+      const float4 a = __ldg(reinterpret_cast<const float4*>(src + (size_t)(2 * q) * NZ + n));
+      const float4 b = __ldg(reinterpret_cast<const float4*>(src + (size_t)(2 * q + 1) * NZ + n));
+      float2* d = s + q * pitch + n;
+      d[0] = make_float2(a.x, b.x);
+      d[1] = make_float2(a.y, b.y);
+      d[2] = make_float2(a.z, b.z);
+      d[3] = make_float2(a.w, b.w);
     }
   }
   __syncthreads();
