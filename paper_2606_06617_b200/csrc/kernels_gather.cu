@@ -303,12 +303,19 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
 #undef PSWF_SLOT
         }
       } else {
+        // slot k holds plane pk = base + k (k >= an mod 8) or base + 8 + k (k < an mod 8), base = an rounded
+        // down to a multiple of 8; M_z is a multiple of 8, so the wrap past M_z hits the second group as a whole:
+        // two base offsets per advance, one select and one multiply-add per slot
+        const int a7 = an & 7, base = an - a7;
+        const unsigned offA = (unsigned)(base >= Mz ? base - Mz : base) * plane;
+        const int baseB = base + SW;
+        const unsigned offB = (unsigned)(baseB >= Mz ? baseB - Mz : baseB) * plane;
+        const int lim = first_new - base;           // load slot k iff k + (k < a7 ? 8 : 0) >= lim
 #pragma unroll
         for (int k = 0; k < SW; ++k) {
-          const int pk = an + ((k - an) & 7);
-          if (pk >= first_new) {
-            const int z = pk >= Mz ? pk - Mz : pk;
-            const unsigned off = (unsigned)z * plane;
+          const bool hi = k < a7;
+          if (k + (hi ? SW : 0) >= lim) {
+            const unsigned off = (hi ? offB : offA) + (unsigned)k * plane;
             ldw(g0 + off, win[k][0]);
             ldw(g1 + off, win[k][1]);
           }
