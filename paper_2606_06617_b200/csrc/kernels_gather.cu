@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
       }
       if (Facc) {
         // the derivative records are along the fractional coordinates: F_e = sum_d hinv[e][d] F^s_d
-        float fx = f.x, fy = f.y, fz = f.z;
+        float fx = -f.x, fy = -f.y, fz = -f.z;   // F = -sum_a q_a grad phi_a
         frac_to_cart(Hi.m, fx, fy, fz);
         float* fp = Facc + 3 * (size_t)perm_l;
         if (accumulate_F) { fp[0] += fx; fp[1] += fy; fp[2] += fz; }
@@ -273,10 +273,17 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   for (int i = 0; i < 8; ++i) pend[i] = 0.f;
   // lane l with (l & 3) == 0 ends up with output index (l>>4)*4 + ((l>>3)&1)*2 + ((l>>2)&1)
   const int out_idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
-  int pend_row = kStage;   // result row of the pending atom; kStage = the spare row (nothing pending)
+  // result slot of the pending atom for this lane; the spare row (kStage) when nothing is pending.  Running
+  // pointers (records, derivative records, result slot) replace a per-atom multiply-and-add chain each.
+  float* const out_spare = s_out + 8 * kStage + out_idx;
+  float* pend_dst = out_spare;
+  const float* rp = s_rec;                 // record of the next atom (atoms of a segment are one contiguous run)
+  const float* dp = s_drec;
+  float* out_cur = s_out + out_idx;
+  int staged_left = kStage;                // atoms left in the staging buffer
   auto retire = [&]() {
     const float tot = reduce8(pend, lane);
-    if ((lane & 3) == 0) s_out[8 * pend_row + out_idx] = tot;
+    if ((lane & 3) == 0) *pend_dst = tot;
   };
 
   // walk the non-empty cells of the segment; the window advances to each of them in one go
@@ -326,17 +333,19 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   // one atom: S = slot of the NEWEST plane of the window; the z contraction visits it last
   auto atom = [&](const int j, auto Sc) {
       constexpr int S = decltype(Sc)::value;
-        if (j - js >= kStage) {   // staging buffer exhausted (dense rows): write results, stage the next atoms
+        if (staged_left == 0) {   // staging buffer exhausted (dense rows): write results, stage the next atoms
           retire();
-          pend_row = kStage;
+          pend_dst = out_spare;
           flush(kStage);
           js += kStage;
           stage();
           cp_async_wait_all();
           __syncwarp();
+          rp = s_rec; dp = s_drec; out_cur = s_out + out_idx; staged_left = kStage;
         }
-        const float* r = s_rec + (j - js) * recf;
-        const float* dr = s_drec + (j - js) * (3 * SW);
+        const float* r = rp;
+        const float* dr = dp;
+        rp += recf; dp += 3 * SW; --staged_left;
         const float4 za = *reinterpret_cast<const float4*>(r + 2 * SW);
         const float4 zb = *reinterpret_cast<const float4*>(r + 2 * SW + 4);
         const float4 da = *reinterpret_cast<const float4*>(dr + 2 * SW);
@@ -393,9 +402,10 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
           unpack2(T01, a, b); const float t01 = a + b;
           unpack2(T10, a, b); const float t10 = a + b;
           unpack2(T11, a, b); const float t11 = a + b;
-          fx = -fmaf(dxy[1], t01, dxy[0] * t00);
-          fy = -fmaf(xdy[1], t01, xdy[0] * t00);
-          fz = -fmaf(xy[1], t11, xy[0] * t10);
+          // (minus sign: applied once per atom in flush())
+          fx = wy * fmaf(dx1, t01, dx0 * t00);
+          fy = dy * fmaf(wx1, t01, wx0 * t00);
+          fz = fmaf(xy[1], t11, xy[0] * t10);
         } else {
 #pragma unroll
         for (int c = 0; c < CB; ++c) {
@@ -414,16 +424,17 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
             gy = fmaf(xdy[u], S0, gy);
           }
           const float qc = qv[c];
-          fx = fmaf(-qc, gx, fx);
-          fy = fmaf(-qc, gy, fy);
-          fz = fmaf(-qc, gz, fz);
+          fx = fmaf(qc, gx, fx);
+          fy = fmaf(qc, gy, fy);
+          fz = fmaf(qc, gz, fz);
           pend[c] = val;
         }
         }
 #pragma unroll
         for (int c = CB; c < 4; ++c) pend[c] = 0.f;
         pend[4] = fx; pend[5] = fy; pend[6] = fz; pend[7] = 0.f;
-        pend_row = j - js;
+        pend_dst = out_cur;
+        out_cur += 8;
   };
   {
   unsigned rem = mask;        // non-empty cells not yet visited
