@@ -28,6 +28,7 @@
 //    channel per lane), combination with the (x,y) weights, 9-shuffle transpose-reduce of
 //    (phi_a, F_x, F_y, F_z), scattered store to the caller's atom order.
 #include <algorithm>
+#include <cstdint>
 #include <type_traits>
 
 #include "kernels_common.cuh"
@@ -140,6 +141,21 @@ __device__ __forceinline__ f32x2 ffma2v(f32x2 a, f32x2 b, f32x2 c) {   // progra
   return d;
 }
 
+// shared-memory accesses by 32-bit shared-space address
+__device__ __forceinline__ float4 lds_f32x4(uint32_t a) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ float lds_f32(uint32_t a) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts_f32(uint32_t a, float v) {
+  asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory");
+}
+
 constexpr int kStage = 32;       // atoms staged per warp at a time (one lane per atom for the output pass)
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -176,8 +192,12 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   // lane -> 2 points of the 8 x 8 (x,y) footprint: y offset c = lane & 7, x offsets b and b + 4
   const int c_off = lane & 7, b0 = lane >> 3;
   int iy = sy + c_off;      if (iy >= My) iy -= My;
-  int ix0 = sx + b0;        if (ix0 >= Mx) ix0 -= Mx;
-  int ix1 = sx + b0 + 4;    if (ix1 >= Mx) ix1 -= Mx;
+  // the lane's two x points are sx + b0 and sx + b0 + 4; "point 0" is the one whose rotated weight index
+  // (x mod 8) has bit 2 clear, so that point 1's weight sits 4 floats further in every record (an immediate)
+  const int xa = sx + b0, xb = sx + b0 + 4;
+  const bool swp = (xa & 4) != 0;
+  int ix0 = swp ? xb : xa;  if (ix0 >= Mx) ix0 -= Mx;
+  int ix1 = swp ? xa : xb;  if (ix1 >= Mx) ix1 -= Mx;
   // loop invariants as shuffle results: ptxas cannot rematerialise those from the constant bank (it
   // re-read Mx, My and cb0 with LDC in every advance / atom otherwise)
   const unsigned plane = __shfl_sync(0xffffffffu, (unsigned)Mx * My, 0), wrap = plane * (unsigned)Mz;
@@ -189,7 +209,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   // samples in profiles/r1c)
   asm volatile("" : "+l"(g0), "+l"(g1));
   // record offsets of this lane's (x,y) weights (records are rotated by the cell index mod 8)
-  const int ox0 = (sx + b0) & 7, ox1 = ox0 ^ 4, oy = SW + ((sy + c_off) & 7);
+  const int ox0 = (sx + b0) & 3, oy = SW + ((sy + c_off) & 7);   // x weights of the lane: ox0 and ox0 + 4
 
   // window registers: channel pairs are held PACKED (one 64-bit register pair = {c, c+1}, exactly as
   // the 16-byte plane loads deliver them), ready to be FFMA2 operands
@@ -245,8 +265,8 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   auto flush = [&](int cnt) {
     __syncwarp();
     if (lane < cnt) {
-      const float4 a = *reinterpret_cast<const float4*>(s_out + 8 * lane);
-      const float4 f = *reinterpret_cast<const float4*>(s_out + 8 * lane + 4);
+      const float4 a = *reinterpret_cast<const float4*>(s_out + 8 * (lane + 1));
+      const float4 f = *reinterpret_cast<const float4*>(s_out + 8 * (lane + 1) + 4);
       const float pv[4] = {a.x, a.y, a.z, a.w};
       if (phi) {
 #pragma unroll
@@ -275,15 +295,20 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   const int out_idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
   // result slot of the pending atom for this lane; the spare row (kStage) when nothing is pending.  Running
   // pointers (records, derivative records, result slot) replace a per-atom multiply-and-add chain each.
-  float* const out_spare = s_out + 8 * kStage + out_idx;
-  float* pend_dst = out_spare;
-  const float* rp = s_rec;                 // record of the next atom (atoms of a segment are one contiguous run)
-  const float* dp = s_drec;
-  float* out_cur = s_out + out_idx;
+  // Result rows: row 0 is a spare, atom t of the staging buffer owns row t + 1; the pending atom's slot is
+  // always the row BEFORE out_cur (the spare when nothing is pending).  Records are read by 32-bit shared
+  // address: two running bases plus lane-constant byte offsets, one add per scalar pair.
+  const uint32_t rec0 = (uint32_t)__cvta_generic_to_shared(s_rec), drec0 = (uint32_t)__cvta_generic_to_shared(s_drec);
+  const uint32_t out0 = (uint32_t)__cvta_generic_to_shared(s_out + 8 + out_idx);
+  uint32_t recB = 4u * (uint32_t)recf;
+  asm volatile("" : "+r"(recB));           // kept in a register (ptxas re-reads kernel parameters in the loop otherwise)
+  const uint32_t cx = 4u * ox0, cy = 4u * oy, cq = 4u * (3 * SW + cb0r);
+  uint32_t ra = rec0, da = drec0;          // record / derivative record of the next atom (one contiguous run per segment)
+  uint32_t out_cur = out0;
   int staged_left = kStage;                // atoms left in the staging buffer
   auto retire = [&]() {
     const float tot = reduce8(pend, lane);
-    if ((lane & 3) == 0) *pend_dst = tot;
+    if ((lane & 3) == 0) sts_f32(out_cur - 32u, tot);
   };
 
   // walk the non-empty cells of the segment; the window advances to each of them in one go
@@ -335,26 +360,25 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
       constexpr int S = decltype(Sc)::value;
         if (staged_left == 0) {   // staging buffer exhausted (dense rows): write results, stage the next atoms
           retire();
-          pend_dst = out_spare;
           flush(kStage);
           js += kStage;
           stage();
           cp_async_wait_all();
           __syncwarp();
-          rp = s_rec; dp = s_drec; out_cur = s_out + out_idx; staged_left = kStage;
+          ra = rec0; da = drec0; out_cur = out0; staged_left = kStage;
         }
-        const float* r = rp;
-        const float* dr = dp;
-        rp += recf; dp += 3 * SW; --staged_left;
-        const float4 za = *reinterpret_cast<const float4*>(r + 2 * SW);
-        const float4 zb = *reinterpret_cast<const float4*>(r + 2 * SW + 4);
-        const float4 da = *reinterpret_cast<const float4*>(dr + 2 * SW);
-        const float4 db = *reinterpret_cast<const float4*>(dr + 2 * SW + 4);
-        const float4 q4 = *reinterpret_cast<const float4*>(r + 3 * SW + cb0r);
-        const float wx0 = r[ox0], wx1 = r[ox1], wy = r[oy];
-        const float dx0 = dr[ox0], dx1 = dr[ox1], dy = dr[oy];
+        --staged_left;
+        const float4 za = lds_f32x4(ra + 4u * 2 * SW);
+        const float4 zb = lds_f32x4(ra + 4u * (2 * SW + 4));
+        const float4 dza = lds_f32x4(da + 4u * 2 * SW);
+        const float4 dzb = lds_f32x4(da + 4u * (2 * SW + 4));
+        const float4 q4 = lds_f32x4(ra + cq);
+        const uint32_t rx = ra + cx, dx = da + cx;
+        const float wx0 = lds_f32(rx), wx1 = lds_f32(rx + 16u), wy = lds_f32(ra + cy);
+        const float dx0 = lds_f32(dx), dx1 = lds_f32(dx + 16u), dy = lds_f32(da + cy);
+        ra += recB; da += 4u * 3 * SW;
         const float wz[SW] = {za.x, za.y, za.z, za.w, zb.x, zb.y, zb.z, zb.w};
-        const float dz[SW] = {da.x, da.y, da.z, da.w, db.x, db.y, db.z, db.w};
+        const float dz[SW] = {dza.x, dza.y, dza.z, dza.w, dzb.x, dzb.y, dzb.z, dzb.w};
         const float qv[4] = {q4.x, q4.y, q4.z, q4.w};
         const float xy[2] = {wx0 * wy, wx1 * wy};      // value and d/dz
         const float dxy[2] = {dx0 * wy, dx1 * wy};     // d/dx
@@ -433,8 +457,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
 #pragma unroll
         for (int c = CB; c < 4; ++c) pend[c] = 0.f;
         pend[4] = fx; pend[5] = fy; pend[6] = fz; pend[7] = 0.f;
-        pend_dst = out_cur;
-        out_cur += 8;
+        out_cur += 32u;   // this atom's row becomes the pending one
   };
   {
   unsigned rem = mask;        // non-empty cells not yet visited
