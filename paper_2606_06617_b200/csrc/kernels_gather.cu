@@ -300,15 +300,21 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   // address: two running bases plus lane-constant byte offsets, one add per scalar pair.
   const uint32_t rec0 = (uint32_t)__cvta_generic_to_shared(s_rec), drec0 = (uint32_t)__cvta_generic_to_shared(s_drec);
   const uint32_t out0 = (uint32_t)__cvta_generic_to_shared(s_out + 8 + out_idx);
-  uint32_t recB = 4u * (uint32_t)recf;
-  asm volatile("" : "+r"(recB));           // kept in a register (ptxas re-reads kernel parameters in the loop otherwise)
+  // Loop invariants that ptxas otherwise re-creates inside the atom loop (the record stride from the kernel
+  // parameters: LDC + LEA per atom; the lane index from SR_TID: an S2R at the head of every atom's shuffle
+  // chain): passed through a volatile shared-memory word, which cannot be rematerialised.
+  __shared__ int s_pin[2][32 * GBX * GBY];
+  s_pin[0][threadIdx.x] = 4 * recf;
+  s_pin[1][threadIdx.x] = lane;
+  const uint32_t recB = (uint32_t) * reinterpret_cast<volatile int*>(&s_pin[0][threadIdx.x]);
+  const int lane_p = *reinterpret_cast<volatile int*>(&s_pin[1][threadIdx.x]);
   const uint32_t cx = 4u * ox0, cy = 4u * oy, cq = 4u * (3 * SW + cb0r);
   uint32_t ra = rec0, da = drec0;          // record / derivative record of the next atom (one contiguous run per segment)
   uint32_t out_cur = out0;
   int staged_left = kStage;                // atoms left in the staging buffer
   auto retire = [&]() {
-    const float tot = reduce8(pend, lane);
-    if ((lane & 3) == 0) sts_f32(out_cur - 32u, tot);
+    const float tot = reduce8(pend, lane_p);
+    if ((lane_p & 3) == 0) sts_f32(out_cur - 32u, tot);
   };
 
   // walk the non-empty cells of the segment; the window advances to each of them in one go
