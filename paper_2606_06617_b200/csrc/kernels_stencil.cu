@@ -740,7 +740,7 @@ void launch_scatter_records(pswf_lr_plan* p, int n, const float* pos, const floa
 void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st) {
   (void)n;
   // 16 x 16 column patches: 4 consumer warps + 1 producer warp, three CTAs per SM (<= 128 registers).
-  // Measured at configuration 4 (round 2): 300 us.  Rejected: 16 x 32 patches x 2 CTAs (113-register cap:
+  // Measured at configuration 4 (end of round 2): 244 us.  Rejected: 16 x 32 patches x 2 CTAs (113-register cap:
   // spills), 16 x 16 x 4 CTAs, 136 registers x 2 CTAs.
   SpreadLaunch<2, 2, 3>::all_channels(p, st);
 }
