@@ -874,6 +874,24 @@ def test_virial_real_space_triclinic_all_components():
     plan.destroy()
 
 
+def test_spread_ranges_spanning_several_patches():
+    """More 16 x 16 column patches than spread CTAs (64 x 256 x 256: 256 patches x 64 planes over 3 x 148 CTAs, so
+    a CTA's range of (patch, plane) pairs runs through two or three patches) and a flat grid where every CTA
+    gets a single cell plane: fast kernels against the reference kernels."""
+    rng = np.random.default_rng(77)
+    for grid, box, N in (([64, 256, 256], [60.0, 240.0, 240.0], 150000), ([16, 128, 128], [16.0, 128.0, 128.0], 30000)):
+        pos = (rng.uniform(0, 1, (N, 3)) * np.asarray(box)).astype(np.float32).astype(np.float64)
+        q = rng.normal(0, 0.5, (2, N)).astype(np.float32).astype(np.float64)
+        wl = dict(pos=pos, q=q, exponents=[1, 6], box=box, grid=grid, w=8, c=12.024, precision="f32")
+        a = run_gpu(wl, kernel_path=0)
+        b = run_gpu(wl, kernel_path=1)
+        assert a["info"]["fast_stencil"] == 1
+        assert abs(a["E"] - b["E"]) <= 2e-5 * abs(b["E"]), grid
+        assert rel(a["phi"], b["phi"]) <= 5e-5, grid
+        assert rel(a["F"], b["F"]) <= 5e-5, grid
+        assert np.abs(a["F"] - b["F"]).max() <= 8 * 5e-5 * np.abs(b["F"]).max(), grid
+
+
 def test_random_configurations_fast_path_consistent_with_reference_kernels():
     """Consistency, not a parity claim: twelve seeded random configurations (grids, densities, channel
     counts, widths; uniform, tightly clustered and slab-shaped systems, the clustered ones drive the
