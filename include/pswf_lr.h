@@ -89,7 +89,7 @@ typedef struct {
   int fast_stencil;      /* 1: the cell-sorted fp32 spread / gather kernels run (fp32, w <= 8, M_d a     */
                          /*    multiple of 8 and >= 16, kernel_path = 0); 0: the one-warp-per-atom ones  */
   int band_limited_fft;  /* 1: z transforms + fused (x,y) transform / scale kernel (fp32, Mx and My      */
-                         /*    powers of two <= 256, kernel_path = 0, virial off); 0: dense 3-D cuFFT    */
+                         /*    powers of two <= 256, kernel_path = 0); 0: dense 3-D cuFFT                 */
   int band_kmax[3];      /* band-limited path: kept DFT indices |m_d| <= band_kmax[d]                    */
   long long own_kernel_launches; /* kernels of this library launched by the plan since creation (counted  */
   long long memsets;             /* at the launch sites), cudaMemsetAsync calls, and cuFFT executions      */

@@ -16,7 +16,8 @@
 //   * cuFFT C2R along z reads a second plane-major buffer whose planes beyond the band are zero from
 //     plan creation on and are never written.
 // Requirements (host-checked; otherwise the dense path runs): fp32, Mx and My powers of two in
-// 8..256 with the padded plane fitting shared memory, no virial accumulation.
+// 8..256 with the padded plane fitting shared memory.  With pswf_lr_set_virial the same pass accumulates the
+// virial of the reciprocal energy (VIR variants).
 #include <algorithm>
 #include <cmath>
 
@@ -182,10 +183,38 @@ __device__ __forceinline__ int freq_of_pos(int pos, int N, int nr, const int* ra
 
 // grid = (kept k_z planes, channels).  spec_in / spec_out: plane-major [kz][c][x][y] complex.
 // DUMP: also write the scaled modes in the dense layout [c][kx][ky][kz] (test hook).
-template <bool DUMP>
+// Virial of one mode, as in k_scale: W_ab += e delta_ab + herm |rho^|^2 (dD/dk / |k|) k_a k_b
+// with e = herm D |rho^|^2 (the factor 1/2 is applied with the final reduction).
+__device__ __forceinline__ void virial_of_mode(double (&w)[6], double e, double g, float kx, float ky, float kz,
+                                               bool zero_mode) {
+  w[0] += e; w[1] += e; w[2] += e;
+  if (!zero_mode) {
+    w[0] += g * kx * kx; w[1] += g * ky * ky; w[2] += g * kz * kz;
+    w[3] += g * kx * ky; w[4] += g * kx * kz; w[5] += g * ky * kz;
+  }
+}
+// block sums of the six components -> Wacc (one atomicAdd per component and CTA); s_red: one double per warp
+__device__ __forceinline__ void virial_reduce(const double (&w)[6], double* s_red, double* Wacc) {
+  const int tid = threadIdx.x;
+#pragma unroll 1
+  for (int i = 0; i < 6; ++i) {
+    __syncthreads();
+    const double t = warp_sum(w[i]);
+    if ((tid & 31) == 0) s_red[tid >> 5] = t;
+    __syncthreads();
+    if (tid < 32) {
+      double u = tid < (int)(blockDim.x >> 5) ? s_red[tid] : 0.0;
+      u = warp_sum(u);
+      if (tid == 0 && u != 0.0) atomicAdd(&Wacc[i], 0.5 * u);
+    }
+  }
+}
+
+template <bool DUMP, bool VIR>
 __global__ void __launch_bounds__(kXYThreads, 1)
     k_xy_scale(const XYParams X, const ScaleParams<float> P, const float2* __restrict__ spec_in,
-               float2* __restrict__ spec_out, double* __restrict__ Ech, float2* __restrict__ dump) {
+               float2* __restrict__ spec_out, double* __restrict__ Ech, float2* __restrict__ dump,
+               double* __restrict__ Wacc) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* s = reinterpret_cast<float2*>(smem_raw);                 // [Mx][pitch]
   float2* twx = s + (size_t)X.Mx * X.pitch;                        // [Mx]  exp(-2 pi i k / Mx)
@@ -241,6 +270,7 @@ __global__ void __launch_bounds__(kXYThreads, 1)
   const float wz = P.invW2[2][kz];
   const float herm = kz == 0 ? 1.f : 2.f;
   double e = 0.0;
+  double wloc[6] = {0, 0, 0, 0, 0, 0};
   for (int it = tid; it < nkx * My; it += kXYThreads) {
     const int a = it / My, py = it - a * My;
     const int px = keptx[a];
@@ -256,10 +286,16 @@ __global__ void __launch_bounds__(kXYThreads, 1)
       const bool zero_mode = (ix | iy | kz) == 0;
       if (zero_mode || x < 1.f) {
         float d;
+        const float wgt = P.base * P.invW2[0][ix] * P.invW2[1][iy] * wz;
         if (zero_mode) d = P.chan_D0[c];
-        else d = P.base * P.invW2[0][ix] * P.invW2[1][iy] * wz * kernel_value(P, slot, x, x * P.c);
+        else d = wgt * kernel_value(P, slot, x, x * P.c);
         v = s[px * pitch + py];
-        e += (double)(herm * (v.x * v.x + v.y * v.y) * d);
+        const float a2 = herm * (v.x * v.x + v.y * v.y);
+        e += (double)(a2 * d);
+        if (VIR) {
+          const double g = zero_mode ? 0.0 : (double)(a2 * (wgt * kernel_dvalue(P, slot, x, x * P.c) / kn));
+          virial_of_mode(wloc, (double)(a2 * d), g, kx, ky, kzv, zero_mode);
+        }
         v.x *= d;
         v.y *= d;
         if (DUMP) dump[(((size_t)c * Mx + ix) * My + iy) * X.Mzh + kz] = v;
@@ -293,6 +329,7 @@ __global__ void __launch_bounds__(kXYThreads, 1)
     t = warp_sum(t);
     if (tid == 0 && t != 0.0) atomicAdd(&Ech[c], 0.5 * t);
   }
+  if (VIR) virial_reduce(wloc, s_red, Wacc);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -375,10 +412,11 @@ __device__ __forceinline__ int freq_of_pos_t(int pos) {
 }
 
 // Same kernel as k_xy_scale with Mx = My = M fixed at compile time.
-template <int M, bool DUMP>
+template <int M, bool DUMP, bool VIR>
 __global__ void __launch_bounds__(kXYThreads, 1)
     k_xy_scale_t(const XYParams X, const ScaleParams<float> P, const float2* __restrict__ spec_in,
-                 float2* __restrict__ spec_out, double* __restrict__ Ech, float2* __restrict__ dump) {
+                 float2* __restrict__ spec_out, double* __restrict__ Ech, float2* __restrict__ dump,
+                 double* __restrict__ Wacc) {
   constexpr int pitch = M + 1, NT = kXYThreads, LG = ilog2(M);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* s = reinterpret_cast<float2*>(smem_raw);                 // [M][pitch]
@@ -431,6 +469,7 @@ __global__ void __launch_bounds__(kXYThreads, 1)
   const float wz = P.invW2[2][kz];
   const float herm = kz == 0 ? 1.f : 2.f;
   double e = 0.0;
+  double wloc[6] = {0, 0, 0, 0, 0, 0};
   for (int it = tid; it < (nkx << LG); it += NT) {
     const int a = it >> LG, py = it & (M - 1);
     const int px = keptx[a];
@@ -446,10 +485,16 @@ __global__ void __launch_bounds__(kXYThreads, 1)
       const bool zero_mode = (ix | iy | kz) == 0;
       if (zero_mode || x < 1.f) {
         float d;
+        const float wgt = P.base * P.invW2[0][ix] * P.invW2[1][iy] * wz;
         if (zero_mode) d = P.chan_D0[c];
-        else d = P.base * P.invW2[0][ix] * P.invW2[1][iy] * wz * kernel_value(P, slot, x, x * P.c);
+        else d = wgt * kernel_value(P, slot, x, x * P.c);
         v = s[px * pitch + py];
-        e += (double)(herm * (v.x * v.x + v.y * v.y) * d);
+        const float a2 = herm * (v.x * v.x + v.y * v.y);
+        e += (double)(a2 * d);
+        if (VIR) {
+          const double g = zero_mode ? 0.0 : (double)(a2 * (wgt * kernel_dvalue(P, slot, x, x * P.c) / kn));
+          virial_of_mode(wloc, (double)(a2 * d), g, kx, ky, kzv, zero_mode);
+        }
         v.x *= d;
         v.y *= d;
         if (DUMP) dump[(((size_t)c * M + ix) * M + iy) * X.Mzh + kz] = v;
@@ -482,6 +527,7 @@ __global__ void __launch_bounds__(kXYThreads, 1)
     t = warp_sum(t);
     if (tid == 0 && t != 0.0) atomicAdd(&Ech[c], 0.5 * t);
   }
+  if (VIR) virial_reduce(wloc, s_red, Wacc);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -689,6 +735,7 @@ void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t 
   const size_t sm = xy_smem_bytes(X.Mx, X.My);
   const dim3 grid((unsigned)(p->fused_kmax[2] + 1), (unsigned)p->C);
   p->n_kernels += 1;
+  double* wacc = p->virial ? p->d_virial : nullptr;   // zeroed by the caller before the launch
   float2* dump = nullptr;
   if (p->debug_dump_spectrum) {
     const size_t Mhalf = (size_t)p->M[0] * p->M[1] * X.Mzh;
@@ -698,12 +745,16 @@ void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t 
 #define PSWF_XY(KERN)                                                                                        \
   do {                                                                                                       \
     cudaFuncSetAttribute(KERN, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);                        \
-    KERN<<<grid, kXYThreads, sm, st>>>(X, P, (const float2*)p->d_spec, (float2*)p->d_spec2, p->d_Ech, dump); \
+    KERN<<<grid, kXYThreads, sm, st>>>(X, P, (const float2*)p->d_spec, (float2*)p->d_spec2, p->d_Ech, dump, \
+                                       wacc);                                                                \
   } while (0)
-#define PSWF_XY_SQ(MV)                                        \
-  case MV:                                                    \
-    if (dump) PSWF_XY((k_xy_scale_t<MV, true>));              \
-    else PSWF_XY((k_xy_scale_t<MV, false>));                  \
+#define PSWF_XY_SQ(MV)                                                  \
+  case MV:                                                              \
+    if (wacc) {  /* virial: accumulated in the same pass */             \
+      if (dump) PSWF_XY((k_xy_scale_t<MV, true, true>));                \
+      else PSWF_XY((k_xy_scale_t<MV, false, true>));                    \
+    } else if (dump) PSWF_XY((k_xy_scale_t<MV, true, false>));          \
+    else PSWF_XY((k_xy_scale_t<MV, false, false>));                     \
     return;
   if (X.Mx == X.My) {
     switch (X.Mx) {
@@ -711,8 +762,11 @@ void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t 
       default: break;
     }
   }
-  if (dump) PSWF_XY(k_xy_scale<true>);
-  else PSWF_XY(k_xy_scale<false>);
+  if (wacc) {
+    if (dump) PSWF_XY((k_xy_scale<true, true>));
+    else PSWF_XY((k_xy_scale<false, true>));
+  } else if (dump) PSWF_XY((k_xy_scale<true, false>));
+  else PSWF_XY((k_xy_scale<false, false>));
 #undef PSWF_XY_SQ
 #undef PSWF_XY
 }

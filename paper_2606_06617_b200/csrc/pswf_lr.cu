@@ -221,7 +221,7 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   if (ev) cudaEventRecord(ev[2], st);
   // a2-a4.  Band-limited path: R2C along z (plane-major spectrum), then per kept (k_z, channel) plane
   // forward (x,y) transform, multiply + energy, inverse (x,y) transform in one kernel, then C2R along z.
-  const bool fused = kIsF32 && p->fused_fft && !p->virial;
+  const bool fused = kIsF32 && p->fused_fft;
   if (fused) {
     if (p->fused_z) {
       launch_z_forward(p, st);
@@ -905,7 +905,7 @@ int pswf_lr_get_info(const pswf_lr_plan* p, pswf_lr_info* info) {
   info->modes_in_ball = p->modes_in_ball;
   info->workspace_bytes = p->workspace_bytes;
   info->fast_stencil = (!p->host_only && p->kernel_path == 0 && stencil_path_supported(p)) ? 1 : 0;
-  info->band_limited_fft = (p->fused_fft && !p->virial) ? 1 : 0;
+  info->band_limited_fft = p->fused_fft ? 1 : 0;
   for (int d = 0; d < 3; ++d) info->band_kmax[d] = p->fused_kmax[d];
   info->own_kernel_launches = p->n_kernels;
   info->memsets = p->n_memsets;
@@ -960,7 +960,7 @@ int pswf_lr_debug_copy(pswf_lr_plan* p, int what, void* dst, void* stream) {
     nb = rs * Mtot * p->C;
   } else if (what == 1) {
     src = p->d_spec;
-    if (p->fused_fft && !p->virial) {   // the band-limited path keeps the dense spectrum only on request
+    if (p->fused_fft) {   // the band-limited path keeps the dense spectrum only on request
       if (!p->d_spec_dump) return PSWF_LR_ERR_INVALID_ARG;
       src = p->d_spec_dump;
     }

@@ -814,6 +814,30 @@ def test_virial_triclinic_all_components_vs_oracle():
         plan.destroy()
 
 
+@pytest.mark.parametrize("grid", [[32, 32, 32], [16, 64, 32], [32, 32, 24]])
+def test_virial_band_limited_path_vs_oracle_and_dense_path(grid):
+    """The virial accumulated inside the fused (x,y) transform / multiply kernel (fp32, band-limited path; the
+    last grid has a non-power-of-two M_z: cuFFT along z): against the oracle's k-sum virial at the fp32 force
+    gate, and against the dense path (reference kernels + k_scale), in a triclinic cell (all six components)."""
+    from oracle.direct import virial_direct
+    wl = _triclinic_workload(500, grid, 8, "f32", seed=93)
+    res = {}
+    for path in (0, 1):
+        plan = make_plan(wl, kernel_path=path)
+        plan.set_virial(True)
+        out = run_gpu(wl, plan=plan)
+        res[path] = (_virial(plan), out["info"]["band_limited_fft"], out["E"], plan.info()["r_c"])
+        plan.destroy()
+    assert res[0][1] == 1 and res[1][1] == 0
+    W_ref = virial_direct(wl["pos"], wl["q"], wl["exponents"], wl["box"], wl["c"], res[0][3], grid=wl["grid"])
+    scale = np.abs(W_ref).max()
+    print("virial fused %s: vs oracle %.2e, vs dense path %.2e" % (grid, np.abs(res[0][0] - W_ref).max() / scale,
+                                                                 np.abs(res[0][0] - res[1][0]).max() / scale))
+    assert np.abs(res[0][0] - W_ref).max() <= 1e-4 * scale
+    assert np.abs(res[0][0] - res[1][0]).max() <= 2e-5 * scale
+    assert abs(res[0][2] - res[1][2]) <= 2e-5 * abs(res[1][2])
+
+
 def test_virial_real_space_vs_strain_derivative_of_scaffold():
     """The pair virial of pswf_lr_execute_real: diagonal = -dE/d(eps_aa) of the scaffold's real-space
     energy by central differences under a homogeneous strain (fp64); symmetric; and execute +
