@@ -131,7 +131,8 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
  * CUDA graph on the second call and replayed afterwards; calls made while `stream` is itself being captured
  * launch plainly into the caller's capture.
  * Outputs are in the caller's atom order.  If phi and F are both NULL the inverse FFT and the
- * gather are skipped (the paper's energy-only path).  n_atoms = 0 is legal. */
+ * gather are skipped (the paper's energy-only path); with phi NULL and F given (an MD
+ * step) the gather runs without the potential sums.  n_atoms = 0 is legal. */
 int pswf_lr_execute(pswf_lr_plan* plan, int n_atoms, const void* pos, const void* q, void* E,
                     void* phi, void* F, void* stream);
 

@@ -117,6 +117,28 @@ __device__ __forceinline__ float reduce8(float (&v)[8], int lane) {
   return v[0];
 }
 
+// The same for 4 values (forces only: the potentials were not asked for): 6 shuffles; on return lane l holds
+// in v[0] the full sum of input index ((l >> 4) & 1) * 2 + ((l >> 3) & 1).
+__device__ __forceinline__ float reduce4(float (&v)[8], int lane) {
+  const bool hi16 = lane & 16;
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const float send = hi16 ? v[i] : v[i + 2];
+    const float keep = hi16 ? v[i + 2] : v[i];
+    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+  }
+  const bool hi8 = lane & 8;
+  {
+    const float send = hi8 ? v[0] : v[1];
+    const float keep = hi8 ? v[1] : v[0];
+    v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+  }
+  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 4);
+  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 2);
+  v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+  return v[0];
+}
+
 // Packed FP32 pairs (sm_100a FFMA2: one instruction, two IEEE fused multiply-adds per lane; ptxas
 // uses its broadcast-scalar operand form for pack2(w, w)).  The gather is issue-bound, not
 // FMA-pipe-bound: pairing adjacent channels halves the FMA instruction count of the contraction.
@@ -169,7 +191,9 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // (+ one spare result row: the sink of the software-pipelined reduction when nothing is pending)
 __host__ __device__ constexpr int gather_warp_floats(int recf) { return kStage * (recf + 3 * SW + 8) + 8; }
 
-template <int CB, int GBX, int GBY, int NCTA>   // GBX x GBY cell rows (warps) per CTA, NCTA resident CTAs per SM
+// PHI = false: the caller passed phi == NULL (an MD step needs E and F only): no potential sums, a 4-value
+// reduction instead of the 8-value one.
+template <int CB, int GBX, int GBY, int NCTA, bool PHI>   // GBX x GBY cell rows (warps) per CTA, NCTA resident CTAs per SM
 __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
     k_gather_rows(int n, int C, int cb0, int Mx, int My, int Mz, int nseg, int nbx, int nby, int recf,
                   const int* __restrict__ start, const float* __restrict__ rec, const float* __restrict__ drec,
@@ -268,7 +292,7 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
       const float4 a = *reinterpret_cast<const float4*>(s_out + 8 * (lane + 1));
       const float4 f = *reinterpret_cast<const float4*>(s_out + 8 * (lane + 1) + 4);
       const float pv[4] = {a.x, a.y, a.z, a.w};
-      if (phi) {
+      if constexpr (PHI) {
 #pragma unroll
         for (int c = 0; c < CB; ++c)
           if (cb0 + c < C) phi[(size_t)(cb0 + c) * n + perm_l] = pv[c];
@@ -292,7 +316,8 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
 #pragma unroll
   for (int i = 0; i < 8; ++i) pend[i] = 0.f;
   // lane l with (l & 3) == 0 ends up with output index (l>>4)*4 + ((l>>3)&1)*2 + ((l>>2)&1)
-  const int out_idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+  const int out_idx = PHI ? ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1)
+                          : 4 + ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);   // forces live in floats 4..6 of a result row
   // result slot of the pending atom for this lane; the spare row (kStage) when nothing is pending.  Running
   // pointers (records, derivative records, result slot) replace a per-atom multiply-and-add chain each.
   // Result rows: row 0 is a spare, atom t of the staging buffer owns row t + 1; the pending atom's slot is
@@ -313,8 +338,13 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
   uint32_t out_cur = out0;
   int staged_left = kStage;                // atoms left in the staging buffer
   auto retire = [&]() {
-    const float tot = reduce8(pend, lane_p);
-    if ((lane_p & 3) == 0) sts_f32(out_cur - 32u, tot);
+    if constexpr (PHI) {
+      const float tot = reduce8(pend, lane_p);
+      if ((lane_p & 3) == 0) sts_f32(out_cur - 32u, tot);
+    } else {
+      const float tot = reduce4(pend, lane_p);
+      if ((lane_p & 7) == 0) sts_f32(out_cur - 32u, tot);
+    }
   };
 
   // walk the non-empty cells of the segment; the window advances to each of them in one go
@@ -433,13 +463,15 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
           const f32x2 xy0 = pack2(xy[0], xy[0]), xy1 = pack2(xy[1], xy[1]);
 #pragma unroll
           for (int h = 0; h < NP; ++h) {
-            const f32x2 val = ffma2(S01[h], xy1, ffma2(S00[h], xy0, 0ull));
             const f32x2 q2 = pack2(qv[2 * h], qv[2 * h + 1]);
             T00 = ffma2(q2, S00[h], T00);
             T01 = ffma2(q2, S01[h], T01);
             T10 = ffma2(q2, S10[h], T10);
             T11 = ffma2(q2, S11[h], T11);
-            unpack2(val, pend[2 * h], pend[2 * h + 1]);
+            if constexpr (PHI) {
+              const f32x2 val = ffma2(S01[h], xy1, ffma2(S00[h], xy0, 0ull));
+              unpack2(val, pend[2 * h], pend[2 * h + 1]);
+            }
           }
           float a, b;
           unpack2(T00, a, b); const float t00 = a + b;
@@ -471,12 +503,16 @@ __global__ void __launch_bounds__(32 * GBX * GBY, NCTA)
           fx = fmaf(qc, gx, fx);
           fy = fmaf(qc, gy, fy);
           fz = fmaf(qc, gz, fz);
-          pend[c] = val;
+          if constexpr (PHI) pend[c] = val;
         }
         }
+        if constexpr (PHI) {
 #pragma unroll
-        for (int c = CB; c < 4; ++c) pend[c] = 0.f;
-        pend[4] = fx; pend[5] = fy; pend[6] = fz; pend[7] = 0.f;
+          for (int c = CB; c < 4; ++c) pend[c] = 0.f;
+          pend[4] = fx; pend[5] = fy; pend[6] = fz; pend[7] = 0.f;
+        } else {
+          pend[0] = fx; pend[1] = fy; pend[2] = fz; pend[3] = 0.f;
+        }
         out_cur += 32u;   // this atom's row becomes the pending one
   };
   {
@@ -542,7 +578,7 @@ void launch_fast_gather_t(pswf_lr_plan* p, int n, float* phi, float* F, bool hav
     using V = typename VecOf<CBV>::type;                                                                    \
     p->n_kernels += have_il ? 1 : 2;                                                                        \
     if (!have_il) k_interleave_t<CBV><<<iblocks, 256, 0, st>>>(Mx, My, Mz, NCH, planar, (V*)gi);            \
-    auto kern = k_gather_rows<CBV, GBX, GBY, NCTAV>;                                                         \
+    auto kern = phi ? k_gather_rows<CBV, GBX, GBY, NCTAV, true> : k_gather_rows<CBV, GBX, GBY, NCTAV, false>; \
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                     \
     kern<<<blocks, 32 * GBX * GBY, smem, st>>>(n, p->C, cb0, Mx, My, Mz, nseg, nbx, nby, recf, p->d_count,        \
                                                (const float*)p->d_rec, (const float*)p->d_drec, p->d_perm,  \

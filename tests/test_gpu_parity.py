@@ -898,6 +898,21 @@ def test_virial_real_space_triclinic_all_components():
     plan.destroy()
 
 
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_forces_only_call_equals_full_call(cfg):
+    """phi == NULL selects the gather variant without potential sums (4-value reduction): same E and F as
+    the full call (different summation order only); 1, 2 and 4 channels per gather pass."""
+    wl = workloads.make(cfg)
+    full = run_gpu(wl)
+    fo = run_gpu(wl, want=("E", "F"))
+    assert abs(full["E"] - fo["E"]) <= 1e-6 * abs(full["E"])
+    assert rel(fo["F"], full["F"]) <= 2e-6
+    assert np.abs(fo["F"] - full["F"]).max() <= 2e-5 * np.abs(full["F"]).max()
+    one = dict(wl, q=wl["q"][:1], exponents=wl["exponents"][:1])
+    a, b = run_gpu(one), run_gpu(one, want=("E", "F"))
+    assert rel(b["F"], a["F"]) <= 2e-6
+
+
 def test_spread_ranges_spanning_several_patches():
     """More 16 x 16 column patches than spread CTAs (64 x 256 x 256: 256 patches x 64 planes over 3 x 148 CTAs, so
     a CTA's range of (patch, plane) pairs runs through two or three patches) and a flat grid where every CTA
