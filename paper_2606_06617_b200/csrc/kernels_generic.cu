@@ -403,14 +403,15 @@ __global__ void k_gather_ref(int n, int C, int cap, GridGeom<T> g, const int* __
 // ------------------------------------------------------------------------------------------------
 template <class T>
 void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, bool scatter,
-                     cudaStream_t st) {
+                     bool zero_energy, cudaStream_t st) {
   const int Mtot = p->M[0] * p->M[1] * p->M[2];
-  cudaMemsetAsync(p->d_count, 0, sizeof(int) * ((size_t)Mtot + 1), st);
-  p->n_memsets += 2;
+  // one memset: cell counts + scan state (+ the energy and virial accumulators in front of them, plan.hpp)
+  const size_t off = zero_energy ? 0 : p->zero_sort_offset;
+  cudaMemsetAsync((char*)p->d_zero_block + off, 0, p->zero_block_bytes - off, st);
+  p->n_memsets += 1;
   p->n_kernels += (n > 0 ? 1 : 0) + 1 + ((n > 0 && scatter) ? 1 : 0);
   if (n > 0)
     k_bin_count<T><<<(n + 255) / 256, 256, 0, st>>>(n, pos, g, p->d_count, p->d_key, p->d_rank);
-  cudaMemsetAsync(p->d_scan_state, 0, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), st);
   k_scan_lookback<<<p->n_scan_blocks, kScanThreads, 0, st>>>(Mtot, p->d_count, p->d_scan_state, Mtot, n);
   if (n > 0 && scatter)
     k_scatter<T><<<(n + 255) / 256, 256, 0, st>>>(n, p->C, p->cap_atoms, pos, q, g, p->d_count, p->d_key,
@@ -455,7 +456,7 @@ void launch_gather_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, T* phi, T* 
 }
 
 #define PSWF_INSTANTIATE(T)                                                                               \
-  template void launch_bin_sort<T>(pswf_lr_plan*, int, const T*, const T*, const GridGeom<T>&, bool, cudaStream_t); \
+  template void launch_bin_sort<T>(pswf_lr_plan*, int, const T*, const T*, const GridGeom<T>&, bool, bool, cudaStream_t); \
   template void launch_spread_ref<T>(pswf_lr_plan*, int, const GridGeom<T>&, cudaStream_t);              \
   template void launch_scale<T>(pswf_lr_plan*, const ScaleParams<T>&, bool, cudaStream_t);               \
   template void launch_gather_ref<T>(pswf_lr_plan*, int, const GridGeom<T>&, T*, T*, cudaStream_t);

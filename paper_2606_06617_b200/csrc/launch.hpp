@@ -6,7 +6,7 @@ namespace pswf {
 
 template <class T>
 void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, bool scatter,
-                     cudaStream_t st);
+                     bool zero_energy, cudaStream_t st);
 int scan_tile_size();   // counts per tile of the single-pass scan (sizes its state array)
 int launch_scan_static(int* data, int n, cudaStream_t st);   // 1 <= n <= PSWF_LR_SCAN_STATIC_MAX; no allocation
 template <class T>

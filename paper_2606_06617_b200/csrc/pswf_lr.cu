@@ -208,7 +208,7 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
     ev = p->events.data() + (size_t)p->prof_count * (PSWF_LR_N_STAGES + 1);
   if (ev) cudaEventRecord(ev[0], st);
   // a0
-  launch_bin_sort<T>(p, n, pos, q, g, !stencil, st);
+  launch_bin_sort<T>(p, n, pos, q, g, !stencil, true, st);   // (zeroes the energy / virial accumulators too)
   if constexpr (kIsF32) {
     if (stencil) launch_scatter_records(p, n, pos, q, g, st);
   }
@@ -240,9 +240,7 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   }
   if (ev) cudaEventRecord(ev[3], st);
   // a3
-  cudaMemsetAsync(p->d_Ech, 0, sizeof(double) * p->C, st);
-  if (p->virial) cudaMemsetAsync(p->d_virial, 0, sizeof(double) * 6, st);
-  p->n_memsets += p->virial ? 2 : 1;
+  // (d_Ech and d_virial were zeroed with the sort's buffers at the start of the evaluation)
   if constexpr (kIsF32) {
     if (fused) launch_xy_scale(p, P, st);
   }
@@ -296,7 +294,7 @@ template <class T>
 int execute_real_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* phi, T* F, int accumulate,
                    cudaStream_t st) {
   GridGeom<T> g = make_geom<T>(p);
-  launch_bin_sort<T>(p, n, pos, q, g, true, st);   // generic sort: perm, si0, sq
+  launch_bin_sort<T>(p, n, pos, q, g, true, false, st);   // generic sort: perm, si0, sq
   RealGeom<T> rg;
   RealParams<T> P;
   memset(&P, 0, sizeof(P));
@@ -566,12 +564,24 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
       if (!rc) rc = dev_alloc(&p->d_grid, rs * Mtot * p->C, &b);
       if (!rc) rc = dev_alloc(&p->d_spec, 2 * rs * Mhalf * p->C, &b);
       if (!rc && stencil_path_supported(p)) rc = dev_alloc(&p->d_gridi, gather_grid_bytes(p), &b);
-      if (!rc) rc = dev_alloc((void**)&p->d_count, sizeof(int) * (Mtot + 1), &b);
       p->n_scan_blocks = (int)((Mtot + scan_tile_size() - 1) / scan_tile_size());
-      if (!rc) rc = dev_alloc((void**)&p->d_scan_state, sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1), &b);
-      if (!rc) rc = dev_alloc((void**)&p->d_Ech, sizeof(double) * kMaxChannels, &b);
+      {
+        // everything an evaluation starts from zero, in one block (one memset node instead of three or four)
+        const size_t bE = sizeof(double) * kMaxChannels, bW = sizeof(double) * 8;   // (6 used; keeps 16-byte alignment)
+        const size_t bS = (sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1) + 15) & ~(size_t)15;
+        const size_t bC = sizeof(int) * (Mtot + 1);
+        p->zero_sort_offset = bE + bW;
+        p->zero_block_bytes = bE + bW + bS + bC;
+        if (!rc) rc = dev_alloc(&p->d_zero_block, p->zero_block_bytes, &b);
+        if (!rc) {
+          char* base = (char*)p->d_zero_block;
+          p->d_Ech = (double*)base;
+          p->d_virial = (double*)(base + bE);
+          p->d_scan_state = (unsigned long long*)(base + bE + bW);
+          p->d_count = (int*)(base + bE + bW + bS);
+        }
+      }
       if (!rc) rc = dev_alloc((void**)&p->d_Ereal, sizeof(double), &b);
-      if (!rc) rc = dev_alloc((void**)&p->d_virial, sizeof(double) * 6, &b);
       p->workspace_bytes += b;
     }
     if (!rc && !p->host_only) {
@@ -1093,8 +1103,8 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   if (p->s_comp) cudaStreamDestroy(p->s_comp);
   if (p->s_out) cudaStreamDestroy(p->s_out);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
-                  p->d_grid,  p->d_spec,    p->d_count,    p->d_scan_state, p->d_Ech,
-                  p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal, p->d_virial, p->d_spec2, p->d_spec_dump};
+                  p->d_grid,  p->d_spec,    p->d_zero_block,    
+                  p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal, p->d_spec2, p->d_spec_dump};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   if (p->have_fft) {
