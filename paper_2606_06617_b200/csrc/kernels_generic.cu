@@ -405,9 +405,10 @@ template <class T>
 void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const GridGeom<T>& g, bool scatter,
                      bool zero_energy, cudaStream_t st) {
   const int Mtot = p->M[0] * p->M[1] * p->M[2];
-  // one memset: cell counts + scan state (+ the energy and virial accumulators in front of them, plan.hpp)
-  const size_t off = zero_energy ? 0 : p->zero_sort_offset;
-  cudaMemsetAsync((char*)p->d_zero_block + off, 0, p->zero_block_bytes - off, st);
+  // one memset: cell counts + scan state (an evaluation: also the energy / virial accumulators in front of them
+  // and the charge grid behind them, plan.hpp)
+  if (zero_energy) cudaMemsetAsync(p->d_zero_block, 0, p->zero_block_bytes, st);
+  else cudaMemsetAsync((char*)p->d_zero_block + p->zero_sort_offset, 0, p->zero_sort_bytes, st);
   p->n_memsets += 1;
   p->n_kernels += (n > 0 ? 1 : 0) + 1 + ((n > 0 && scatter) ? 1 : 0);
   if (n > 0)
@@ -421,9 +422,7 @@ void launch_bin_sort(pswf_lr_plan* p, int n, const T* pos, const T* q, const Gri
 
 template <class T>
 void launch_spread_ref(pswf_lr_plan* p, int n, const GridGeom<T>& g, cudaStream_t st) {
-  const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
-  cudaMemsetAsync(p->d_grid, 0, sizeof(T) * Mtot * p->C, st);
-  p->n_memsets += 1;
+  // (the grid was zeroed with the sort's buffers at the start of the evaluation, launch_bin_sort)
   p->n_kernels += n > 0 ? 1 : 0;
   if (n > 0)
     k_spread_ref<T><<<(n + 7) / 8, 256, 0, st>>>(n, p->C, p->cap_atoms, g, p->d_si0, (const T*)p->d_sdelta,

@@ -680,9 +680,8 @@ struct SpreadLaunch {
     // chain of ~2.5 us each (42 -> 15 us at configuration 2 against 8 planes per CTA).
     const int npatch = ((p->M[1] + S::TY - 1) / S::TY) * ((p->M[2] + S::TZ - 1) / S::TZ);
     const int nseg = std::max(1, std::min(NCTA * p->sm_count, npatch * p->M[0]));
-    const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
-    cudaMemsetAsync(p->d_grid, 0, sizeof(float) * Mtot * p->C, st);   // the RED-merged planes start from zero
-    p->n_memsets += 1;
+    // (the RED-merged planes start from zero: the grid is zeroed with the sort's buffers at the start of the
+    // evaluation, launch_bin_sort)
     int cb0 = 0;
     while (cb0 < p->C) {
       const int left = p->C - cb0;

@@ -132,10 +132,11 @@ struct pswf_lr_plan {
   int* d_count = nullptr;         // [Mtot + 1] cell counts -> exclusive starts
   unsigned long long* d_scan_state = nullptr;   // [1 + n_scan_blocks] ticket counter + tile states of the scan
   int n_scan_blocks = 0;
-  // One allocation, zero-filled by ONE memset per evaluation: [d_Ech | d_virial | d_scan_state | d_count] (the
-  // sort of pswf_lr_execute_real zeroes the last two only: the energies of the preceding execute stay readable)
+  // One allocation, zero-filled by ONE memset per evaluation: [d_Ech | d_virial | d_scan_state | d_count | d_grid]
+  // (the sort of pswf_lr_execute_real zeroes d_scan_state and d_count only: the energies and the potential grid
+  // of the preceding execute stay readable)
   void* d_zero_block = nullptr;
-  size_t zero_block_bytes = 0, zero_sort_offset = 0;
+  size_t zero_block_bytes = 0, zero_sort_offset = 0, zero_sort_bytes = 0;
   double* d_Ech = nullptr;        // [C]
   // per-atom workspaces (capacity cap_atoms)
   int cap_atoms = 0;

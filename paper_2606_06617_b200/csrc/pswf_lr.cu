@@ -561,7 +561,6 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
       const size_t rs = real_size(p);
       const size_t Mtot = (size_t)p->M[0] * p->M[1] * p->M[2];
       const size_t Mhalf = (size_t)p->M[0] * p->M[1] * (p->M[2] / 2 + 1);
-      if (!rc) rc = dev_alloc(&p->d_grid, rs * Mtot * p->C, &b);
       if (!rc) rc = dev_alloc(&p->d_spec, 2 * rs * Mhalf * p->C, &b);
       if (!rc && stencil_path_supported(p)) rc = dev_alloc(&p->d_gridi, gather_grid_bytes(p), &b);
       p->n_scan_blocks = (int)((Mtot + scan_tile_size() - 1) / scan_tile_size());
@@ -569,9 +568,11 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
         // everything an evaluation starts from zero, in one block (one memset node instead of three or four)
         const size_t bE = sizeof(double) * kMaxChannels, bW = sizeof(double) * 8;   // (6 used; keeps 16-byte alignment)
         const size_t bS = (sizeof(unsigned long long) * ((size_t)p->n_scan_blocks + 1) + 15) & ~(size_t)15;
-        const size_t bC = sizeof(int) * (Mtot + 1);
+        const size_t bC = (sizeof(int) * (Mtot + 1) + 255) & ~(size_t)255;
+        const size_t bG = rs * Mtot * p->C;                                          // the charge grid
         p->zero_sort_offset = bE + bW;
-        p->zero_block_bytes = bE + bW + bS + bC;
+        p->zero_sort_bytes = bS + bC;
+        p->zero_block_bytes = bE + bW + bS + bC + bG;
         if (!rc) rc = dev_alloc(&p->d_zero_block, p->zero_block_bytes, &b);
         if (!rc) {
           char* base = (char*)p->d_zero_block;
@@ -579,6 +580,7 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
           p->d_virial = (double*)(base + bE);
           p->d_scan_state = (unsigned long long*)(base + bE + bW);
           p->d_count = (int*)(base + bE + bW + bS);
+          p->d_grid = base + bE + bW + bS + bC;
         }
       }
       if (!rc) rc = dev_alloc((void**)&p->d_Ereal, sizeof(double), &b);
@@ -1103,7 +1105,7 @@ int pswf_lr_destroy(pswf_lr_plan* p) {
   if (p->s_comp) cudaStreamDestroy(p->s_comp);
   if (p->s_out) cudaStreamDestroy(p->s_out);
   void* ptrs[] = {p->d_wcoef, p->d_wdcoef,  p->d_kcoef,    p->d_invW2[0], p->d_invW2[1], p->d_invW2[2],
-                  p->d_grid,  p->d_spec,    p->d_zero_block,    
+                  p->d_spec,  p->d_zero_block,
                   p->d_gridi, p->d_rcoef, p->d_rdcoef, p->d_Ereal, p->d_spec2, p->d_spec_dump};
   for (void* q : ptrs)
     if (q) cudaFree(q);
