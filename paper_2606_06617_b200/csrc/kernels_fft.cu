@@ -193,6 +193,21 @@ __device__ __forceinline__ void virial_of_mode(double (&w)[6], double e, double 
     w[3] += g * kx * ky; w[4] += g * kx * kz; w[5] += g * ky * kz;
   }
 }
+// The CTA that finishes last adds the channel energies up (E = sum_c E_c): no separate one-warp kernel between
+// the multiply and the inverse z transform.  `done` counts finished CTAs; it is zeroed with the evaluation's
+// other accumulators.  Called by thread 0 after its atomicAdd into Ech.
+__device__ __forceinline__ void finish_energy(double* Ech, int C, double* E_out, unsigned int* done) {
+  if (E_out == nullptr) return;
+  __threadfence();
+  const unsigned int t = atomicAdd(done, 1u);
+  if (t == gridDim.x * gridDim.y - 1u) {
+    __threadfence();
+    double e = 0.0;
+    for (int c = 0; c < C; ++c) e += atomicAdd(&Ech[c], 0.0);   // (read at L2, where the other CTAs' atomics landed)
+    *E_out = e;
+  }
+}
+
 // block sums of the six components -> Wacc (one atomicAdd per component and CTA); s_red: one double per warp
 __device__ __forceinline__ void virial_reduce(const double (&w)[6], double* s_red, double* Wacc) {
   const int tid = threadIdx.x;
@@ -214,7 +229,7 @@ template <bool DUMP, bool VIR>
 __global__ void __launch_bounds__(kXYThreads, 1)
     k_xy_scale(const XYParams X, const ScaleParams<float> P, const float2* __restrict__ spec_in,
                float2* __restrict__ spec_out, double* __restrict__ Ech, float2* __restrict__ dump,
-               double* __restrict__ Wacc) {
+               double* __restrict__ Wacc, double* __restrict__ E_out, unsigned int* __restrict__ done) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* s = reinterpret_cast<float2*>(smem_raw);                 // [Mx][pitch]
   float2* twx = s + (size_t)X.Mx * X.pitch;                        // [Mx]  exp(-2 pi i k / Mx)
@@ -327,7 +342,10 @@ __global__ void __launch_bounds__(kXYThreads, 1)
   if (tid < 32) {
     double t = tid < kXYThreads / 32 ? s_red[tid] : 0.0;
     t = warp_sum(t);
-    if (tid == 0 && t != 0.0) atomicAdd(&Ech[c], 0.5 * t);
+    if (tid == 0) {
+      if (t != 0.0) atomicAdd(&Ech[c], 0.5 * t);
+      finish_energy(Ech, X.C, E_out, done);
+    }
   }
   if (VIR) virial_reduce(wloc, s_red, Wacc);
 }
@@ -416,7 +434,7 @@ template <int M, bool DUMP, bool VIR>
 __global__ void __launch_bounds__(kXYThreads, 1)
     k_xy_scale_t(const XYParams X, const ScaleParams<float> P, const float2* __restrict__ spec_in,
                  float2* __restrict__ spec_out, double* __restrict__ Ech, float2* __restrict__ dump,
-                 double* __restrict__ Wacc) {
+                 double* __restrict__ Wacc, double* __restrict__ E_out, unsigned int* __restrict__ done) {
   constexpr int pitch = M + 1, NT = kXYThreads, LG = ilog2(M);
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* s = reinterpret_cast<float2*>(smem_raw);                 // [M][pitch]
@@ -525,7 +543,10 @@ __global__ void __launch_bounds__(kXYThreads, 1)
   if (tid < 32) {
     double t = tid < NT / 32 ? s_red[tid] : 0.0;
     t = warp_sum(t);
-    if (tid == 0 && t != 0.0) atomicAdd(&Ech[c], 0.5 * t);
+    if (tid == 0) {
+      if (t != 0.0) atomicAdd(&Ech[c], 0.5 * t);
+      finish_energy(Ech, X.C, E_out, done);
+    }
   }
   if (VIR) virial_reduce(wloc, s_red, Wacc);
 }
@@ -725,7 +746,7 @@ void fused_fft_limits(const pswf_lr_plan* p, int kmax[3]) {
 }
 
 // forward z transform (cuFFT, plane-major output) must already be in p->d_spec; writes p->d_spec2
-void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t st) {
+void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, double* E, cudaStream_t st) {
   XYParams X;
   X.Mx = p->M[0]; X.My = p->M[1]; X.pitch = p->M[1] + 1; X.C = p->C;
   X.nrx = factor_radices(X.Mx, X.rx);
@@ -746,7 +767,7 @@ void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t 
   do {                                                                                                       \
     cudaFuncSetAttribute(KERN, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);                        \
     KERN<<<grid, kXYThreads, sm, st>>>(X, P, (const float2*)p->d_spec, (float2*)p->d_spec2, p->d_Ech, dump, \
-                                       wacc);                                                                \
+                                       wacc, E, p->d_done);                                                  \
   } while (0)
 #define PSWF_XY_SQ(MV)                                                  \
   case MV:                                                              \

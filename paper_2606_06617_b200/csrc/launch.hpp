@@ -32,7 +32,7 @@ void launch_stencil_spread(pswf_lr_plan* p, int n, cudaStream_t st);
 // band-limited transform path (kernels_fft.cu)
 bool fused_fft_supported(const pswf_lr_plan* p);
 void fused_fft_limits(const pswf_lr_plan* p, int kmax[3]);
-void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, cudaStream_t st);
+void launch_xy_scale(pswf_lr_plan* p, const ScaleParams<float>& P, double* E, cudaStream_t st);   // E (device, may be NULL): total energy
 bool fused_z_supported(const pswf_lr_plan* p);   // own z transforms (power-of-two Mz); else cuFFT along z
 void launch_z_forward(pswf_lr_plan* p, cudaStream_t st);
 void launch_z_inverse(pswf_lr_plan* p, cudaStream_t st);

@@ -136,6 +136,7 @@ struct pswf_lr_plan {
   // (the sort of pswf_lr_execute_real zeroes d_scan_state and d_count only: the energies and the potential grid
   // of the preceding execute stay readable)
   void* d_zero_block = nullptr;
+  unsigned int* d_done = nullptr;   // finished CTAs of the fused multiply kernel (last one sums the energies)
   size_t zero_block_bytes = 0, zero_sort_offset = 0, zero_sort_bytes = 0;
   double* d_Ech = nullptr;        // [C]
   // per-atom workspaces (capacity cap_atoms)

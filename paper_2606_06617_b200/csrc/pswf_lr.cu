@@ -242,10 +242,12 @@ int execute_t(pswf_lr_plan* p, int n, const T* pos, const T* q, double* E, T* ph
   // a3
   // (d_Ech and d_virial were zeroed with the sort's buffers at the start of the evaluation)
   if constexpr (kIsF32) {
-    if (fused) launch_xy_scale(p, P, st);
+    if (fused) launch_xy_scale(p, P, E, st);   // (its last CTA writes E)
   }
-  if (!fused) launch_scale<T>(p, P, true, st);
-  if (E) launch_finalize_energy(p, E, st);
+  if (!fused) {
+    launch_scale<T>(p, P, true, st);
+    if (E) launch_finalize_energy(p, E, st);
+  }
   if (ev) cudaEventRecord(ev[4], st);
   if (phi || F) {
     // a4
@@ -578,6 +580,7 @@ int pswf_lr_plan_create_cell(pswf_lr_plan** plan, const double cell[9], const in
           char* base = (char*)p->d_zero_block;
           p->d_Ech = (double*)base;
           p->d_virial = (double*)(base + bE);
+          p->d_done = (unsigned int*)(base + bE + 7 * sizeof(double));
           p->d_scan_state = (unsigned long long*)(base + bE + bW);
           p->d_count = (int*)(base + bE + bW + bS);
           p->d_grid = base + bE + bW + bS + bC;
