@@ -561,11 +561,15 @@ __global__ void __launch_bounds__(kXYThreads, 1)
 constexpr int kZThreads = 256;
 constexpr int kZTile = 32;   // real pencils per CTA
 
+// real pencils per CTA of the forward transform: 64 (32 complex pencils: the radix-16 pass then has one butterfly
+// per thread) while the tile fits 48 KB of static shared memory
+__host__ __device__ constexpr int z_tile_fwd(int NZ) { return NZ > 128 ? 32 : 64; }
+
 template <int NZ>
 __global__ void __launch_bounds__(kZThreads)
     k_z_forward(int C, int Mx, int My, int YT, int kmaxz, const float* __restrict__ grid, float2* __restrict__ spec) {
   constexpr int pitch = NZ + 1, NT = kZThreads;
-  __shared__ __align__(16) float2 s[(kZTile / 2) * pitch];
+  __shared__ __align__(16) float2 s[(z_tile_fwd(NZ) / 2) * pitch];
   __shared__ float2 tw[NZ];
   __shared__ short pos_of[NZ];
   const int tid = threadIdx.x;
@@ -807,7 +811,9 @@ int z_tile(int My) {
 }  // namespace
 
 void launch_z_forward(pswf_lr_plan* p, cudaStream_t st) {
-  const int C = p->C, Mx = p->M[0], My = p->M[1], YT = z_tile(My);
+  const int C = p->C, Mx = p->M[0], My = p->M[1];
+  int YT = std::min(z_tile_fwd(p->M[2]), My);
+  while (My % YT) YT >>= 1;
   const unsigned nb = (unsigned)(C * Mx * (My / YT));
   p->n_kernels += 1;
 #define PSWF_ZF(NZ) \
