@@ -467,11 +467,25 @@ __global__ void __launch_bounds__(kXYThreads, 1)
   const size_t plane = ((size_t)kz * X.C + c) * M * M;
   {
     const float4* src = reinterpret_cast<const float4*>(spec_in + plane);   // two complex per load
-    for (int i = tid; i < M * M / 2; i += NT) {
-      const int x = i >> (LG - 1), y = (i & (M / 2 - 1)) * 2;
-      const float4 t = __ldg(src + i);
-      s[x * pitch + y] = make_float2(t.x, t.y);
-      s[x * pitch + y + 1] = make_float2(t.z, t.w);
+    // all of a thread's loads in flight before the first store (the plane comes from L2 / HBM: one round trip
+    // instead of one per element pair)
+    constexpr int kPer = (M * M / 2 + NT - 1) / NT, kBatch = kPer < 8 ? kPer : 8;
+    for (int i0 = tid; i0 < M * M / 2; i0 += NT * kBatch) {
+      float4 t[kBatch];
+#pragma unroll
+      for (int u = 0; u < kBatch; ++u) {
+        const int i = i0 + u * NT;
+        t[u] = i < M * M / 2 ? __ldg(src + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int u = 0; u < kBatch; ++u) {
+        const int i = i0 + u * NT;
+        if (i < M * M / 2) {
+          const int x = i >> (LG - 1), y = (i & (M / 2 - 1)) * 2;
+          s[x * pitch + y] = make_float2(t[u].x, t[u].y);
+          s[x * pitch + y + 1] = make_float2(t[u].z, t[u].w);
+        }
+      }
     }
   }
   __syncthreads();
